@@ -1,0 +1,189 @@
+/*
+ * e2e.h -- C ABI of libe2e: B200-native echellogram rendering (sm_100a).
+ *
+ * The one data-parallel hot path of the end-to-end spectrograph simulator of Genoni, Landoni et al.
+ * (arXiv 2008.05858; PAPER.md, cited as P:line): the Image Simulation Module,
+ *
+ *     "The final image of the echellogram is obtained as a superposition of individual spectral
+ *      images of the fiber sampled on a proper wavelength grid.  Those are estimated as a surface
+ *      integral of the convolution between the spatial profile of the fiber and the PSF ..."
+ *
+ *   frame[j][i] = sum_f sum_m sum_k  w_{f,m,k} * P(i - x_{f,m,k}, j - y_{f,m,k})
+ *
+ * over fibers f, echelle orders m and oversampled wavelength samples k.  Steps (the
+ * readings of the paper they rest on are listed in DESIGN.md):
+ *   a1  lam_k = lam_min + (k + 1/2) dlam,  N_m = ceil(samples_per_px * |x(lam_max) - x(lam_min)|)
+ *   a2  w_k   = scale_f * S_f(lam_k / doppler_f) * E_m(lam_k) * T(lam_k) * dlam
+ *   a3  (x_k, y_k) = spectral-format polynomials in (lam, m) + per-fiber offset
+ *   a4  P = pixel-integrated (fiber image (x) optical PSF), analytic or tabulated
+ *   a5  accumulate into the fp64 frame
+ *   a6  optional detector stage: Poisson photon noise + gaussian read noise
+ *
+ * Conventions: pixel (i, j) = column i (x, main dispersion), row j (y, cross dispersion); it covers
+ * [i-1/2, i+1/2) x [j-1/2, j+1/2); frames are row-major, frame[j*nx + i], fp64.
+ *
+ * Every function returns 0 (E2E_OK) or a negative error code; e2e_last_error() gives a message for
+ * the last failing call of the calling thread.  Nothing aborts, throws or prints.  Pointers are HOST
+ * pointers unless the name starts with d_ (DEVICE pointer, same CUDA device as the handles).
+ * There is no CPU fallback: without a CUDA device every call that needs one returns E2E_ERR_CUDA.
+ */
+#ifndef E2E_H
+#define E2E_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define E2E_API __attribute__((visibility("default")))
+#else
+#define E2E_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    E2E_OK = 0,
+    E2E_ERR_INVALID_ARG = -1,    /* NULL pointer, bad shape, NaN, negative sigma ... */
+    E2E_ERR_NOT_MONOTONIC = -2,  /* x(lam) is not strictly monotone inside an order */
+    E2E_ERR_CUDA = -3,           /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+    E2E_ERR_NOMEM = -4,
+    E2E_ERR_UNSUPPORTED = -5,    /* valid input outside what the kernels handle (limits below) */
+    E2E_ERR_WORKSPACE = -6       /* workspace pointer NULL / misaligned / too small */
+};
+
+/* message for the last failing call of this thread ("" if none); pointer valid until the next call */
+E2E_API const char* e2e_last_error(void);
+/* library version string, e.g. "e2e-b200 0.1 sm_100a" */
+E2E_API const char* e2e_version(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * Spectral format + efficiency ("spectral format data", P:165 blaze and throughput)
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct e2e_format e2e_format_t; /* opaque; immutable after create */
+
+typedef struct {
+    int32_t nx, ny;                 /* detector size in pixels */
+    int32_t n_orders;
+    const int32_t* order_m;         /* [n_orders] echelle order numbers m */
+    const double* lam_min;          /* [n_orders] wavelength range rendered per order, lam_min < lam_max */
+    const double* lam_max;
+    int32_t n_fibers;
+    const double* fiber_dx;         /* [n_fibers] offsets of each fiber image in px */
+    const double* fiber_dy;
+    int32_t deg_l, deg_m;           /* tensor degree of the format polynomials, each 0..5 */
+    const double* coef_x;           /* [(deg_l+1)*(deg_m+1)], c[p*(deg_m+1)+q] multiplies L^p M^q */
+    const double* coef_y;
+    double lam0, inv_dlam;          /* L = (lam - lam0) * inv_dlam */
+    double m0, inv_dm;              /* M = (m - m0) * inv_dm */
+    const double* blaze_lam_c;      /* [n_orders] blaze wavelength: E = amp * sinc^2(pi m (lam_c/lam - 1)) */
+    const double* blaze_amp;        /* [n_orders] or NULL (= 1) */
+    const double* eff_table;        /* optional common throughput T(lam) on a uniform grid, linear interp; NULL = 1 */
+    int64_t eff_n;
+    double eff_lam0, eff_dlam;
+    double samples_per_px;          /* wavelength samples per pixel of dispersion */
+} e2e_format_desc_t;
+
+/* Copies everything (caller keeps ownership of the arrays).  Evaluates every sample position once on the
+ * device to (i) check that x(lam_k) is strictly monotone in k inside each order, (ii) record the smallest
+ * sample spacing and the row range of each order per 64-column bin (used to schedule renders without atomics).
+ * Polynomial evaluation is the fixed fma-Horner sequence of DESIGN.md "O2" (inner over q=deg_m..0 in M,
+ * outer over p=deg_l..0 in L), bit-identical on host and device. */
+E2E_API int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* desc);
+E2E_API void e2e_format_destroy(e2e_format_t* fmt);
+
+/* number of wavelength samples: per order (same for every fiber) into n_per_order[n_orders] (may be NULL),
+ * and the total over orders AND fibers into *n_total (may be NULL) */
+E2E_API int e2e_format_num_samples(const e2e_format_t* fmt, int64_t* n_per_order, int64_t* n_total);
+
+/* ------------------------------------------------------------------------------------------------
+ * Instrument PSF = fiber image (x) optical PSF
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct e2e_psf e2e_psf_t; /* opaque; immutable after create */
+
+typedef struct {
+    int32_t kind;                   /* 0 analytic: uniform ellipse (x) axis-aligned gaussian; 1 tabulated */
+    double fiber_dx_px, fiber_dy_px;/* kind 0: full widths of the fiber image, main / cross dispersion; 0,0 = pure gaussian */
+    double sigma_x, sigma_y;        /* kind 0: optical PSF sigmas in px ("asymmetric Gaussian"), > 0 */
+    double support_nsigma;          /* kind 0: t of the footprint rule H = D/2 + t*sigma (G9); <= 0 selects 7.5 */
+    int32_t n_nodes;                /* kind 0: chord-quadrature nodes Q; 0 = chosen from D/sigma so that the
+                                       quadrature error is < 1e-12 of the PSF peak */
+    int32_t tab_npix, tab_os;       /* kind 1: kernel size in px (e.g. 11) and cells per px (e.g. 8) */
+    int32_t tab_gx, tab_gy;         /* kind 1: field grid of kernels across the detector (e.g. 5 x 5), each >= 1 */
+    const double* tab;              /* kind 1: [gy][gx][npix*os][npix*os] cell values, every kernel sums to 1 */
+} e2e_psf_desc_t;
+
+/* Limits (E2E_ERR_UNSUPPORTED beyond them): footprint (2H+2) <= 96 px per axis; Q <= 64; tab_npix*tab_os <= 256. */
+E2E_API int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* desc, int32_t nx, int32_t ny);
+E2E_API void e2e_psf_destroy(e2e_psf_t* psf);
+
+/* ------------------------------------------------------------------------------------------------
+ * Rendering (a1-a5)
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    const double* d_flux;           /* DEVICE (or HOST for the *_host entry point) photon-flux table, uniform grid */
+    int64_t n;                      /* table length, >= 2 */
+    double lam0, dlam;              /* wavelength of flux[0], grid step > 0 */
+    double scale;                   /* per-fiber illumination factor */
+    double doppler;                 /* 1 + v/c: the fiber sees S(lam / doppler) */
+} e2e_spectrum_t;
+
+/* bytes of device scratch e2e_render_frame needs for this (format, psf): the per-sample arrays x, y, w of
+ * step a1-a3 (24 B per sample) plus the schedule.  256-byte aligned workspace required. */
+E2E_API int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, size_t* bytes);
+
+/* a1-a3 only, for one (fiber, order): writes lam, x, y, w of its samples to DEVICE arrays of length
+ * `capacity` >= that order's sample count (any of the four may be NULL).  Asynchronous on cuda_stream. */
+E2E_API int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spectrum, int32_t fiber, int32_t order_index,
+                      double* d_lam, double* d_x, double* d_y, double* d_w, int64_t capacity, void* cuda_stream);
+
+/* a1-a5.  spectra: HOST array [n_fibers] whose d_flux members are DEVICE pointers.  d_frame: DEVICE
+ * [ny*nx] fp64 row-major; accumulate = 0 overwrites it (it is zero-filled first), 1 adds to it.
+ * Deterministic: the same inputs give the same bits; no atomics are used.  Asynchronous on cuda_stream
+ * (a cudaStream_t, NULL = default stream); launch errors are returned, later device faults surface at the
+ * caller's next synchronisation.  The call allocates nothing on the device except, the first time a
+ * (format, psf) pair is seen, the cached schedule (a few hundred KB). */
+E2E_API int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                     double* d_frame, int32_t accumulate, void* d_workspace, size_t workspace_bytes,
+                     void* cuda_stream);
+
+/* Same as e2e_render_frame with HOST buffers: spectra[f].d_flux are HOST pointers and h_frame is a HOST
+ * [ny*nx] array (pinned memory gives full PCIe speed).  The call copies the tables to the device, renders,
+ * copies the frame back and synchronises the stream before returning.  Device scratch is taken from
+ * d_workspace, which must hold e2e_render_host_workspace_bytes() bytes. */
+E2E_API int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                                    size_t* bytes);
+E2E_API int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                          double* h_frame, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Detector stage (a6; "photon noise and all other specific detector noises ... are added on the
+ * final synthetic echellogram").  out[p] = (Poisson(max(0, gain*in[p] + dark_e)) + bias) + ron_e * N(0,1),
+ * drawn from a Philox4x32-10 stream keyed by (seed, pixel index p = j*nx + i): the result does not depend
+ * on launch geometry and is reproducible bit for bit (algorithm: DESIGN.md G12).
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    double gain, dark_e, ron_e, bias;
+    uint64_t seed;
+} e2e_detector_t;
+
+/* d_frame_in / d_frame_out: DEVICE [ny*nx]; may be the same pointer.  Asynchronous on cuda_stream. */
+E2E_API int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny,
+                       const e2e_detector_t* det, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Measurement helpers (used by bench.py; not part of the rendering path)
+ * ------------------------------------------------------------------------------------------------ */
+/* Runs an all-SM kernel of independent DFMA chains `repeats` times and returns the best sustained rate in
+ * *dfma_per_s (fused multiply-adds per second; flop/s = 2x) and the kernel time of that run in *ms.
+ * Synchronous. */
+E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* dfma_per_s, double* ms);
+
+/* Number of kernel launches the library has issued since load (all entry points), for bench.py's gpu_launches. */
+E2E_API int64_t e2e_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* E2E_H */

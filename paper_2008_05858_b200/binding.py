@@ -1,0 +1,323 @@
+"""ctypes binding of ``libe2e.so`` (``include/e2e.h``): argument marshalling only.
+
+Same names as the C entry points.  Every step of the hot path runs in the CUDA kernels of the library;
+PyTorch supplies device memory (``torch.empty(..., device="cuda")``) and streams, nothing else.  There is
+no CPU fallback: if the library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libe2e.so"
+
+E2E_OK = 0
+ERROR_NAMES = {-1: "E2E_ERR_INVALID_ARG", -2: "E2E_ERR_NOT_MONOTONIC", -3: "E2E_ERR_CUDA", -4: "E2E_ERR_NOMEM",
+               -5: "E2E_ERR_UNSUPPORTED", -6: "E2E_ERR_WORKSPACE"}
+
+# every symbol include/e2e.h declares (tests/test_abi.py checks the header against this list and the .so)
+SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_destroy", "e2e_format_num_samples",
+           "e2e_psf_create", "e2e_psf_destroy", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
+           "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_measure_fp64_peak",
+           "e2e_launch_count"]
+
+
+class E2EError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{ERROR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class FormatDesc(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("n_orders", C.c_int32), ("order_m", C.c_void_p),
+                ("lam_min", C.c_void_p), ("lam_max", C.c_void_p), ("n_fibers", C.c_int32),
+                ("fiber_dx", C.c_void_p), ("fiber_dy", C.c_void_p), ("deg_l", C.c_int32), ("deg_m", C.c_int32),
+                ("coef_x", C.c_void_p), ("coef_y", C.c_void_p), ("lam0", C.c_double), ("inv_dlam", C.c_double),
+                ("m0", C.c_double), ("inv_dm", C.c_double), ("blaze_lam_c", C.c_void_p), ("blaze_amp", C.c_void_p),
+                ("eff_table", C.c_void_p), ("eff_n", C.c_int64), ("eff_lam0", C.c_double), ("eff_dlam", C.c_double),
+                ("samples_per_px", C.c_double)]
+
+
+class PsfDesc(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("fiber_dx_px", C.c_double), ("fiber_dy_px", C.c_double),
+                ("sigma_x", C.c_double), ("sigma_y", C.c_double), ("support_nsigma", C.c_double),
+                ("n_nodes", C.c_int32), ("tab_npix", C.c_int32), ("tab_os", C.c_int32), ("tab_gx", C.c_int32),
+                ("tab_gy", C.c_int32), ("tab", C.c_void_p)]
+
+
+class SpectrumDesc(C.Structure):
+    _fields_ = [("d_flux", C.c_void_p), ("n", C.c_int64), ("lam0", C.c_double), ("dlam", C.c_double),
+                ("scale", C.c_double), ("doppler", C.c_double)]
+
+
+class DetectorDesc(C.Structure):
+    _fields_ = [("gain", C.c_double), ("dark_e", C.c_double), ("ron_e", C.c_double), ("bias", C.c_double),
+                ("seed", C.c_uint64)]
+
+
+_lib = None
+
+
+def load():
+    """dlopen libe2e.so (built in-tree by ``paper_2008_05858_b200.build``); raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2008_05858_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.e2e_last_error.restype = C.c_char_p
+    L.e2e_last_error.argtypes = []
+    L.e2e_version.restype = C.c_char_p
+    L.e2e_version.argtypes = []
+    L.e2e_format_create.restype = C.c_int
+    L.e2e_format_create.argtypes = [C.POINTER(vp), C.POINTER(FormatDesc)]
+    L.e2e_format_destroy.restype = None
+    L.e2e_format_destroy.argtypes = [vp]
+    L.e2e_format_num_samples.restype = C.c_int
+    L.e2e_format_num_samples.argtypes = [vp, vp, C.POINTER(i64)]
+    L.e2e_psf_create.restype = C.c_int
+    L.e2e_psf_create.argtypes = [C.POINTER(vp), C.POINTER(PsfDesc), i32, i32]
+    L.e2e_psf_destroy.restype = None
+    L.e2e_psf_destroy.argtypes = [vp]
+    L.e2e_render_workspace_bytes.restype = C.c_int
+    L.e2e_render_workspace_bytes.argtypes = [vp, vp, C.POINTER(C.c_size_t)]
+    L.e2e_setup_samples.restype = C.c_int
+    L.e2e_setup_samples.argtypes = [vp, C.POINTER(SpectrumDesc), i32, i32, vp, vp, vp, vp, i64, vp]
+    L.e2e_render_frame.restype = C.c_int
+    L.e2e_render_frame.argtypes = [vp, vp, C.POINTER(SpectrumDesc), vp, i32, vp, C.c_size_t, vp]
+    L.e2e_render_host_workspace_bytes.restype = C.c_int
+    L.e2e_render_host_workspace_bytes.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(C.c_size_t)]
+    L.e2e_render_frame_host.restype = C.c_int
+    L.e2e_render_frame_host.argtypes = [vp, vp, C.POINTER(SpectrumDesc), vp, vp, C.c_size_t, vp]
+    L.e2e_apply_detector.restype = C.c_int
+    L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
+    L.e2e_measure_fp64_peak.restype = C.c_int
+    L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
+    L.e2e_launch_count.restype = i64
+    L.e2e_launch_count.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != E2E_OK:
+        raise E2EError(rc, load().e2e_last_error().decode())
+
+
+def e2e_version() -> str:
+    return load().e2e_version().decode()
+
+
+def e2e_last_error() -> str:
+    return load().e2e_last_error().decode()
+
+
+def e2e_launch_count() -> int:
+    return int(load().e2e_launch_count())
+
+
+def _host(a, dt=np.float64):
+    return np.ascontiguousarray(np.asarray(a, dtype=dt))
+
+
+class Format:
+    """Owns an ``e2e_format_t*``.  Built from a scene-like object (see ``workloads.Scene``)."""
+
+    def __init__(self, scene):
+        s = scene
+        keep = []
+
+        def k(a, dt=np.float64):
+            a = _host(a, dt)
+            keep.append(a)
+            return a.ctypes.data
+
+        d = FormatDesc()
+        d.nx, d.ny = int(s.nx), int(s.ny)
+        d.n_orders = int(np.asarray(s.order_m).shape[0])
+        d.order_m = k(s.order_m, np.int32)
+        d.lam_min, d.lam_max = k(s.lam_min), k(s.lam_max)
+        d.n_fibers = int(np.asarray(s.fiber_dx).shape[0])
+        d.fiber_dx, d.fiber_dy = k(s.fiber_dx), k(s.fiber_dy)
+        d.deg_l, d.deg_m = int(s.deg_l), int(s.deg_m)
+        d.coef_x, d.coef_y = k(s.coef_x), k(s.coef_y)
+        d.lam0, d.inv_dlam, d.m0, d.inv_dm = float(s.lam0), float(s.inv_dlam), float(s.m0), float(s.inv_dm)
+        d.blaze_lam_c = k(s.blaze_lam_c)
+        d.blaze_amp = k(s.blaze_amp) if getattr(s, "blaze_amp", None) is not None else None
+        if getattr(s, "eff_table", None) is not None:
+            d.eff_table = k(s.eff_table)
+            d.eff_n = int(np.asarray(s.eff_table).shape[0])
+            d.eff_lam0, d.eff_dlam = float(s.eff_lam0), float(s.eff_dlam)
+        else:
+            d.eff_table, d.eff_n, d.eff_lam0, d.eff_dlam = None, 0, 0.0, 1.0
+        d.samples_per_px = float(s.samples_per_px)
+        self.nx, self.ny, self.n_orders, self.n_fibers = d.nx, d.ny, d.n_orders, d.n_fibers
+        self.handle = C.c_void_p()
+        _check(load().e2e_format_create(C.byref(self.handle), C.byref(d)))
+
+    def num_samples(self):
+        per = np.zeros(self.n_orders, dtype=np.int64)
+        tot = C.c_int64()
+        _check(load().e2e_format_num_samples(self.handle, per.ctypes.data, C.byref(tot)))
+        return per, int(tot.value)
+
+    def close(self):
+        if getattr(self, "handle", None) is not None and self.handle.value:
+            load().e2e_format_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Psf:
+    """Owns an ``e2e_psf_t*``.  ``psf`` is a ``workloads.Psf``-like object."""
+
+    def __init__(self, psf, nx: int, ny: int):
+        d = PsfDesc()
+        d.kind = int(psf.kind)
+        d.fiber_dx_px, d.fiber_dy_px = float(psf.fiber_dx_px), float(psf.fiber_dy_px)
+        d.sigma_x, d.sigma_y = float(psf.sigma_x), float(psf.sigma_y)
+        d.support_nsigma = float(psf.support_nsigma)
+        d.n_nodes = int(psf.n_nodes)
+        d.tab_npix, d.tab_os, d.tab_gx, d.tab_gy = int(psf.tab_npix), int(psf.tab_os), int(psf.tab_gx), int(psf.tab_gy)
+        tab = _host(psf.tab) if psf.tab is not None else None
+        d.tab = tab.ctypes.data if tab is not None else None
+        self.handle = C.c_void_p()
+        _check(load().e2e_psf_create(C.byref(self.handle), C.byref(d), int(nx), int(ny)))
+
+    def close(self):
+        if getattr(self, "handle", None) is not None and self.handle.value:
+            load().e2e_psf_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def e2e_format_create(scene) -> Format:
+    return Format(scene)
+
+
+def e2e_psf_create(psf, nx: int, ny: int) -> Psf:
+    return Psf(psf, nx, ny)
+
+
+def spectra_array(spectra: Sequence, flux_ptrs: Sequence[int]):
+    """``e2e_spectrum_t[n_fibers]`` from ``workloads.Spectrum``-like objects and the addresses of their tables."""
+    arr = (SpectrumDesc * len(spectra))()
+    for i, (sp, ptr) in enumerate(zip(spectra, flux_ptrs)):
+        arr[i].d_flux = int(ptr)
+        arr[i].n = int(np.asarray(sp.flux).shape[0]) if not hasattr(sp.flux, "numel") else int(sp.flux.numel())
+        arr[i].lam0, arr[i].dlam, arr[i].scale, arr[i].doppler = float(sp.lam0), float(sp.dlam), float(sp.scale), float(sp.doppler)
+    return arr
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def e2e_render_workspace_bytes(fmt: Format, psf: Psf) -> int:
+    n = C.c_size_t()
+    _check(load().e2e_render_workspace_bytes(fmt.handle, psf.handle, C.byref(n)))
+    return int(n.value)
+
+
+def e2e_setup_samples(fmt: Format, spectrum_desc, fiber: int, order_index: int, d_lam, d_x, d_y, d_w, capacity: int,
+                      stream=None):
+    def p(t):
+        return None if t is None else int(t.data_ptr())
+    _check(load().e2e_setup_samples(fmt.handle, C.byref(spectrum_desc), fiber, order_index, p(d_lam), p(d_x), p(d_y),
+                                    p(d_w), int(capacity), _stream_ptr(stream)))
+
+
+def e2e_render_frame(fmt: Format, psf: Psf, spectra_desc, d_frame, accumulate: bool, d_workspace, stream=None):
+    """d_frame: float64 CUDA tensor [ny, nx]; d_workspace: uint8 CUDA tensor of e2e_render_workspace_bytes bytes."""
+    _check(load().e2e_render_frame(fmt.handle, psf.handle, spectra_desc, int(d_frame.data_ptr()), int(bool(accumulate)),
+                                   int(d_workspace.data_ptr()), int(d_workspace.numel() * d_workspace.element_size()),
+                                   _stream_ptr(stream)))
+
+
+def e2e_render_host_workspace_bytes(fmt: Format, psf: Psf, spectra_desc) -> int:
+    n = C.c_size_t()
+    _check(load().e2e_render_host_workspace_bytes(fmt.handle, psf.handle, spectra_desc, C.byref(n)))
+    return int(n.value)
+
+
+def e2e_render_frame_host(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: int, d_workspace, stream=None):
+    _check(load().e2e_render_frame_host(fmt.handle, psf.handle, spectra_desc, int(h_frame_ptr), int(d_workspace.data_ptr()),
+                                        int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
+
+
+def e2e_apply_detector(d_in, d_out, nx: int, ny: int, det, stream=None):
+    d = DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed))
+    _check(load().e2e_apply_detector(int(d_in.data_ptr()), int(d_out.data_ptr()), int(nx), int(ny), C.byref(d),
+                                     _stream_ptr(stream)))
+
+
+def e2e_measure_fp64_peak(repeats: int = 5):
+    rate, ms = C.c_double(), C.c_double()
+    _check(load().e2e_measure_fp64_peak(int(repeats), C.byref(rate), C.byref(ms)))
+    return float(rate.value), float(ms.value)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# convenience on top of the calls above (still marshalling only): a scene rendered with torch-owned buffers
+# ---------------------------------------------------------------------------------------------------------
+class Renderer:
+    """Holds the handles, the device copies of the spectra and the workspace of one scene."""
+
+    def __init__(self, scene, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.scene = scene
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.fmt = Format(scene)
+        self.psf = Psf(scene.psf, scene.nx, scene.ny)
+        self.flux = [torch.from_numpy(_host(sp.flux)).to(self.device) for sp in scene.spectra]
+        self.spectra = spectra_array(scene.spectra, [t.data_ptr() for t in self.flux])
+        nbytes = e2e_render_workspace_bytes(self.fmt, self.psf)
+        self.workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        self.per_order, self.n_samples = self.fmt.num_samples()
+
+    def render(self, frame=None, accumulate=False, stream=None):
+        torch = self.torch
+        if frame is None:
+            frame = torch.empty((self.scene.ny, self.scene.nx), dtype=torch.float64, device=self.device)
+        e2e_render_frame(self.fmt, self.psf, self.spectra, frame, accumulate, self.workspace, stream)
+        return frame
+
+    def samples(self, fiber: int, order_index: int):
+        torch = self.torch
+        n = int(self.per_order[order_index])
+        out = [torch.empty(max(n, 1), dtype=torch.float64, device=self.device) for _ in range(4)]
+        e2e_setup_samples(self.fmt, self.spectra[fiber], fiber, order_index, *out, capacity=max(n, 1))
+        torch.cuda.synchronize()
+        return tuple(o[:n].cpu().numpy() for o in out)
+
+    def detector(self, frame, det=None, out=None, stream=None):
+        det = det if det is not None else self.scene.detector
+        out = out if out is not None else self.torch.empty_like(frame)
+        e2e_apply_detector(frame, out, self.scene.nx, self.scene.ny, det, stream)
+        return out
+
+    def close(self):
+        self.psf.close()
+        self.fmt.close()

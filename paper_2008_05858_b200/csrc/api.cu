@@ -1,0 +1,661 @@
+// api.cu -- the C ABI of include/e2e.h: handle creation / validation, the host-side schedule, kernel launches.
+#include "common.cuh"
+#include "setup.cuh"
+#include "render_analytic.cuh"
+#include "render_tabulated.cuh"
+
+#include <algorithm>
+#include <cstring>
+#include <cmath>
+
+namespace e2e {
+
+// ------------------------------------------------------------------------------------------------
+// error plumbing
+// ------------------------------------------------------------------------------------------------
+static thread_local std::string t_error;
+std::atomic<long long> g_launches{0};
+
+void set_error(const std::string& msg) { t_error = msg; }
+int fail(int code, const std::string& msg) { t_error = msg; return code; }
+int fail_cuda(cudaError_t e, const char* what)
+{
+    t_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return E2E_ERR_CUDA;
+}
+
+int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream);
+int measure_fp64_peak(int repeats, double* dfma_per_s, double* ms_out);
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static inline bool is_fin(double v) { return std::isfinite(v); }
+
+// host copy of sample_position's x (same operation sequence: O1, O2)
+static double host_x_of_lambda(const e2e_format_desc_t& d, int o, double lam)
+{
+    double L = (lam - d.lam0) * d.inv_dlam;
+    double M = ((double)d.order_m[o] - d.m0) * d.inv_dm;
+    return poly2(d.coef_x, d.deg_l, d.deg_m, L, M);
+}
+
+}  // namespace e2e
+
+using namespace e2e;
+
+e2e_plan::~e2e_plan()
+{
+    if (d_strips) cudaFree(d_strips);
+    if (d_items) cudaFree(d_items);
+}
+
+extern "C" {
+
+const char* e2e_last_error(void) { return t_error.c_str(); }
+const char* e2e_version(void) { return "e2e-b200 0.1 sm_100a"; }
+int64_t e2e_launch_count(void) { return (int64_t)g_launches.load(); }
+
+// ================================================================================================
+// format
+// ================================================================================================
+int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* d)
+{
+    if (!out) return fail(E2E_ERR_INVALID_ARG, "format_create: out is NULL");
+    *out = nullptr;
+    if (!d) return fail(E2E_ERR_INVALID_ARG, "format_create: desc is NULL");
+    if (d->nx <= 0 || d->ny <= 0 || d->nx > (1 << 20) || d->ny > (1 << 20))
+        return fail(E2E_ERR_INVALID_ARG, "format_create: bad detector size");
+    if (d->n_orders <= 0 || d->n_orders > 4096) return fail(E2E_ERR_INVALID_ARG, "format_create: n_orders out of range");
+    if (d->n_fibers <= 0) return fail(E2E_ERR_INVALID_ARG, "format_create: n_fibers must be >= 1");
+    if (d->n_fibers > kMaxFibers) return fail(E2E_ERR_UNSUPPORTED, "format_create: more than 64 fibers");
+    if (d->deg_l < 0 || d->deg_l > kMaxDeg || d->deg_m < 0 || d->deg_m > kMaxDeg)
+        return fail(E2E_ERR_INVALID_ARG, "format_create: polynomial degree must be 0..5");
+    if (!d->order_m || !d->lam_min || !d->lam_max || !d->fiber_dx || !d->fiber_dy || !d->coef_x || !d->coef_y ||
+        !d->blaze_lam_c)
+        return fail(E2E_ERR_INVALID_ARG, "format_create: NULL array");
+    if (!(d->samples_per_px > 0.0) || !is_fin(d->samples_per_px))
+        return fail(E2E_ERR_INVALID_ARG, "format_create: samples_per_px must be > 0");
+    if (!is_fin(d->lam0) || !is_fin(d->inv_dlam) || !is_fin(d->m0) || !is_fin(d->inv_dm))
+        return fail(E2E_ERR_INVALID_ARG, "format_create: non-finite normalisation");
+    const int nc = (d->deg_l + 1) * (d->deg_m + 1);
+    for (int i = 0; i < nc; ++i)
+        if (!is_fin(d->coef_x[i]) || !is_fin(d->coef_y[i])) return fail(E2E_ERR_INVALID_ARG, "format_create: non-finite coefficient");
+    for (int o = 0; o < d->n_orders; ++o) {
+        if (!is_fin(d->lam_min[o]) || !is_fin(d->lam_max[o]) || !(d->lam_min[o] < d->lam_max[o]))
+            return fail(E2E_ERR_INVALID_ARG, "format_create: need lam_min < lam_max for every order");
+        if (!is_fin(d->blaze_lam_c[o]) || (d->blaze_amp && !is_fin(d->blaze_amp[o])))
+            return fail(E2E_ERR_INVALID_ARG, "format_create: non-finite blaze parameter");
+    }
+    for (int f = 0; f < d->n_fibers; ++f)
+        if (!is_fin(d->fiber_dx[f]) || !is_fin(d->fiber_dy[f])) return fail(E2E_ERR_INVALID_ARG, "format_create: non-finite fiber offset");
+    if (d->eff_table && (d->eff_n < 2 || !(d->eff_dlam > 0.0) || !is_fin(d->eff_lam0)))
+        return fail(E2E_ERR_INVALID_ARG, "format_create: bad efficiency table");
+
+    std::unique_ptr<e2e_format> F(new (std::nothrow) e2e_format);
+    if (!F) return fail(E2E_ERR_NOMEM, "format_create: out of host memory");
+    const int no = d->n_orders, nf = d->n_fibers;
+    F->order_m.assign(d->order_m, d->order_m + no);
+    F->lam_min.assign(d->lam_min, d->lam_min + no);
+    F->lam_max.assign(d->lam_max, d->lam_max + no);
+    F->fiber_dx.assign(d->fiber_dx, d->fiber_dx + nf);
+    F->fiber_dy.assign(d->fiber_dy, d->fiber_dy + nf);
+    F->samples_per_px = d->samples_per_px;
+    F->dl.resize(no);
+    F->nsamp.resize(no);
+    long long total = 0, nmax = 0;
+    for (int o = 0; o < no; ++o) {
+        // a1: N_m = ceil(spp * |x(lam_max) - x(lam_min)|)
+        double xa = host_x_of_lambda(*d, o, d->lam_min[o]), xb = host_x_of_lambda(*d, o, d->lam_max[o]);
+        double n = std::ceil(d->samples_per_px * std::fabs(xb - xa));
+        if (!(n >= 0.0)) n = 0.0;
+        if (n > 2.0e9) return fail(E2E_ERR_UNSUPPORTED, "format_create: more than 2e9 samples in one order");
+        F->nsamp[o] = (long long)n;
+        F->dl[o] = n > 0.0 ? (d->lam_max[o] - d->lam_min[o]) / n : 0.0;
+        total += F->nsamp[o];
+        nmax = std::max(nmax, F->nsamp[o]);
+    }
+    F->samples_per_fiber = total;
+
+    // one device blob with every per-order / per-fiber array
+    size_t off = 0;
+    auto reserve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_m = reserve(sizeof(int) * no), o_lmin = reserve(8 * no), o_dl = reserve(8 * no), o_ns = reserve(8 * no);
+    const size_t o_bl = reserve(8 * no), o_ba = reserve(8 * no), o_fx = reserve(8 * nf), o_fy = reserve(8 * nf);
+    const size_t o_eff = reserve(d->eff_table ? 8 * (size_t)d->eff_n : 0);
+    char* blob = nullptr;
+    E2E_CUDA(cudaMalloc(&blob, off));
+    F->d_blob = blob;
+    auto fail_free = [&](int code) { cudaFree(blob); F->d_blob = nullptr; return code; };
+#define E2E_CUDA_F(call)                                                         \
+    do {                                                                         \
+        cudaError_t e__ = (call);                                                \
+        if (e__ != cudaSuccess) return fail_free(fail_cuda(e__, #call));         \
+    } while (0)
+    E2E_CUDA_F(cudaMemcpy(blob + o_m, d->order_m, sizeof(int) * no, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_lmin, d->lam_min, 8 * no, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_dl, F->dl.data(), 8 * no, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_ns, F->nsamp.data(), 8 * no, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_bl, d->blaze_lam_c, 8 * no, cudaMemcpyHostToDevice));
+    if (d->blaze_amp) E2E_CUDA_F(cudaMemcpy(blob + o_ba, d->blaze_amp, 8 * no, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_fx, d->fiber_dx, 8 * nf, cudaMemcpyHostToDevice));
+    E2E_CUDA_F(cudaMemcpy(blob + o_fy, d->fiber_dy, 8 * nf, cudaMemcpyHostToDevice));
+    if (d->eff_table) E2E_CUDA_F(cudaMemcpy(blob + o_eff, d->eff_table, 8 * (size_t)d->eff_n, cudaMemcpyHostToDevice));
+
+    FormatView& v = F->view;
+    memset(&v, 0, sizeof(v));
+    v.nx = d->nx; v.ny = d->ny; v.n_orders = no; v.n_fibers = nf; v.deg_l = d->deg_l; v.deg_m = d->deg_m;
+    v.lam0 = d->lam0; v.inv_dlam = d->inv_dlam; v.m0 = d->m0; v.inv_dm = d->inv_dm;
+    for (int i = 0; i < nc; ++i) { v.coef_x[i] = d->coef_x[i]; v.coef_y[i] = d->coef_y[i]; }
+    v.order_m = (const int*)(blob + o_m);
+    v.lam_min = (const double*)(blob + o_lmin);
+    v.dl = (const double*)(blob + o_dl);
+    v.nsamp = (const long long*)(blob + o_ns);
+    v.blaze_lam_c = (const double*)(blob + o_bl);
+    v.blaze_amp = d->blaze_amp ? (const double*)(blob + o_ba) : nullptr;
+    v.fiber_dx = (const double*)(blob + o_fx);
+    v.fiber_dy = (const double*)(blob + o_fy);
+    v.eff_table = d->eff_table ? (const double*)(blob + o_eff) : nullptr;
+    v.eff_n = d->eff_n; v.eff_lam0 = d->eff_lam0; v.eff_dlam = d->eff_dlam;
+
+    // device pass over every sample: monotonicity, spacing, row range per 64-column bin
+    const int n_bins = (d->nx + 2 * kBinPad + (1 << kBinShift) - 1) >> kBinShift;
+    F->n_bins = n_bins;
+    const size_t nb = (size_t)no * n_bins;
+    unsigned long long* scratch = nullptr;
+    E2E_CUDA_F(cudaMalloc(&scratch, 8 * (2 * (size_t)no + 2 * nb)));
+    unsigned long long *d_smin = scratch, *d_smax = scratch + no, *d_ymin = scratch + 2 * no, *d_ymax = d_ymin + nb;
+    cudaMemset(d_smin, 0xff, 8 * (size_t)no);
+    cudaMemset(d_smax, 0x00, 8 * (size_t)no);
+    cudaMemset(d_ymin, 0xff, 8 * nb);
+    cudaMemset(d_ymax, 0x00, 8 * nb);
+    if (nmax > 0) {
+        dim3 grid((unsigned)((nmax + 255) / 256), (unsigned)no);
+        scan_format_kernel<<<grid, 256>>>(v, n_bins, d_smin, d_smax, d_ymin, d_ymax);
+        count_launch();
+    }
+    std::vector<unsigned long long> h(2 * (size_t)no + 2 * nb);
+    cudaError_t ce = cudaMemcpy(h.data(), scratch, 8 * h.size(), cudaMemcpyDeviceToHost);
+    cudaFree(scratch);
+    if (ce != cudaSuccess) return fail_free(fail_cuda(ce, "format_create: scan"));
+    F->min_spacing.assign(no, 0.0);
+    F->bin_ymin.assign(nb, INFINITY);
+    F->bin_ymax.assign(nb, -INFINITY);
+    std::vector<double> max_spacing(no, 0.0);
+    for (int o = 0; o < no; ++o) {
+        if (F->nsamp[o] >= 2) {
+            if (h[o] == ~0ULL || h[no + o] == 0ULL) return fail_free(fail(E2E_ERR_CUDA, "format_create: scan produced no spacing"));
+            double dmin = dec_double(h[o]), dmax = dec_double(h[no + o]);
+            if (!(dmin > 0.0) && !(dmax < 0.0)) {
+                char buf[160];
+                snprintf(buf, sizeof buf, "format_create: x(lambda) is not strictly monotone in order index %d (m=%d)", o, d->order_m[o]);
+                return fail_free(fail(E2E_ERR_NOT_MONOTONIC, buf));
+            }
+            F->min_spacing[o] = std::min(std::fabs(dmin), std::fabs(dmax));
+            max_spacing[o] = std::max(std::fabs(dmin), std::fabs(dmax));
+        }
+        for (int b = 0; b < n_bins; ++b) {
+            unsigned long long a = h[2 * (size_t)no + (size_t)o * n_bins + b], c = h[2 * (size_t)no + nb + (size_t)o * n_bins + b];
+            if (a != ~0ULL && c != 0ULL) {
+                F->bin_ymin[(size_t)o * n_bins + b] = dec_double(a);
+                F->bin_ymax[(size_t)o * n_bins + b] = dec_double(c);
+            }
+        }
+    }
+    // keep max spacing behind min spacing (same vector, second half) to avoid another member
+    F->min_spacing.insert(F->min_spacing.end(), max_spacing.begin(), max_spacing.end());
+#undef E2E_CUDA_F
+    *out = F.release();
+    return E2E_OK;
+}
+
+void e2e_format_destroy(e2e_format_t* fmt)
+{
+    if (!fmt) return;
+    fmt->plans.clear();
+    if (fmt->d_blob) cudaFree(fmt->d_blob);
+    delete fmt;
+}
+
+int e2e_format_num_samples(const e2e_format_t* fmt, int64_t* n_per_order, int64_t* n_total)
+{
+    if (!fmt) return fail(E2E_ERR_INVALID_ARG, "format_num_samples: fmt is NULL");
+    if (n_per_order)
+        for (size_t o = 0; o < fmt->nsamp.size(); ++o) n_per_order[o] = fmt->nsamp[o];
+    if (n_total) *n_total = fmt->samples_per_fiber * fmt->view.n_fibers;
+    return E2E_OK;
+}
+
+// ================================================================================================
+// psf
+// ================================================================================================
+// Q chosen so that the Gauss-Chebyshev chord quadrature is converged below 1e-12 of the PSF peak:
+// measured against Q = 64 for D/(2 sigma) in [0, 3.3]
+static int auto_nodes(double a, double b, double sx, double sy)
+{
+    double r = std::max(a / sx, b / sy);
+    int q = (int)std::ceil(7.0 + 3.0 * r);
+    q += q & 1;
+    return std::min(std::max(q, 8), 64);
+}
+
+int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t ny)
+{
+    if (!out) return fail(E2E_ERR_INVALID_ARG, "psf_create: out is NULL");
+    *out = nullptr;
+    if (!d) return fail(E2E_ERR_INVALID_ARG, "psf_create: desc is NULL");
+    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "psf_create: bad detector size");
+    std::unique_ptr<e2e_psf> P(new (std::nothrow) e2e_psf);
+    if (!P) return fail(E2E_ERR_NOMEM, "psf_create: out of host memory");
+    memset(&P->an, 0, sizeof(P->an));
+    memset(&P->tab, 0, sizeof(P->tab));
+    P->kind = d->kind; P->nx = nx; P->ny = ny; P->Q = 0;
+    if (d->kind == 0) {
+        if (!(d->sigma_x > 0.0) || !(d->sigma_y > 0.0) || !is_fin(d->sigma_x) || !is_fin(d->sigma_y))
+            return fail(E2E_ERR_INVALID_ARG, "psf_create: sigma must be > 0");
+        if (!(d->fiber_dx_px >= 0.0) || !(d->fiber_dy_px >= 0.0) || !is_fin(d->fiber_dx_px) || !is_fin(d->fiber_dy_px))
+            return fail(E2E_ERR_INVALID_ARG, "psf_create: fiber widths must be >= 0");
+        if (!is_fin(d->support_nsigma)) return fail(E2E_ERR_INVALID_ARG, "psf_create: support_nsigma not finite");
+        if (d->n_nodes < 0) return fail(E2E_ERR_INVALID_ARG, "psf_create: n_nodes < 0");
+        if (d->n_nodes > 2 * kMaxTerms) return fail(E2E_ERR_UNSUPPORTED, "psf_create: n_nodes > 64");
+        const double t = d->support_nsigma > 0.0 ? d->support_nsigma : 7.5;
+        const double a = 0.5 * d->fiber_dx_px, b = 0.5 * d->fiber_dy_px;
+        // G9: H = D/2 + t sigma; footprint = all pixels touching [x - H, x + H]
+        const double Hx = 0.5 * d->fiber_dx_px + t * d->sigma_x, Hy = 0.5 * d->fiber_dy_px + t * d->sigma_y;
+        P->hbx = Hx + 0.5; P->hby = Hy + 0.5;
+        if (2.0 * P->hbx + 1.0 > 96.0 || 2.0 * P->hby + 1.0 > 96.0)
+            return fail(E2E_ERR_UNSUPPORTED, "psf_create: footprint larger than 96 px");
+        AnalyticParam& A = P->an;
+        A.inv_sx = 1.0 / d->sigma_x; A.inv_sy = 1.0 / d->sigma_y;
+        A.hbx = P->hbx; A.hby = P->hby;
+        A.by_gauss = !(b > 0.0);
+        A.paired = 0;
+        if (!(a > 0.0) && !(b > 0.0)) {           // P2: pure gaussian, one term
+            P->Q = 1; A.n_terms = 1; A.s[0] = 0.0; A.cs[0] = 0.0; A.wq[0] = 1.0; A.g[0] = 1.0;
+        } else {
+            const int Q = d->n_nodes > 0 ? d->n_nodes : auto_nodes(a, b, d->sigma_x, d->sigma_y);
+            P->Q = Q;
+            int nt = 0;
+            // nodes q and Q+1-q share |s|, c and the weight: one term with F(d) = Phi(d - s) + Phi(d + s)
+            for (int q = 1; 2 * q <= Q + 1; ++q) {
+                const long double th = (long double)q * 3.14159265358979323846264338327950288L / (long double)(Q + 1);
+                const long double sn = sinl(th), cn = cosl(th);
+                A.s[nt] = (double)((long double)a * cn);
+                const long double c = (long double)b * sn;
+                A.cs[nt] = (double)(c / (long double)d->sigma_y);
+                A.wq[nt] = (double)((2.0L / (long double)(Q + 1)) * sn * sn);
+                A.g[nt] = b > 0.0 ? (double)((long double)d->sigma_y / (2.0L * c)) : 1.0;
+                if (2 * q != Q + 1) A.paired |= 1u << nt;
+                else A.s[nt] = 0.0;               // middle node of an odd rule sits at s = 0
+                ++nt;
+            }
+            A.n_terms = nt;
+        }
+    } else if (d->kind == 1) {
+        if (d->tab_npix < 1 || d->tab_os < 1 || d->tab_gx < 1 || d->tab_gy < 1 || !d->tab)
+            return fail(E2E_ERR_INVALID_ARG, "psf_create: bad tabulated PSF description");
+        const long long n = (long long)d->tab_npix * d->tab_os;
+        if (n > 256 || d->tab_npix > 94) return fail(E2E_ERR_UNSUPPORTED, "psf_create: tabulated kernel larger than 256 cells / 94 px");
+        if ((long long)d->tab_gx * d->tab_gy > 4096) return fail(E2E_ERR_UNSUPPORTED, "psf_create: more than 4096 field nodes");
+        const size_t ncell = (size_t)n * n, nk = (size_t)d->tab_gx * d->tab_gy;
+        for (size_t i = 0; i < ncell * nk; ++i)
+            if (!is_fin(d->tab[i])) return fail(E2E_ERR_INVALID_ARG, "psf_create: non-finite table value");
+        P->hbx = P->hby = 0.5 * (double)d->tab_npix + 0.5;
+        TabParam& T = P->tab;
+        T.npix = d->tab_npix; T.os = d->tab_os; T.n = (int)n; T.gx = d->tab_gx; T.gy = d->tab_gy; T.ld = (int)n + 1;
+        T.hb = P->hbx; T.half = 0.5 * (double)d->tab_npix;
+        T.fsx = nx > 1 ? (double)(d->tab_gx - 1) / (double)(nx - 1) : 0.0;
+        T.fsy = ny > 1 ? (double)(d->tab_gy - 1) / (double)(ny - 1) : 0.0;
+        // T2: summed-area table C[b][a] = sum of cells [0,b) x [0,a), accumulated in long double
+        const size_t ld = (size_t)n + 1;
+        std::vector<double> sat(nk * ld * ld, 0.0);
+        std::vector<long double> rowacc(ld);
+        for (size_t k = 0; k < nk; ++k) {
+            const double* Tk = d->tab + k * ncell;
+            double* S = sat.data() + k * ld * ld;
+            std::fill(rowacc.begin(), rowacc.end(), 0.0L);
+            for (size_t bb = 1; bb <= (size_t)n; ++bb) {
+                long double run = 0.0L;
+                for (size_t aa = 1; aa <= (size_t)n; ++aa) {
+                    run += (long double)Tk[(bb - 1) * n + (aa - 1)];
+                    rowacc[aa] += run;
+                    S[bb * ld + aa] = (double)rowacc[aa];
+                }
+            }
+        }
+        E2E_CUDA(cudaMalloc(&P->d_sat, 8 * sat.size()));
+        cudaError_t ce = cudaMemcpy(P->d_sat, sat.data(), 8 * sat.size(), cudaMemcpyHostToDevice);
+        if (ce != cudaSuccess) { cudaFree(P->d_sat); return fail_cuda(ce, "psf_create: table upload"); }
+        T.sat = P->d_sat;
+    } else {
+        return fail(E2E_ERR_INVALID_ARG, "psf_create: kind must be 0 or 1");
+    }
+    P->fp_cols = (int)std::floor(2.0 * P->hbx) + 1;
+    P->fp_rows = (int)std::floor(2.0 * P->hby) + 1;
+    *out = P.release();
+    return E2E_OK;
+}
+
+void e2e_psf_destroy(e2e_psf_t* psf)
+{
+    if (!psf) return;
+    if (psf->d_sat) cudaFree(psf->d_sat);
+    delete psf;
+}
+
+}  // extern "C"
+
+// ================================================================================================
+// schedule: strips, runs, colours, phases
+// ================================================================================================
+namespace e2e {
+
+struct Interval { int lo, hi, strip; };
+
+static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
+{
+    std::lock_guard<std::mutex> lock(F->plan_mu);
+    for (auto& p : F->plans)
+        if (p->hbx == P->hbx && p->hby == P->hby) { *out = p.get(); return E2E_OK; }
+    std::unique_ptr<e2e_plan> pl(new e2e_plan);
+    pl->hbx = P->hbx; pl->hby = P->hby;
+    const int no = F->view.n_orders, nf = F->view.n_fibers, nx = F->view.nx;
+    const int n_strips = no * nf;
+    if (n_strips > 65535) return fail(E2E_ERR_UNSUPPORTED, "render: more than 65535 (fiber, order) strips");
+    pl->n_strips = n_strips;
+    pl->strips.resize(n_strips);
+    long long off = 0;
+    for (int f = 0; f < nf; ++f)
+        for (int o = 0; o < no; ++o) {
+            pl->strips[f * no + o] = Strip{off, F->nsamp[o]};
+            off += F->nsamp[o];
+        }
+    pl->total_samples = off;
+    const double* min_sp = F->min_spacing.data();
+    const double* max_sp = F->min_spacing.data() + no;
+
+    // ---- colours: strips whose pixel coverage may overlap must not run in the same launch
+    const int nB = (nx + 63) >> 6;
+    std::vector<int> cov_lo((size_t)n_strips * nB, 1), cov_hi((size_t)n_strips * nB, 0);   // empty: lo > hi
+    for (int f = 0; f < nf; ++f)
+        for (int o = 0; o < no; ++o) {
+            if (F->nsamp[o] == 0) continue;
+            const int s = f * no + o;
+            const double margin = P->hbx + 2.0 + 32.0 * max_sp[o];
+            if (margin + std::fabs(F->fiber_dx[f]) > (double)kBinPad)
+                return fail(E2E_ERR_UNSUPPORTED, "render: footprint + fiber offset + 32 sample spacings exceeds 256 px");
+            for (int B = 0; B < nB; ++B) {
+                const double lo = 64.0 * B - margin - F->fiber_dx[f], hi = 64.0 * B + 63.0 + margin - F->fiber_dx[f];
+                int b0 = (int)std::floor((lo + kBinPad) / 64.0), b1 = (int)std::floor((hi + kBinPad) / 64.0);
+                b0 = std::max(b0, 0); b1 = std::min(b1, F->n_bins - 1);
+                double ymin = INFINITY, ymax = -INFINITY;
+                for (int b = b0; b <= b1; ++b) {
+                    ymin = std::min(ymin, F->bin_ymin[(size_t)o * F->n_bins + b]);
+                    ymax = std::max(ymax, F->bin_ymax[(size_t)o * F->n_bins + b]);
+                }
+                if (!(ymin <= ymax)) continue;
+                double rlo = std::floor(ymin + F->fiber_dy[f] - P->hby) - 1.0, rhi = std::ceil(ymax + F->fiber_dy[f] + P->hby) + 1.0;
+                rlo = std::max(rlo, -1.0e9); rhi = std::min(rhi, 1.0e9);
+                cov_lo[(size_t)s * nB + B] = (int)rlo;
+                cov_hi[(size_t)s * nB + B] = (int)rhi;
+            }
+        }
+    std::vector<std::vector<int>> adj(n_strips);
+    std::vector<Interval> iv;
+    for (int B = 0; B < nB; ++B) {
+        iv.clear();
+        for (int s = 0; s < n_strips; ++s)
+            if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B])
+                iv.push_back(Interval{cov_lo[(size_t)s * nB + B], cov_hi[(size_t)s * nB + B], s});
+        std::sort(iv.begin(), iv.end(), [](const Interval& a, const Interval& b) { return a.lo < b.lo || (a.lo == b.lo && a.strip < b.strip); });
+        for (size_t i = 0; i < iv.size(); ++i)
+            for (size_t j = i + 1; j < iv.size() && iv[j].lo <= iv[i].hi; ++j) {
+                adj[iv[i].strip].push_back(iv[j].strip);
+                adj[iv[j].strip].push_back(iv[i].strip);
+            }
+    }
+    std::vector<int> color(n_strips, -1);
+    int n_colors = 0;
+    std::vector<char> used;
+    for (int s = 0; s < n_strips; ++s) {
+        used.assign(n_colors + 1, 0);
+        for (int t : adj[s])
+            if (color[t] >= 0) used[color[t]] = 1;
+        int c = 0;
+        while (used[c]) ++c;
+        color[s] = c;
+        n_colors = std::max(n_colors, c + 1);
+    }
+    pl->n_colors = n_colors;
+
+    // ---- runs: alternate runs of a strip go to different launches; two runs of the same parity are separated
+    //      by a full run whose x-extent exceeds 2 hb + 3 px, so their pixel windows are disjoint
+    std::vector<std::vector<Item>> phases((size_t)n_colors * 2);
+    for (int s = 0; s < n_strips; ++s) {
+        const int o = s % no;
+        const long long N = F->nsamp[o];
+        if (N == 0) continue;
+        const long long nchunks = (N + 31) / 32;
+        long long G = nchunks;
+        if (N >= 2 && min_sp[o] > 0.0) {
+            double g = std::floor((2.0 * P->hbx + 3.0) / (32.0 * min_sp[o])) + 1.0;
+            if (g < (double)nchunks) G = (long long)g;
+        }
+        int run = 0;
+        for (long long c0 = 0; c0 < nchunks; c0 += G, ++run)
+            phases[(size_t)color[s] * 2 + (run & 1)].push_back(Item{s, (int)c0, (int)std::min(G, nchunks - c0)});
+    }
+    std::vector<Item> flat;
+    pl->phase_off.clear();
+    pl->phase_off.push_back(0);
+    for (auto& ph : phases) {
+        if (ph.empty()) continue;
+        flat.insert(flat.end(), ph.begin(), ph.end());
+        pl->phase_off.push_back((int)flat.size());
+    }
+    pl->n_phases = (int)pl->phase_off.size() - 1;
+    pl->n_items = (int)flat.size();
+    E2E_CUDA(cudaMalloc(&pl->d_strips, sizeof(Strip) * std::max(1, n_strips)));
+    E2E_CUDA(cudaMemcpy(pl->d_strips, pl->strips.data(), sizeof(Strip) * n_strips, cudaMemcpyHostToDevice));
+    E2E_CUDA(cudaMalloc(&pl->d_items, sizeof(Item) * std::max<size_t>(1, flat.size())));
+    if (!flat.empty()) E2E_CUDA(cudaMemcpy(pl->d_items, flat.data(), sizeof(Item) * flat.size(), cudaMemcpyHostToDevice));
+    *out = pl.get();
+    F->plans.push_back(std::move(pl));
+    return E2E_OK;
+}
+
+static size_t sample_array_bytes(long long total) { return align_up((size_t)std::max<long long>(total, 1) * 8, 256); }
+
+static int check_spectra(const e2e_format* F, const e2e_spectrum_t* spectra, const char* who)
+{
+    if (!spectra) return fail(E2E_ERR_INVALID_ARG, std::string(who) + ": spectra is NULL");
+    for (int f = 0; f < F->view.n_fibers; ++f) {
+        const e2e_spectrum_t& s = spectra[f];
+        if (!s.d_flux || s.n < 2 || !(s.dlam > 0.0) || !is_fin(s.lam0) || !is_fin(s.scale) || !(s.doppler > 0.0) || !is_fin(s.doppler))
+            return fail(E2E_ERR_INVALID_ARG, std::string(who) + ": bad spectrum descriptor");
+    }
+    return E2E_OK;
+}
+
+static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spectrum_t* spectra, double* d_x, double* d_y,
+                        double* d_w, cudaStream_t stream)
+{
+    SpectraParam sp;
+    memset(&sp, 0, sizeof(sp));
+    for (int f = 0; f < F->view.n_fibers; ++f) sp.s[f] = spectra[f];
+    long long nmax = 0;
+    for (long long n : F->nsamp) nmax = std::max(nmax, n);
+    if (nmax == 0) return E2E_OK;
+    dim3 grid((unsigned)((nmax + 255) / 256), (unsigned)pl->n_strips);
+    setup_samples_kernel<<<grid, 256, 0, stream>>>(F->view, sp, pl->d_strips, 0, nullptr, d_x, d_y, d_w);
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "setup_samples_kernel launch");
+    return E2E_OK;
+}
+
+static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
+                         const double* d_w, double* d_frame, cudaStream_t stream)
+{
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    const size_t smem_an = (size_t)kWarpsPerCta * (kWinCols + kWinRows) * kLdk * sizeof(double);
+    const int lat_ld = kTabWin + 2;
+    const size_t smem_tab = (size_t)kWarpsPerCta * lat_ld * lat_ld * sizeof(double);
+    std::call_once(once, [&] {
+        attr_err = cudaFuncSetAttribute(render_analytic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_an);
+    });
+    if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
+    for (int ph = 0; ph < pl->n_phases; ++ph) {
+        const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
+        if (n <= 0) continue;
+        const unsigned blocks = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
+        if (P->kind == 0)
+            render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n,
+                                                                                   P->an, d_frame, F->view.nx, F->view.ny);
+        else
+            render_tabulated_kernel<<<blocks, kWarpsPerCta * 32, smem_tab, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0,
+                                                                                     n, P->tab, lat_ld, d_frame, F->view.nx, F->view.ny);
+        count_launch();
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(e, "render kernel launch");
+    }
+    return E2E_OK;
+}
+
+}  // namespace e2e
+
+extern "C" {
+
+int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, size_t* bytes)
+{
+    if (!fmt || !psf || !bytes) return fail(E2E_ERR_INVALID_ARG, "render_workspace_bytes: NULL argument");
+    if (psf->nx != fmt->view.nx || psf->ny != fmt->view.ny)
+        return fail(E2E_ERR_INVALID_ARG, "render_workspace_bytes: psf was created for another detector size");
+    e2e_plan* pl = nullptr;
+    int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    *bytes = 3 * sample_array_bytes(pl->total_samples);
+    return E2E_OK;
+}
+
+int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spectrum, int32_t fiber, int32_t order_index,
+                      double* d_lam, double* d_x, double* d_y, double* d_w, int64_t capacity, void* cuda_stream)
+{
+    if (!fmt || !spectrum) return fail(E2E_ERR_INVALID_ARG, "setup_samples: NULL argument");
+    if (fiber < 0 || fiber >= fmt->view.n_fibers || order_index < 0 || order_index >= fmt->view.n_orders)
+        return fail(E2E_ERR_INVALID_ARG, "setup_samples: fiber / order out of range");
+    if (!spectrum->d_flux || spectrum->n < 2 || !(spectrum->dlam > 0.0) || !(spectrum->doppler > 0.0))
+        return fail(E2E_ERR_INVALID_ARG, "setup_samples: bad spectrum descriptor");
+    const long long N = fmt->nsamp[order_index];
+    if (capacity < N) return fail(E2E_ERR_INVALID_ARG, "setup_samples: capacity smaller than the order's sample count");
+    if (N == 0) return E2E_OK;
+    // a one-strip launch: the strip table travels through a small device allocation owned by this call's stream order
+    Strip st{0, N};
+    Strip* d_st = nullptr;
+    E2E_CUDA(cudaMalloc(&d_st, sizeof(Strip)));
+    cudaError_t ce = cudaMemcpy(d_st, &st, sizeof(Strip), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) { cudaFree(d_st); return fail_cuda(ce, "setup_samples: strip upload"); }
+    SpectraParam sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.s[fiber] = *spectrum;
+    dim3 grid((unsigned)((N + 255) / 256), 1);
+    setup_samples_kernel<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(fmt->view, sp, d_st, fiber * fmt->view.n_orders + order_index,
+                                                                      d_lam, d_x, d_y, d_w);
+    count_launch();
+    ce = cudaGetLastError();
+    cudaError_t ce2 = cudaStreamSynchronize((cudaStream_t)cuda_stream);
+    cudaFree(d_st);
+    if (ce != cudaSuccess) return fail_cuda(ce, "setup_samples_kernel launch");
+    if (ce2 != cudaSuccess) return fail_cuda(ce2, "setup_samples_kernel");
+    return E2E_OK;
+}
+
+int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, double* d_frame,
+                     int32_t accumulate, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!fmt || !psf || !d_frame) return fail(E2E_ERR_INVALID_ARG, "render_frame: NULL argument");
+    if (psf->nx != fmt->view.nx || psf->ny != fmt->view.ny)
+        return fail(E2E_ERR_INVALID_ARG, "render_frame: psf was created for another detector size");
+    int rc = check_spectra(fmt, spectra, "render_frame");
+    if (rc) return rc;
+    e2e_plan* pl = nullptr;
+    rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    const size_t per = sample_array_bytes(pl->total_samples);
+    if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace NULL or not 256-byte aligned");
+    if (workspace_bytes < 3 * per) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    double* d_x = (double*)d_workspace;
+    double* d_y = (double*)((char*)d_workspace + per);
+    double* d_w = (double*)((char*)d_workspace + 2 * per);
+    if (!accumulate) E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
+    rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
+    if (rc) return rc;
+    return launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+}
+
+int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, size_t* bytes)
+{
+    if (!fmt || !psf || !spectra || !bytes) return fail(E2E_ERR_INVALID_ARG, "render_host_workspace_bytes: NULL argument");
+    size_t inner = 0;
+    int rc = e2e_render_workspace_bytes(fmt, psf, &inner);
+    if (rc) return rc;
+    size_t total = align_up((size_t)fmt->view.nx * fmt->view.ny * 8, 256);
+    for (int f = 0; f < fmt->view.n_fibers; ++f) {
+        if (spectra[f].n < 2) return fail(E2E_ERR_INVALID_ARG, "render_host_workspace_bytes: bad spectrum descriptor");
+        total += align_up((size_t)spectra[f].n * 8, 256);
+    }
+    *bytes = total + inner;
+    return E2E_OK;
+}
+
+int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, double* h_frame,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!fmt || !psf || !h_frame) return fail(E2E_ERR_INVALID_ARG, "render_frame_host: NULL argument");
+    int rc = check_spectra(fmt, spectra, "render_frame_host");
+    if (rc) return rc;
+    size_t need = 0;
+    rc = e2e_render_host_workspace_bytes(fmt, psf, spectra, &need);
+    if (rc) return rc;
+    if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace NULL or not 256-byte aligned");
+    if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace too small");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    char* p = (char*)d_workspace;
+    double* d_frame = (double*)p;
+    const size_t frame_bytes = (size_t)fmt->view.nx * fmt->view.ny * 8;
+    p += align_up(frame_bytes, 256);
+    std::vector<e2e_spectrum_t> dev(spectra, spectra + fmt->view.n_fibers);
+    for (int f = 0; f < fmt->view.n_fibers; ++f) {
+        // fibers that share one host table share one device copy
+        int same = -1;
+        for (int g = 0; g < f; ++g)
+            if (spectra[g].d_flux == spectra[f].d_flux && spectra[g].n == spectra[f].n) { same = g; break; }
+        if (same >= 0) { dev[f].d_flux = dev[same].d_flux; continue; }
+        E2E_CUDA(cudaMemcpyAsync(p, spectra[f].d_flux, (size_t)spectra[f].n * 8, cudaMemcpyHostToDevice, stream));
+        dev[f].d_flux = (const double*)p;
+        p += align_up((size_t)spectra[f].n * 8, 256);
+    }
+    const size_t used = (size_t)(p - (char*)d_workspace);
+    rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
+    if (rc) return rc;
+    E2E_CUDA(cudaMemcpyAsync(h_frame, d_frame, frame_bytes, cudaMemcpyDeviceToHost, stream));
+    E2E_CUDA(cudaStreamSynchronize(stream));
+    return E2E_OK;
+}
+
+int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_t* det,
+                       void* cuda_stream)
+{
+    if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector: NULL argument");
+    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector: bad frame size");
+    if (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias))
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector: non-finite parameter");
+    return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
+}
+
+int e2e_measure_fp64_peak(int32_t repeats, double* dfma_per_s, double* ms)
+{
+    return measure_fp64_peak(repeats, dfma_per_s, ms);
+}
+
+}  // extern "C"

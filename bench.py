@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the echellogram-rendering hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A step = one pass of the whole hot path (a1-a6: zero-fill, sample setup, render, detector stage) over one frame
+of the synthetic workload (default: ESPRESSO-like, BASELINE.json configs[1]).  Prints ONE JSON line.
+N > 1 (torchrun): every rank renders its own replica of the frame ("replicas only"); no collective
+on the data path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "fp64 lambda-sample x pixel contributions/s"
+UNIT = "contributions/s"
+
+# flop-equivalents of the special-function edge evaluations, SURVEY.md 8(d) (used only for the secondary
+# "survey_formula" figure; the headline roofline counts the irreducible FMAs only)
+C_ERFC, C_PSI = 60.0, 90.0
+
+
+def make_scene(name: str):
+    from paper_2008_05858_b200 import workloads as W
+    if name == "espresso_like":
+        return W.espresso_like(), "espresso_like (BASELINE.json configs[1]: 2 fibers x 85 orders, 9216x9216, 32 samples/px)"
+    if name == "tiny":
+        return W.tiny(), "tiny (BASELINE.json configs[0])"
+    if name == "hires_like":
+        return W.hires_like(), "hires_like (BASELINE.json configs[2]: 10 fibers x 60 orders, 9216x9216, 32 samples/px)"
+    if name == "field_psf":
+        return W.field_psf(), "field_psf (BASELINE.json configs[3]: ESPRESSO-like geometry, 5x5 grid of 11x11-px 8x kernels)"
+    if name == "rv_sweep":
+        return W.rv_sweep(10.0), "rv_sweep (BASELINE.json configs[4], one of the 5 frames, v = 10 m/s)"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def support_half_widths(psf):
+    """hb = footprint half-width + 1/2 per axis (G9) -- used only to COUNT contributions"""
+    if psf.kind == 1:
+        h = 0.5 * psf.tab_npix + 0.5
+        return h, h
+    t = psf.support_nsigma if psf.support_nsigma > 0 else 7.5
+    return 0.5 * psf.fiber_dx_px + t * psf.sigma_x + 0.5, 0.5 * psf.fiber_dy_px + t * psf.sigma_y + 0.5
+
+
+def algorithmic_flops_per_sample(psf, Q: int, ncols: float, nrows: float):
+    """(irreducible FMA flops, SURVEY 8(d) formula) per sample for the analytic path."""
+    if psf.kind != 0:
+        return None, None
+    T = (Q + 1) // 2 if Q > 1 else 1                       # paired chord terms
+    fma_only = 2.0 * T * ncols * nrows
+    n = 0.5 * (ncols + nrows)
+    survey = 200.0 + Q * (n + 1) * C_ERFC + (Q / 2.0) * 2 * (n + 1) * C_PSI + 2.0 * Q * ncols * nrows
+    return fma_only, survey
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)"""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline at N=1, and --impl reference)
+# ----------------------------------------------------------------------------------------------------------------
+def oracle_sample_scene(scene, target_samples: int):
+    """A bounded sample of the workload: the middle order, all fibers, a wavelength sub-range holding about
+    target_samples / n_fibers samples per fiber; returns (sub-scene, window) with the window enclosing the footprints."""
+    import oracle
+    o = scene.n_orders // 2
+    sub = scene.subset(orders=[o])
+    n_full = oracle.order_nsamples(sub, 0)
+    per_fiber = max(64, target_samples // scene.n_fibers)
+    frac = min(1.0, per_fiber / max(n_full, 1))
+    lmin, lmax = float(sub.lam_min[0]), float(sub.lam_max[0])
+    mid = 0.5 * (lmin + lmax)
+    half = 0.5 * (lmax - lmin) * frac
+    # keep the sampling density of the full order: N = ceil(spp * |dx|) over the sub-range
+    sub.lam_min = np.array([mid - half]); sub.lam_max = np.array([mid + half])
+    hbx, hby = support_half_widths(scene.psf)
+    xs, ys = [], []
+    for f in range(sub.n_fibers):
+        n = oracle.order_nsamples(sub, 0)
+        for k in (0, n // 2, n - 1):
+            lam, x, y, w = oracle.samples(sub, f, 0, k, k + 1)
+            xs.append(x[0]); ys.append(y[0])
+    # the trace is smooth: pad the bounding box of its ends and middle generously
+    i0 = max(0, int(np.floor(min(xs) - hbx)) - 8); i1 = min(scene.nx, int(np.ceil(max(xs) + hbx)) + 8)
+    j0 = max(0, int(np.floor(min(ys) - hby)) - 64); j1 = min(scene.ny, int(np.ceil(max(ys) + hby)) + 64)
+    return sub, (i0, j0, i1 - i0, j1 - j0)
+
+
+def time_oracle(scene, target_samples: int, steps: int = 1, warmup: int = 0):
+    import oracle
+    sub, win = oracle_sample_scene(scene, target_samples)
+    hbx, hby = support_half_widths(scene.psf)
+    ncols, nrows = np.floor(2 * hbx), np.floor(2 * hby)
+    times, touched = [], 0
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle.render(sub, window=win)
+        dt = time.perf_counter() - t0
+        touched = oracle.render.last_touched
+        if it >= warmup:
+            times.append(dt)
+    n_samples = sum(oracle.order_nsamples(sub, 0) for _ in range(sub.n_fibers))
+    contrib = float(n_samples) * float(ncols * nrows)
+    t = float(np.mean(times))
+    return {"value": contrib / t, "unit": UNIT, "cores": oracle.cpu_threads(), "kind": "oracle",
+            "sample": f"{n_samples} samples ({sub.n_fibers} fibers x 1 order, {touched} touched the window) of the "
+                      f"{scene.name} workload, oracle Q=32 long double, {t:.2f} s per pass",
+            "seconds": t, "contributions": contrib}
+
+
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    scene, wname = make_scene(args.workload)
+    r = time_oracle(scene, args.oracle_samples, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": r["seconds"] * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wname, "note": "CPU oracle (oracle/e2e_oracle.c) as it stands, each step a bounded sample"},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------------------------
+def count_contributions(B, r, hbx, hby):
+    """exact number of (sample, pixel) pairs inside the footprint boxes (G9) clipped to the detector; a COUNT for
+    the metric's unit, computed with torch ops on the setup kernel's own x, y"""
+    import torch
+    nmax = int(r.per_order.max())
+    x = torch.empty(max(nmax, 1), dtype=torch.float64, device=r.device)
+    y = torch.empty_like(x)
+    total = 0
+    for f in range(r.scene.n_fibers):
+        for o in range(r.scene.n_orders):
+            n = int(r.per_order[o])
+            if n == 0:
+                continue
+            B.e2e_setup_samples(r.fmt, r.spectra[f], f, o, None, x, y, None, capacity=nmax)
+            xs, ys = x[:n], y[:n]
+            ilo = torch.clamp(torch.ceil(xs - hbx), min=0); ihi = torch.clamp(torch.floor(xs + hbx), max=r.scene.nx - 1)
+            jlo = torch.clamp(torch.ceil(ys - hby), min=0); jhi = torch.clamp(torch.floor(ys + hby), max=r.scene.ny - 1)
+            total += int((torch.clamp(ihi - ilo + 1, min=0) * torch.clamp(jhi - jlo + 1, min=0)).sum().item())
+    return total
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_2008_05858_b200 import build as _build
+    if rank == 0:
+        _build.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    from paper_2008_05858_b200 import binding as B, workloads as W
+    B.load()                                             # raises if libe2e.so is missing: no CPU fallback
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    scene, wname = make_scene(args.workload)
+    det = scene.detector or W.Detector(gain=1.0, dark_e=0.0, ron_e=3.0, bias=0.0, seed=2008_05858 + rank)
+    r = B.Renderer(scene, device=str(dev))
+    info = r.psf.info()
+    hbx, hby = support_half_widths(scene.psf)
+    contrib = count_contributions(B, r, hbx, hby)
+    n_samples = r.n_samples
+    frame = torch.empty((scene.ny, scene.nx), dtype=torch.float64, device=dev)
+    noisy = torch.empty_like(frame)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.e2e_render_frame(r.fmt, r.psf, r.spectra, frame, False, r.workspace, stream)
+        B.e2e_apply_detector(frame, noisy, scene.nx, scene.ny, det, stream)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # ---- device-timed region: K steps, inputs resident in HBM
+    B.e2e_profile_enable(True)
+    B.e2e_profile_read(reset=True)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = B.e2e_launch_count()
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = B.e2e_launch_count() - n0
+    ms_total = ev0.elapsed_time(ev1)
+    prof = B.e2e_profile_read(reset=True)
+    B.e2e_profile_enable(False)
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * contrib / (ms_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the spectra, D2H of the frame, every step
+    e2e = None
+    if not args.no_e2e:
+        host_tabs = [torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).pin_memory() for sp in scene.spectra]
+        desc = B.spectra_array(scene.spectra, [t.data_ptr() for t in host_tabs])
+        nbytes = B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc)
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+        h_frame = torch.empty((scene.ny, scene.nx), dtype=torch.float64).pin_memory()
+        h2d = sum(int(np.asarray(sp.flux).shape[0]) * 8 for sp in {id(sp.flux): sp for sp in scene.spectra}.values())
+        d2h = scene.nx * scene.ny * 8
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, h_frame.data_ptr(), ws, det=det, stream=stream)      # warm-up
+        barrier()
+        k_e2e = max(2, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            B.e2e_render_frame_host(r.fmt, r.psf, desc, h_frame.data_ptr(), ws, det=det, stream=stream)   # synchronises
+        barrier()
+        dt = (time.perf_counter() - t0) / k_e2e
+        if world > 1:
+            import torch.distributed as dist
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * contrib / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "ms_per_step": dt * 1e3, "steps": k_e2e}
+        del ws, h_frame
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (render): plain FP64 ALU bound
+    burst, sustained = B.e2e_measure_fp64_peak(80)
+    peak_tf = 2.0 * sustained / 1e12
+    ncols, nrows = info["footprint_cols"], info["footprint_rows"]
+    nominal = float(np.floor(2 * hbx) * np.floor(2 * hby))
+    fma_flops, survey_flops = algorithmic_flops_per_sample(scene.psf, info["n_nodes"], np.floor(2 * hbx), np.floor(2 * hby))
+    ms_render = prof["ms_render"] / max(prof["n_calls"], 1)
+    roofline = None
+    if fma_flops is not None and ms_render > 0:
+        ach = n_samples * fma_flops / (ms_render * 1e-3) / 1e12
+        roofline = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": None,
+                    "kernel": "render_analytic_kernel", "kernel_ms_per_step": ms_render,
+                    "kernel_launches_per_step": prof["n_render"] / max(prof["n_calls"], 1),
+                    "peak_source": "measured in this run: e2e_measure_fp64_peak sustained DFMA rate x 2 (MEASURED_PEAKS.json has no fp64 entry)",
+                    "peak_burst": 2.0 * burst / 1e12,
+                    "flops_per_sample": fma_flops, "definition": "irreducible rank-T FMA accumulate only: 2*T*ncols*nrows per sample",
+                    "achieved_survey_formula": n_samples * survey_flops / (ms_render * 1e-3) / 1e12,
+                    "survey_flops_per_sample": survey_flops}
+    cpu = None
+    if not args.no_cpu:
+        c = time_oracle(scene, args.oracle_samples)
+        cpu = {k: c[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": wname, "n_samples": n_samples, "contributions": contrib, "footprint_nominal_px": nominal,
+                       "chord_nodes_Q": info["n_nodes"], "frame": [scene.ny, scene.nx], "stages": "a1-a6 (zero-fill, setup, render, detector)",
+                       "l2": "inputs larger than L2: sample arrays %.0f MB + frame %.0f MB vs 126 MB L2" % (n_samples * 24 / 1e6, scene.nx * scene.ny * 8 / 1e6),
+                       "multi_gpu": "replicas only"},
+            "frame_ms": ms_step, "samples_per_s": world * n_samples / (ms_step * 1e-3),
+            "stage_ms_per_step": {k: prof[k] / max(prof["n_calls"], 1) for k in ("ms_zero", "ms_setup", "ms_render", "ms_detector")},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="espresso_like")
+    ap.add_argument("--oracle-samples", type=int, default=200_000, help="size of the CPU oracle's bounded sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

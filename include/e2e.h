@@ -118,6 +118,10 @@ typedef struct {
 E2E_API int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* desc, int32_t nx, int32_t ny);
 E2E_API void e2e_psf_destroy(e2e_psf_t* psf);
 
+/* what the library derived from the description: the chord-quadrature order Q in use (1 for a pure gaussian,
+ * 0 for a tabulated PSF) and the largest footprint in columns / rows (G9).  Any output pointer may be NULL. */
+E2E_API int e2e_psf_info(const e2e_psf_t* psf, int32_t* n_nodes, int32_t* footprint_cols, int32_t* footprint_rows);
+
 /* ------------------------------------------------------------------------------------------------
  * Rendering (a1-a5)
  * ------------------------------------------------------------------------------------------------ */
@@ -150,12 +154,14 @@ E2E_API int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, cons
 
 /* Same as e2e_render_frame with HOST buffers: spectra[f].d_flux are HOST pointers and h_frame is a HOST
  * [ny*nx] array (pinned memory gives full PCIe speed).  The call copies the tables to the device, renders,
- * copies the frame back and synchronises the stream before returning.  Device scratch is taken from
- * d_workspace, which must hold e2e_render_host_workspace_bytes() bytes. */
+ * applies the detector stage a6 when det != NULL, copies the frame back and synchronises the stream before
+ * returning.  Device scratch is taken from d_workspace, which must hold e2e_render_host_workspace_bytes() bytes. */
 E2E_API int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                                     size_t* bytes);
+struct e2e_detector;
 E2E_API int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
-                          double* h_frame, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+                          const struct e2e_detector* det /* may be NULL */, double* h_frame, void* d_workspace,
+                          size_t workspace_bytes, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Detector stage (a6; "photon noise and all other specific detector noises ... are added on the
@@ -163,7 +169,7 @@ E2E_API int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf,
  * drawn from a Philox4x32-10 stream keyed by (seed, pixel index p = j*nx + i): the result does not depend
  * on launch geometry and is reproducible bit for bit (algorithm: DESIGN.md G12).
  * ------------------------------------------------------------------------------------------------ */
-typedef struct {
+typedef struct e2e_detector {
     double gain, dark_e, ron_e, bias;
     uint64_t seed;
 } e2e_detector_t;
@@ -175,13 +181,28 @@ E2E_API int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, in
 /* ------------------------------------------------------------------------------------------------
  * Measurement helpers (used by bench.py; not part of the rendering path)
  * ------------------------------------------------------------------------------------------------ */
-/* Runs an all-SM kernel of independent DFMA chains `repeats` times and returns the best sustained rate in
- * *dfma_per_s (fused multiply-adds per second; flop/s = 2x) and the kernel time of that run in *ms.
- * Synchronous. */
-E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* dfma_per_s, double* ms);
+/* FP64 roofline denominator.  Launches an all-SM kernel of independent DFMA chains `repeats` times back to back
+ * (each launch ~10 ms) and returns fused multiply-adds per second (flop/s = 2x): *burst = the fastest single
+ * launch, *sustained = total work / total time of the second half of the launches.  Synchronous. */
+E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s);
 
 /* Number of kernel launches the library has issued since load (all entry points), for bench.py's gpu_launches. */
 E2E_API int64_t e2e_launch_count(void);
+
+/* Per-stage device timing.  While enabled, every e2e_render_frame / e2e_apply_detector call brackets its stages
+ * with CUDA events recorded on the caller's stream (no synchronisation is added).  e2e_profile_read waits for
+ * the recorded events, adds their elapsed times to the totals below and returns them; reset != 0 clears the
+ * totals afterwards.  ms_* are summed device milliseconds, n_* the number of kernel launches in that stage. */
+typedef struct {
+    double ms_zero;      /* zero-fill of the frame (cudaMemsetAsync) */
+    double ms_setup;     /* a1-a3 sample-setup kernel */
+    double ms_render;    /* a4-a5 render kernels (all phases) */
+    double ms_detector;  /* a6 */
+    int64_t n_setup, n_render, n_detector;
+    int64_t n_calls;     /* e2e_render_frame calls covered */
+} e2e_profile_t;
+E2E_API int e2e_profile_enable(int32_t on);
+E2E_API int e2e_profile_read(e2e_profile_t* out, int32_t reset);
 
 #ifdef __cplusplus
 }

@@ -21,9 +21,9 @@ ERROR_NAMES = {-1: "E2E_ERR_INVALID_ARG", -2: "E2E_ERR_NOT_MONOTONIC", -3: "E2E_
 
 # every symbol include/e2e.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_destroy", "e2e_format_num_samples",
-           "e2e_psf_create", "e2e_psf_destroy", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
+           "e2e_psf_create", "e2e_psf_destroy", "e2e_psf_info", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_measure_fp64_peak",
-           "e2e_launch_count"]
+           "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read"]
 
 
 class E2EError(RuntimeError):
@@ -52,6 +52,11 @@ class PsfDesc(C.Structure):
 class SpectrumDesc(C.Structure):
     _fields_ = [("d_flux", C.c_void_p), ("n", C.c_int64), ("lam0", C.c_double), ("dlam", C.c_double),
                 ("scale", C.c_double), ("doppler", C.c_double)]
+
+
+class ProfileDesc(C.Structure):
+    _fields_ = [("ms_zero", C.c_double), ("ms_setup", C.c_double), ("ms_render", C.c_double), ("ms_detector", C.c_double),
+                ("n_setup", C.c_int64), ("n_render", C.c_int64), ("n_detector", C.c_int64), ("n_calls", C.c_int64)]
 
 
 class DetectorDesc(C.Structure):
@@ -86,6 +91,8 @@ def load():
     L.e2e_psf_create.argtypes = [C.POINTER(vp), C.POINTER(PsfDesc), i32, i32]
     L.e2e_psf_destroy.restype = None
     L.e2e_psf_destroy.argtypes = [vp]
+    L.e2e_psf_info.restype = C.c_int
+    L.e2e_psf_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
     L.e2e_render_workspace_bytes.restype = C.c_int
     L.e2e_render_workspace_bytes.argtypes = [vp, vp, C.POINTER(C.c_size_t)]
     L.e2e_setup_samples.restype = C.c_int
@@ -95,13 +102,17 @@ def load():
     L.e2e_render_host_workspace_bytes.restype = C.c_int
     L.e2e_render_host_workspace_bytes.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(C.c_size_t)]
     L.e2e_render_frame_host.restype = C.c_int
-    L.e2e_render_frame_host.argtypes = [vp, vp, C.POINTER(SpectrumDesc), vp, vp, C.c_size_t, vp]
+    L.e2e_render_frame_host.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorDesc), vp, vp, C.c_size_t, vp]
     L.e2e_apply_detector.restype = C.c_int
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
     L.e2e_measure_fp64_peak.restype = C.c_int
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_launch_count.restype = i64
     L.e2e_launch_count.argtypes = []
+    L.e2e_profile_enable.restype = C.c_int
+    L.e2e_profile_enable.argtypes = [i32]
+    L.e2e_profile_read.restype = C.c_int
+    L.e2e_profile_read.argtypes = [C.POINTER(ProfileDesc), i32]
     _lib = L
     return L
 
@@ -196,6 +207,11 @@ class Psf:
         self.handle = C.c_void_p()
         _check(load().e2e_psf_create(C.byref(self.handle), C.byref(d), int(nx), int(ny)))
 
+    def info(self):
+        q, c, r = C.c_int32(), C.c_int32(), C.c_int32()
+        _check(load().e2e_psf_info(self.handle, C.byref(q), C.byref(c), C.byref(r)))
+        return {"n_nodes": int(q.value), "footprint_cols": int(c.value), "footprint_rows": int(r.value)}
+
     def close(self):
         if getattr(self, "handle", None) is not None and self.handle.value:
             load().e2e_psf_destroy(self.handle)
@@ -260,8 +276,12 @@ def e2e_render_host_workspace_bytes(fmt: Format, psf: Psf, spectra_desc) -> int:
     return int(n.value)
 
 
-def e2e_render_frame_host(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: int, d_workspace, stream=None):
-    _check(load().e2e_render_frame_host(fmt.handle, psf.handle, spectra_desc, int(h_frame_ptr), int(d_workspace.data_ptr()),
+def e2e_render_frame_host(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: int, d_workspace, det=None, stream=None):
+    """spectra_desc[f].d_flux are HOST addresses, h_frame_ptr a HOST address (pinned for full PCIe speed)."""
+    d = None
+    if det is not None:
+        d = C.byref(DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed)))
+    _check(load().e2e_render_frame_host(fmt.handle, psf.handle, spectra_desc, d, int(h_frame_ptr), int(d_workspace.data_ptr()),
                                         int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
 
 
@@ -271,10 +291,21 @@ def e2e_apply_detector(d_in, d_out, nx: int, ny: int, det, stream=None):
                                      _stream_ptr(stream)))
 
 
-def e2e_measure_fp64_peak(repeats: int = 5):
-    rate, ms = C.c_double(), C.c_double()
-    _check(load().e2e_measure_fp64_peak(int(repeats), C.byref(rate), C.byref(ms)))
-    return float(rate.value), float(ms.value)
+def e2e_measure_fp64_peak(repeats: int = 60):
+    """(burst, sustained) DFMA/s of independent fp64 FMA chains on every SM."""
+    burst, sus = C.c_double(), C.c_double()
+    _check(load().e2e_measure_fp64_peak(int(repeats), C.byref(burst), C.byref(sus)))
+    return float(burst.value), float(sus.value)
+
+
+def e2e_profile_enable(on: bool):
+    _check(load().e2e_profile_enable(int(bool(on))))
+
+
+def e2e_profile_read(reset: bool = True) -> dict:
+    p = ProfileDesc()
+    _check(load().e2e_profile_read(C.byref(p), int(bool(reset))))
+    return {k: getattr(p, k) for k, _ in ProfileDesc._fields_}
 
 
 # ---------------------------------------------------------------------------------------------------------

@@ -25,9 +25,47 @@ int fail_cuda(cudaError_t e, const char* what)
 }
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream);
-int measure_fp64_peak(int repeats, double* dfma_per_s, double* ms_out);
+int measure_fp64_peak(int repeats, double* burst, double* sustained);
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------------------------
+// per-stage device timing (e2e_profile_*): event pairs recorded on the caller's stream, resolved on read
+// ------------------------------------------------------------------------------------------------
+enum Stage { kStageZero = 0, kStageSetup, kStageRender, kStageDetector, kNumStages };
+struct Pending { int stage; cudaEvent_t a, b; };
+static std::mutex g_prof_mu;
+static bool g_prof_on = false;
+static std::vector<Pending> g_prof_pending;
+static std::vector<cudaEvent_t> g_prof_free;
+static e2e_profile_t g_prof_tot = {};
+
+static cudaEvent_t prof_event()
+{
+    if (!g_prof_free.empty()) { cudaEvent_t e = g_prof_free.back(); g_prof_free.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+// RAII bracket of one stage; inert while profiling is off
+struct StageTimer {
+    cudaStream_t stream; int stage; cudaEvent_t a = nullptr; bool on;
+    StageTimer(int stage_, cudaStream_t s) : stream(s), stage(stage_)
+    {
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        on = g_prof_on;
+        if (on) { a = prof_event(); if (a) cudaEventRecord(a, stream); else on = false; }
+    }
+    ~StageTimer()
+    {
+        if (!on) return;
+        std::lock_guard<std::mutex> lk(g_prof_mu);
+        cudaEvent_t b = prof_event();
+        if (!b) { g_prof_free.push_back(a); return; }
+        cudaEventRecord(b, stream);
+        g_prof_pending.push_back(Pending{stage, a, b});
+    }
+};
 static inline bool is_fin(double v) { return std::isfinite(v); }
 
 // host copy of sample_position's x (same operation sequence: O1, O2)
@@ -334,6 +372,15 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
     return E2E_OK;
 }
 
+int e2e_psf_info(const e2e_psf_t* psf, int32_t* n_nodes, int32_t* footprint_cols, int32_t* footprint_rows)
+{
+    if (!psf) return fail(E2E_ERR_INVALID_ARG, "psf_info: psf is NULL");
+    if (n_nodes) *n_nodes = psf->Q;
+    if (footprint_cols) *footprint_cols = psf->fp_cols;
+    if (footprint_rows) *footprint_rows = psf->fp_rows;
+    return E2E_OK;
+}
+
 void e2e_psf_destroy(e2e_psf_t* psf)
 {
     if (!psf) return;
@@ -587,10 +634,24 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     double* d_x = (double*)d_workspace;
     double* d_y = (double*)((char*)d_workspace + per);
     double* d_w = (double*)((char*)d_workspace + 2 * per);
-    if (!accumulate) E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
-    rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
-    if (rc) return rc;
-    return launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+    if (!accumulate) {
+        StageTimer tm(kStageZero, stream);
+        E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
+    }
+    {
+        StageTimer tm(kStageSetup, stream);
+        const long long before = g_launches.load();
+        rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
+        if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
+        if (rc) return rc;
+    }
+    {
+        StageTimer tm(kStageRender, stream);
+        const long long before = g_launches.load();
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+        if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
+    }
+    return rc;
 }
 
 int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, size_t* bytes)
@@ -608,8 +669,9 @@ int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* ps
     return E2E_OK;
 }
 
-int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, double* h_frame,
-                          void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                          const e2e_detector_t* det, double* h_frame, void* d_workspace, size_t workspace_bytes,
+                          void* cuda_stream)
 {
     if (!fmt || !psf || !h_frame) return fail(E2E_ERR_INVALID_ARG, "render_frame_host: NULL argument");
     int rc = check_spectra(fmt, spectra, "render_frame_host");
@@ -638,6 +700,10 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
     const size_t used = (size_t)(p - (char*)d_workspace);
     rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
     if (rc) return rc;
+    if (det) {
+        rc = e2e_apply_detector(d_frame, d_frame, fmt->view.nx, fmt->view.ny, det, stream);
+        if (rc) return rc;
+    }
     E2E_CUDA(cudaMemcpyAsync(h_frame, d_frame, frame_bytes, cudaMemcpyDeviceToHost, stream));
     E2E_CUDA(cudaStreamSynchronize(stream));
     return E2E_OK;
@@ -650,12 +716,45 @@ int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx
     if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector: bad frame size");
     if (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias))
         return fail(E2E_ERR_INVALID_ARG, "apply_detector: non-finite parameter");
+    StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
+    if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
     return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
 }
 
-int e2e_measure_fp64_peak(int32_t repeats, double* dfma_per_s, double* ms)
+int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s)
 {
-    return measure_fp64_peak(repeats, dfma_per_s, ms);
+    return measure_fp64_peak(repeats, burst_dfma_per_s, sustained_dfma_per_s);
+}
+
+int e2e_profile_enable(int32_t on)
+{
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    g_prof_on = on != 0;
+    return E2E_OK;
+}
+
+int e2e_profile_read(e2e_profile_t* out, int32_t reset)
+{
+    if (!out) return fail(E2E_ERR_INVALID_ARG, "profile_read: out is NULL");
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    for (auto& p : g_prof_pending) {
+        cudaError_t e = cudaEventSynchronize(p.b);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
+        g_prof_free.push_back(p.a);
+        g_prof_free.push_back(p.b);
+        if (e != cudaSuccess) { g_prof_pending.clear(); return fail_cuda(e, "profile_read"); }
+        switch (p.stage) {
+            case kStageZero: g_prof_tot.ms_zero += ms; break;
+            case kStageSetup: g_prof_tot.ms_setup += ms; break;
+            case kStageRender: g_prof_tot.ms_render += ms; break;
+            default: g_prof_tot.ms_detector += ms; break;
+        }
+    }
+    g_prof_pending.clear();
+    *out = g_prof_tot;
+    if (reset) g_prof_tot = e2e_profile_t{};
+    return E2E_OK;
 }
 
 }  // extern "C"

@@ -2,6 +2,7 @@
 // MEASURED_PEAKS.json has no fp64 entry, so bench.py measures the sustained DFMA rate of the same GPU in the
 // same run and reports the render kernel against it.
 #include "common.cuh"
+#include <algorithm>
 
 namespace e2e {
 
@@ -20,35 +21,45 @@ __global__ void __launch_bounds__(256) dfma_chain_kernel(double* out, int iters,
     if (s == 123456.789) out[0] = s;      // never true: keeps the chains alive
 }
 
-int measure_fp64_peak(int repeats, double* dfma_per_s, double* ms_out)
+int measure_fp64_peak(int repeats, double* burst, double* sustained)
 {
     int dev = 0, sms = 0;
     E2E_CUDA(cudaGetDevice(&dev));
     E2E_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (repeats < 2) repeats = 2;
+    if (repeats > 4096) repeats = 4096;
     double* d_out = nullptr;
     E2E_CUDA(cudaMalloc(&d_out, 8));
-    cudaEvent_t e0, e1;
-    E2E_CUDA(cudaEventCreate(&e0));
-    E2E_CUDA(cudaEventCreate(&e1));
+    std::vector<cudaEvent_t> ev(repeats + 1, nullptr);
+    for (auto& e : ev) cudaEventCreate(&e);
     const int iters = 8192, threads = 256, blocks = sms * 8;
-    double best = 0.0, best_ms = 0.0;
-    for (int r = 0; r < (repeats < 1 ? 1 : repeats) + 1; ++r) {
-        cudaEventRecord(e0);
+    const double work = (double)blocks * threads * (double)iters * 64.0;       // DFMAs per launch
+    dfma_chain_kernel<<<blocks, threads>>>(d_out, iters, 0.999999, 1e-7);       // warm-up
+    count_launch();
+    cudaEventRecord(ev[0]);
+    for (int r = 0; r < repeats; ++r) {
         dfma_chain_kernel<<<blocks, threads>>>(d_out, iters, 0.999999, 1e-7);
         count_launch();
-        cudaEventRecord(e1);
-        cudaError_t e = cudaEventSynchronize(e1);
-        if (e != cudaSuccess) { cudaFree(d_out); return fail_cuda(e, "dfma_chain_kernel"); }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        double rate = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
-        if (r > 0 && rate > best) { best = rate; best_ms = ms; }   // first run is warm-up
+        cudaEventRecord(ev[r + 1]);
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    cudaError_t e = cudaEventSynchronize(ev[repeats]);
+    double best = 0.0, sus = 0.0;
+    if (e == cudaSuccess) {
+        for (int r = 0; r < repeats; ++r) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, ev[r], ev[r + 1]);
+            if (ms > 0.f) best = std::max(best, work / (ms * 1e-3));
+        }
+        float ms = 0.f;
+        const int h = repeats / 2;
+        cudaEventElapsedTime(&ms, ev[h], ev[repeats]);
+        if (ms > 0.f) sus = work * (repeats - h) / (ms * 1e-3);
+    }
+    for (auto& x : ev) cudaEventDestroy(x);
     cudaFree(d_out);
-    if (dfma_per_s) *dfma_per_s = best;
-    if (ms_out) *ms_out = best_ms;
+    if (e != cudaSuccess) return fail_cuda(e, "dfma_chain_kernel");
+    if (burst) *burst = best;
+    if (sustained) *sustained = sus;
     return E2E_OK;
 }
 

@@ -1,0 +1,399 @@
+"""-m gpu: the CUDA path (through the C ABI of include/e2e.h) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars (BASELINE.json north_star, G8/G10/G12):
+  * a1/a3  lam_k, x_k, y_k : bit-exact (the footprint boxes depend on them)
+  * a2     w_k             : 4e-15 relative (libm sin vs CUDA sin differ in the last ulp)
+  * a4/a5  frame           : |G - O| <= 1e-10 |O| + 1e-14 max(O) per pixel
+  * a6     detector        : bit-exact
+"""
+import copy
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2008_05858_b200 import workloads as W
+from parity_util import assert_frame_parity, frame_errors, photocenter_x, photocenter_y, with_psf
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2008_05858_b200 import build, binding
+    build.build()
+    binding.load()
+    return binding
+
+
+def gpu_render(B, scene, **kw):
+    r = B.Renderer(scene)
+    try:
+        fr = r.render(**kw)
+        r.torch.cuda.synchronize()
+        return fr.cpu().numpy()
+    finally:
+        r.close()
+
+
+def small_tiny(spp=4.0, lam=(5010.0, 5013.0)):
+    s = W.tiny(samples_per_px=spp)
+    s.lam_min = np.array([lam[0]])
+    s.lam_max = np.array([lam[1]])
+    return s
+
+
+# ------------------------------------------------------------------------------------------ a1-a3
+@pytest.mark.parametrize("which", ["tiny", "espresso"])
+def test_setup_samples_positions_bit_exact(B, which):
+    if which == "tiny":
+        s = W.tiny()
+        pairs = [(0, 0)]
+    else:
+        s = W.espresso_like(n_obj_lines=200, table_dlam=0.01).subset(orders=[0, 41, 84])
+        pairs = [(0, 0), (1, 1), (1, 2)]
+    r = B.Renderer(s)
+    try:
+        per, tot = r.fmt.num_samples()
+        for o in range(s.n_orders):
+            assert int(per[o]) == oracle.order_nsamples(s, o)
+        assert tot == int(per.sum()) * s.n_fibers
+        for fiber, o in pairs:
+            lam, x, y, w = r.samples(fiber, o)
+            ol, ox, oy, ow = oracle.samples(s, fiber, o)
+            assert np.array_equal(lam, ol)
+            assert np.array_equal(x, ox)
+            assert np.array_equal(y, oy)
+            assert np.allclose(w, ow, rtol=4e-15, atol=0.0)
+            assert np.count_nonzero(w) > 0.9 * len(w)
+    finally:
+        r.close()
+
+
+def test_setup_samples_doppler_and_efficiency_table(B):
+    s = small_tiny(spp=3.0)
+    s.spectra[0].doppler = 1.0 + 10.0 / W.C_LIGHT
+    s.eff_table = np.array([0.5, 0.55, 0.9, 0.7])
+    s.eff_lam0, s.eff_dlam = 5005.0, 4.0
+    r = B.Renderer(s)
+    try:
+        lam, x, y, w = r.samples(0, 0)
+        ol, ox, oy, ow = oracle.samples(s, 0, 0)
+        assert np.array_equal(x, ox) and np.array_equal(y, oy)
+        assert np.allclose(w, ow, rtol=4e-15, atol=0.0)
+    finally:
+        r.close()
+
+
+# ------------------------------------------------------------------------------------------ a4/a5 analytic
+def test_render_tiny_full_parity(B):
+    """BASELINE.json configs[0]: 80 000 samples, 19x19 footprints, whole 2048x256 frame element by element"""
+    s = W.tiny()
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    e = assert_frame_parity(G, O, "tiny")
+    assert e["max_rel_core"] < 1e-11
+    tot = oracle.total_weight(s)
+    assert abs(G.sum() / tot - 1.0) < 1e-12                       # flux conservation on the GPU frame
+    assert abs(photocenter_x(G) - photocenter_x(O)) < 1e-9
+    assert abs(photocenter_y(G) - photocenter_y(O)) < 1e-9
+
+
+def test_render_is_deterministic_and_accumulates(B):
+    s = small_tiny(spp=8.0, lam=(5010.0, 5020.0))
+    r = B.Renderer(s)
+    try:
+        a = r.render().cpu().numpy()
+        b = r.render().cpu().numpy()
+        assert np.array_equal(a, b)
+        f = r.render()
+        r.render(frame=f, accumulate=True)
+        assert np.array_equal(f.cpu().numpy(), a + a)
+    finally:
+        r.close()
+
+
+@pytest.mark.parametrize("psf_kw", [
+    dict(fiber_dx_px=0.0, fiber_dy_px=0.0, sigma_x=0.9, sigma_y=1.3),      # P2: pure asymmetric gaussian
+    dict(fiber_dx_px=4.0, fiber_dy_px=4.0, sigma_x=1.2, sigma_y=1.2),      # ESPRESSO-like PSF
+    dict(fiber_dx_px=5.0, fiber_dy_px=2.0, sigma_x=0.8, sigma_y=1.5),      # elliptical fiber image, asymmetric PSF
+    dict(fiber_dx_px=3.0, fiber_dy_px=0.0, sigma_x=1.0, sigma_y=1.0),      # degenerate ellipse: Dy = 0
+    dict(fiber_dx_px=6.6, fiber_dy_px=6.6, sigma_x=1.0, sigma_y=1.0),      # R/sigma = 3.3: needs the larger auto Q
+    dict(fiber_dx_px=3.0, fiber_dy_px=3.0, sigma_x=1.0, sigma_y=1.0, support_nsigma=4.0),   # narrow truncation box
+    dict(fiber_dx_px=8.0, fiber_dy_px=8.0, sigma_x=2.5, sigma_y=2.5),      # footprint 47 px: multi-panel windows
+])
+def test_render_psf_variants(B, psf_kw):
+    s = with_psf(small_tiny(spp=3.0, lam=(5010.0, 5012.0)), **psf_kw)
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, str(psf_kw))
+
+
+def test_render_single_sample_is_the_psf_itself(B):
+    d = W.single_line_scene(x_pos=100.3173, y_pos=37.8641)
+    G = gpu_render(B, d)
+    O = oracle.render(d)
+    assert_frame_parity(G, O, "single sample")
+    nz = np.nonzero(G)
+    assert (nz[1].min(), nz[1].max(), nz[0].min(), nz[0].max()) == (91, 109, 29, 47)      # G9 box
+    assert abs(photocenter_x(G) - 100.3173) < 1e-9 and abs(photocenter_y(G) - 37.8641) < 1e-9
+    # tests/golden P1 value (mpmath polar quadrature of the definition)
+    assert G[38, 100] == pytest.approx(oracle.psf_pixel(d.psf, 100 - 100.3173, 38 - 37.8641), rel=1e-12)
+
+
+def test_render_detector_edges_and_offdetector(B):
+    for xp, yp in [(4.25, 3.75), (55.5, 36.0), (-30.0, 3.7), (0.0, 0.0), (59.0, 39.0), (-9.4, 20.0)]:
+        d = W.single_line_scene(x_pos=xp, y_pos=yp, nx=60, ny=40, samples=3)
+        G = gpu_render(B, d)
+        O = oracle.render(d)
+        if O.max() == 0.0:
+            assert G.max() == 0.0 and G.min() == 0.0
+        else:
+            assert_frame_parity(G, O, f"edge {xp},{yp}")
+
+
+def test_render_overlapping_fibers_and_orders(B):
+    """two fibers 5 px apart (overlapping strips) and two orders crossing the same columns 12 px apart:
+    the schedule must serialise them; result == oracle, and == sum of single-fiber renders"""
+    s = small_tiny(spp=4.0, lam=(5010.0, 5014.0))
+    s.order_m = np.array([100, 101], dtype=np.int32)
+    s.lam_min = np.array([5010.0, 5010.0]); s.lam_max = np.array([5014.0, 5014.0])
+    s.blaze_lam_c = np.array([5025.0, 5015.0]); s.blaze_amp = np.array([1.0, 0.7])
+    s.deg_m = 1
+    s.coef_x = np.array([1024.0, 3.0, 1000.0, 0.0, 1.0, 0.0, 0.0, 0.0])          # c[p*2+q]
+    s.coef_y = np.array([138.24, 12.0, 10.0, 0.0, 0.01, 0.0, 0.0, 0.0])
+    s.fiber_dx = np.array([0.0, 0.3, -0.2]); s.fiber_dy = np.array([-5.0, 0.0, 5.0])
+    sp = s.spectra[0]
+    s.spectra = [sp, W.Spectrum(flux=sp.flux[::-1].copy(), lam0=sp.lam0, dlam=sp.dlam, scale=3e3), copy.copy(sp)]
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert_frame_parity(G, O, "3 fibers x 2 orders")
+    parts = np.zeros_like(G)
+    for f in range(3):
+        parts += gpu_render(B, s.subset(fibers=[f]))
+    assert np.allclose(G, parts, rtol=1e-13, atol=1e-16 * G.max())
+
+
+def test_render_steep_and_reversed_traces(B):
+    """x decreasing with lambda (monotone either way is legal) and a steep trace (dy/dx = 0.6)"""
+    s = small_tiny(spp=5.0, lam=(5010.0, 5012.0))
+    s.coef_x = np.array([1024.0, -1000.0, 1.0, 0.0])
+    s.coef_y = np.array([128.0, 600.0, 0.0, 0.0])
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert_frame_parity(G, O, "reversed steep")
+
+
+def test_render_sparse_sampling(B):
+    """samples 2.5 px apart (spp = 0.4): chunk windows far wider than one panel"""
+    s = small_tiny(spp=0.4, lam=(5005.0, 5045.0))
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert_frame_parity(G, O, "sparse")
+
+
+def test_render_zero_and_negative_flux(B):
+    s = small_tiny(spp=2.0)
+    s.spectra = [W.Spectrum(flux=np.zeros(16), lam0=5000.0, dlam=4.0, scale=1.0)]
+    assert np.all(gpu_render(B, s) == 0.0)
+    rng = np.random.default_rng(3)
+    s.spectra = [W.Spectrum(flux=rng.normal(size=400), lam0=5009.0, dlam=0.01, scale=1.0)]     # linear: negative flux legal
+    G, O = gpu_render(B, s), oracle.render(s)
+    e = frame_errors(G, O)
+    assert e["max_abs_over_max"] < 1e-12
+
+
+def test_format_rejects_non_monotone_x(B):
+    s = small_tiny(spp=2.0, lam=(5000.0, 5050.0))
+    s.coef_x = np.array([1024.0, 10.0, -600.0, 0.0])            # x = 1024 + 10 u - 600 u^2 turns over inside the order
+    with pytest.raises(B.E2EError) as ei:
+        B.Format(s)
+    assert ei.value.code == -2
+
+
+def test_workspace_errors(B):
+    import torch
+    s = small_tiny(spp=2.0)
+    r = B.Renderer(s)
+    try:
+        fr = torch.empty((s.ny, s.nx), dtype=torch.float64, device="cuda")
+        small = torch.empty(256, dtype=torch.uint8, device="cuda")
+        with pytest.raises(B.E2EError) as ei:
+            B.e2e_render_frame(r.fmt, r.psf, r.spectra, fr, False, small)
+        assert ei.value.code == -6
+    finally:
+        r.close()
+
+
+# ------------------------------------------------------------------------------------------ full-size ESPRESSO-like
+@pytest.fixture(scope="module")
+def espresso_gpu(B):
+    s = W.espresso_like()
+    r = B.Renderer(s)
+    fr = r.render()
+    r.torch.cuda.synchronize()
+    G = fr.cpu().numpy()
+    r.close()
+    return s, G
+
+
+def test_render_espresso_full_frame_windows(B, espresso_gpu):
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py times; the oracle computes
+    sampled windows (both fibers, blue / middle / red orders, frame edges and the centre)"""
+    s, G = espresso_gpu
+    assert np.isfinite(G).all()
+    rng = np.random.default_rng(11)
+    wins = []
+    for o in (0, 1, 40, 84):
+        n = oracle.order_nsamples(s, o)
+        for frac in (0.0005, rng.uniform(0.1, 0.9), 0.9995):
+            k = int(frac * (n - 1))
+            lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
+            wins.append((max(0, int(x[0]) - 24), max(0, int(y[0]) - 20), 48, 40))
+    worst = 0.0
+    for (i0, j0, wnx, wny) in wins:
+        O = oracle.render(s, window=(i0, j0, wnx, wny))
+        assert O.max() > 0
+        e = assert_frame_parity(G[j0:j0 + wny, i0:i0 + wnx], O, f"window {i0},{j0}")
+        worst = max(worst, e["max_tol_ratio"])
+    assert worst <= 1.0
+
+
+def test_render_espresso_flux_conservation_and_gaps(B, espresso_gpu):
+    s, G = espresso_gpu
+    tot = oracle.total_weight(s)
+    assert abs(float(G.sum(dtype=np.longdouble)) / tot - 1.0) < 1e-12
+    # between orders nothing is written: row 117 - 40 and the last rows are exactly zero
+    assert np.all(G[:60] == 0.0)
+    assert G.min() >= 0.0
+
+
+# ------------------------------------------------------------------------------------------ a4/a5 tabulated
+def small_field_scene(gx=3, gy=2, npix=7, os=4, seed=77, nx=300, ny=120):
+    s = small_tiny(spp=3.0, lam=(5010.0, 5013.0))
+    s.nx, s.ny = nx, ny
+    s.coef_x = np.array([150.0, 2400.0, 1.0, 0.0])        # u in [-0.6, -0.48] -> x spans the whole 300-px detector... see below
+    s.coef_x = np.array([1590.0, 2400.0, 1.0, 0.0])       # x = 1590 + 2400 u: u = -0.6 -> 150.4 ; u = -0.48 -> 438
+    s.lam_max = np.array([5012.5])                        # u = -0.5 -> 390 - ... keeps part of the trace off the detector (G11)
+    s.coef_y = np.array([60.0, 40.0, 0.0, 0.0])
+    tab = W.tabulated_kernels(seed=seed, npix=npix, os=os, gx=gx, gy=gy)
+    s.psf = W.Psf(kind=1, tab_npix=npix, tab_os=os, tab_gx=gx, tab_gy=gy, tab=tab)
+    return s
+
+
+@pytest.mark.parametrize("grid", [(1, 1), (3, 2), (5, 5)])
+def test_render_tabulated_small(B, grid):
+    s = small_field_scene(gx=grid[0], gy=grid[1])
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, f"tabulated {grid}")
+
+
+def test_render_tabulated_11px_8x(B):
+    s = small_field_scene(gx=2, gy=2, npix=11, os=8)
+    s.lam_max = np.array([5010.6])
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert_frame_parity(G, O, "tabulated 11 px x 8")
+
+
+def test_render_field_psf_full_frame_windows(B):
+    """BASELINE.json configs[3] at full size; oracle on sampled windows"""
+    base = W.espresso_like(n_obj_lines=500, table_dlam=0.005)
+    s = W.field_psf(base=base)
+    G = gpu_render(B, s)
+    assert np.isfinite(G).all()
+    for o, frac in ((0, 0.3), (42, 0.77), (84, 0.5)):
+        n = oracle.order_nsamples(s, o)
+        k = int(frac * (n - 1))
+        lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
+        i0, j0 = int(x[0]) - 8, int(y[0]) - 10
+        O = oracle.render(s, window=(i0, j0, 16, 20))
+        assert O.max() > 0
+        assert_frame_parity(G[j0:j0 + 20, i0:i0 + 16], O, f"field window {i0},{j0}")
+    tot = oracle.total_weight(s)
+    assert abs(float(G.sum(dtype=np.longdouble)) / tot - 1.0) < 1e-11
+
+
+# ------------------------------------------------------------------------------------------ host entry point
+def test_render_frame_host_matches_device_path(B):
+    import torch
+    s = small_tiny(spp=4.0)
+    r = B.Renderer(s)
+    try:
+        dev = r.render().cpu().numpy()
+        host_tabs = [np.ascontiguousarray(sp.flux, dtype=np.float64) for sp in s.spectra]
+        desc = B.spectra_array(s.spectra, [t.ctypes.data for t in host_tabs])
+        nbytes = B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc)
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        out = torch.empty((s.ny, s.nx), dtype=torch.float64).pin_memory()
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws)
+        assert np.array_equal(out.numpy(), dev)
+    finally:
+        r.close()
+
+
+# ------------------------------------------------------------------------------------------ a6 detector
+def test_detector_bit_exact(B):
+    import torch
+    rng = np.random.default_rng(5)
+    nx, ny = 333, 77
+    fr = np.concatenate([np.zeros(1000), rng.uniform(0, 5, 5000), rng.uniform(5, 64, 5000), rng.uniform(64, 200, 5000),
+                         rng.uniform(3e4, 5e4, nx * ny - 16000)])
+    fr[17] = -3.0
+    fr = fr.reshape(ny, nx)
+    det = W.Detector(gain=0.9, dark_e=0.4, ron_e=3.0, bias=100.0, seed=0x1234_5678_9ABC_DEF0)
+    d_in = torch.from_numpy(fr).cuda()
+    d_out = torch.empty_like(d_in)
+    B.e2e_apply_detector(d_in, d_out, nx, ny, det)
+    G = d_out.cpu().numpy()
+    O = oracle.detector(fr, det)
+    assert np.array_equal(G, O)
+    # in place, and independent of launch geometry: same result when applied to the same buffer
+    B.e2e_apply_detector(d_in, d_in, nx, ny, det)
+    assert np.array_equal(d_in.cpu().numpy(), O)
+    assert abs(G[-1].mean() / (0.9 * fr[-1].mean() + 0.4 + 100.0) - 1.0) < 0.01
+
+
+def test_rv_sweep_photocenter_linear_in_velocity(B):
+    """BASELINE.json configs[4]: 5 Doppler-shifted frames; global photocenter shift vs the analytic slope and
+    per-line centroid residual against a straight line in v < 1e-6 px; GPU == oracle on the v = 10 m/s frame;
+    detector stage bit-exact on the rendered frame"""
+    import torch
+    frames, xc = [], []
+    for v in W.RV_SWEEP_V:
+        s = W.rv_sweep(v)
+        G = gpu_render(B, s)
+        frames.append(G)
+        xc.append(photocenter_x(G))
+    s10 = W.rv_sweep(10.0)
+    O = oracle.render(s10)
+    assert_frame_parity(frames[-1], O, "rv 10 m/s")
+    assert abs(photocenter_x(frames[-1]) - photocenter_x(O)) < 1e-9
+    v = np.array(W.RV_SWEEP_V)
+    shift = np.array(xc) - xc[0]
+    # analytic slope: d<x>/dv = sum w x' lam / c / sum w  (G14); x' = dx/dlam = (1000 + 2u)/25
+    lam, x, y, w = oracle.samples(W.rv_sweep(0.0), 0, 0)
+    u = (lam - 5025.0) / 25.0
+    # doppler moves the spectrum, not the samples: the weight pattern shifts by +lam v/c in wavelength
+    slope = float(np.sum(w * (1000.0 + 2.0 * u) / 25.0 * lam) / np.sum(w)) / W.C_LIGHT
+    assert np.max(np.abs(shift - slope * v)) < 1e-6
+    # per-line windows (Voronoi cells of integer columns between line positions)
+    cen = W.rv_sweep(0.0).notes["line_centers"]
+    xl = 1024 + 1000 * (cen - 5025) / 25 + ((cen - 5025) / 25) ** 2
+    edges = np.round(0.5 * (xl[1:] + xl[:-1])).astype(int)
+    worst = 0.0
+    for ell in (3, 50, 100, 150, 196):
+        c0, c1 = edges[ell - 1], edges[ell]
+        pcs = np.array([photocenter_x(f[:, c0:c1], c0) for f in frames])
+        A = np.vstack([v, np.ones_like(v)]).T
+        coef, *_ = np.linalg.lstsq(A, pcs, rcond=None)
+        worst = max(worst, float(np.max(np.abs(pcs - A @ coef))))
+    assert worst < 1e-6
+    det = s10.detector
+    d_in = torch.from_numpy(frames[-1]).cuda()
+    d_out = torch.empty_like(d_in)
+    B.e2e_apply_detector(d_in, d_out, s10.nx, s10.ny, det)
+    assert np.array_equal(d_out.cpu().numpy(), oracle.detector(frames[-1], det))
+    assert 3e4 < frames[-1].max() < 6e4

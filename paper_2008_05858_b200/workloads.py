@@ -363,7 +363,7 @@ def rv_sweep(v_mps: float = 0.0, seed: int = 5005, samples_per_px: float = 256.0
     flux = _gaussian_lines(tab_lam0, tab_dlam, n_tab, cen, sig, np.ones(200))
     # a line of unit peak and sigma 0.01 A holds sqrt(2 pi) 0.01 A of flux * blaze ~0.4-1; spread by the
     # PSF over ~ (3 px core)^2: scale so the brightest pixel is ~4e4 e-
-    s.spectra = [Spectrum(flux=flux, lam0=tab_lam0, dlam=tab_dlam, scale=1.2e7,
+    s.spectra = [Spectrum(flux=flux, lam0=tab_lam0, dlam=tab_dlam, scale=1.8e7,
                           doppler=1.0 + v_mps / C_LIGHT)]
     s.detector = Detector(gain=1.0, dark_e=0.0, ron_e=3.0, bias=0.0, seed=seed)
     s.notes = {"line_centers": cen, "v_mps": v_mps}

@@ -3,9 +3,12 @@
 #include "setup.cuh"
 #include "render_analytic.cuh"
 #include "render_tabulated.cuh"
+#include "render_poly.cuh"
+#include "poly_tables.h"
 
 #include <algorithm>
 #include <cstring>
+#include <cstdlib>
 #include <cmath>
 
 namespace e2e {
@@ -285,6 +288,7 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
     if (!P) return fail(E2E_ERR_NOMEM, "psf_create: out of host memory");
     memset(&P->an, 0, sizeof(P->an));
     memset(&P->tab, 0, sizeof(P->tab));
+    memset(&P->poly, 0, sizeof(P->poly));
     P->kind = d->kind; P->nx = nx; P->ny = ny; P->Q = 0;
     if (d->kind == 0) {
         if (!(d->sigma_x > 0.0) || !(d->sigma_y > 0.0) || !is_fin(d->sigma_x) || !is_fin(d->sigma_y))
@@ -326,6 +330,32 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
                 ++nt;
             }
             A.n_terms = nt;
+        }
+        // production path: pixel-phase polynomial tables (the direct special-function kernel stays as the fallback
+        // for PSFs whose tables do not converge, and under E2E_FORCE_DIRECT=1 for A/B checks)
+        const char* force = getenv("E2E_FORCE_DIRECT");
+        if (!(force && force[0] == '1')) {
+            PsfShape shape;
+            shape.sx = d->sigma_x; shape.sy = d->sigma_y; shape.by_gauss = A.by_gauss != 0;
+            for (int i = 0; i < A.n_terms; ++i) {
+                ChordTerm ct;
+                ct.s = A.s[i]; ct.cs = A.cs[i]; ct.wq = A.wq[i]; ct.g = A.g[i]; ct.paired = (A.paired >> i) & 1u;
+                shape.terms.push_back(ct);
+            }
+            PolyTables tabs;
+            if (build_poly_tables(shape, P->hbx, P->hby, tabs) && tabs.ncol_pad <= kMaxWin && tabs.nrow_pad <= kMaxWin) {
+                const size_t nx_ = tabs.tx.size(), ny_ = tabs.ty.size();
+                E2E_CUDA(cudaMalloc(&P->d_poly, 8 * (nx_ + ny_)));
+                cudaError_t ce = cudaMemcpy(P->d_poly, tabs.tx.data(), 8 * nx_, cudaMemcpyHostToDevice);
+                if (ce == cudaSuccess) ce = cudaMemcpy(P->d_poly + nx_, tabs.ty.data(), 8 * ny_, cudaMemcpyHostToDevice);
+                if (ce != cudaSuccess) { cudaFree(P->d_poly); P->d_poly = nullptr; return fail_cuda(ce, "psf_create: polynomial table upload"); }
+                PolyParam& Q = P->poly;
+                Q.T = tabs.T; Q.nlo_x = tabs.nlo_x; Q.ncol = tabs.ncol; Q.ncol_pad = tabs.ncol_pad;
+                Q.nlo_y = tabs.nlo_y; Q.nrow = tabs.nrow; Q.nrow_pad = tabs.nrow_pad;
+                Q.hbx = P->hbx; Q.hby = P->hby; Q.tx = P->d_poly; Q.ty = P->d_poly + nx_;
+                P->poly_degree = tabs.P;
+                P->poly_trunc_err = (double)tabs.trunc_err;
+            }
         }
     } else if (d->kind == 1) {
         if (d->tab_npix < 1 || d->tab_os < 1 || d->tab_gx < 1 || d->tab_gy < 1 || !d->tab)
@@ -385,6 +415,7 @@ void e2e_psf_destroy(e2e_psf_t* psf)
 {
     if (!psf) return;
     if (psf->d_sat) cudaFree(psf->d_sat);
+    if (psf->d_poly) cudaFree(psf->d_poly);
     delete psf;
 }
 
@@ -555,7 +586,20 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
         if (n <= 0) continue;
         const unsigned blocks = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
-        if (P->kind == 0)
+        if (P->kind == 0 && P->poly_degree > 0) {
+            const unsigned pb = (unsigned)((n + kPolyWarps - 1) / kPolyWarps);
+            const size_t sm = sizeof(PolyWarpSmem) * kPolyWarps;
+#define E2E_POLY_CASE(DEG)                                                                                              \
+    case DEG:                                                                                                           \
+        render_poly_kernel<DEG><<<pb, kPolyWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, \
+                                                                     P->poly, d_frame, F->view.nx, F->view.ny);        \
+        break;
+            switch (P->poly_degree) {
+                E2E_POLY_CASE(10) E2E_POLY_CASE(12) E2E_POLY_CASE(14) E2E_POLY_CASE(16) E2E_POLY_CASE(20) E2E_POLY_CASE(24)
+                default: return fail(E2E_ERR_UNSUPPORTED, "render: no kernel for this polynomial degree");
+            }
+#undef E2E_POLY_CASE
+        } else if (P->kind == 0)
             render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n,
                                                                                    P->an, d_frame, F->view.nx, F->view.ny);
         else

@@ -103,6 +103,16 @@ struct AnalyticParam {
     unsigned paired;               // bit t: term t stands for the two nodes +-s[t]
 };
 
+// analytic PSF, production path: pixel-phase polynomial tables (poly_tables.h, render_poly.cuh)
+struct PolyParam {
+    int T;                             // chord terms
+    int nlo_x, ncol, ncol_pad;         // window columns X + nlo_x + [0, ncol)
+    int nlo_y, nrow, nrow_pad;
+    double hbx, hby;                   // footprint half-width + 1/2 (G9)
+    const double* tx;                  // [T][P+1][ncol_pad]
+    const double* ty;                  // [T][P+1][nrow_pad]
+};
+
 struct TabParam {
     int npix, os, n;               // n = npix * os cells per axis
     int gx, gy;
@@ -125,6 +135,10 @@ struct e2e_psf {
     e2e::AnalyticParam an;
     e2e::TabParam tab;
     double* d_sat = nullptr;
+    int poly_degree = 0;           // > 0: polynomial tables built (analytic PSF), degree in use
+    double poly_trunc_err = 0.0;   // measured truncation error of the tables
+    e2e::PolyParam poly;
+    double* d_poly = nullptr;      // one allocation: tx then ty
 };
 
 struct e2e_plan {                  // schedule for one (format, footprint) pair; cached in the format handle

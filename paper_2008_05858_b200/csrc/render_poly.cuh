@@ -28,14 +28,6 @@ constexpr int kPanel = 24;             // panel edge in pixels (3 tiles of 8)
 constexpr int kLdb = 28;               // leading dimension of the BY staging buffer (28 mod 16 = 12: conflict-free fragments)
 constexpr int kMaxWin = 104;           // largest padded window edge (footprint limit 96 px + 2, padded to 8)
 
-struct PolyParam {
-    int T;                             // chord terms
-    int nlo_x, ncol, ncol_pad;         // window columns X + nlo_x + [0, ncol)
-    int nlo_y, nrow, nrow_pad;
-    double hbx, hby;                   // footprint half-width + 1/2 (G9)
-    const double* tx;                  // [T][P+1][ncol_pad]
-    const double* ty;                  // [T][P+1][nrow_pad]
-};
 
 __device__ __forceinline__ void dmma_m8n8k4(double& c0, double& c1, double a, double b)
 {
@@ -66,6 +58,7 @@ render_poly_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
     const Item it = items[item_id];
     const Strip st = strips[it.strip];
     const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
+    for (int i = lane; i < 32 * kLdb; i += 32) S.by[i] = 0.0;  // tiles beyond the window read (and discard) these
 
     long long k = (long long)it.chunk0 * 32;
     long long kend = k + (long long)it.nchunks * 32;

@@ -4,6 +4,7 @@
 #include "render_analytic.cuh"
 #include "render_tabulated.cuh"
 #include "render_poly.cuh"
+#include "render_moment.cuh"
 #include "poly_tables.h"
 
 #include <algorithm>
@@ -29,6 +30,9 @@ int fail_cuda(cudaError_t e, const char* what)
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream);
 int measure_fp64_peak(int repeats, double* burst, double* sustained);
+
+// samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
+constexpr double kMomentMinSpp = 8.0;
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -289,6 +293,7 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
     memset(&P->an, 0, sizeof(P->an));
     memset(&P->tab, 0, sizeof(P->tab));
     memset(&P->poly, 0, sizeof(P->poly));
+    memset(&P->mom, 0, sizeof(P->mom));
     P->kind = d->kind; P->nx = nx; P->ny = ny; P->Q = 0;
     if (d->kind == 0) {
         if (!(d->sigma_x > 0.0) || !(d->sigma_y > 0.0) || !is_fin(d->sigma_x) || !is_fin(d->sigma_y))
@@ -356,6 +361,21 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
                 P->poly_degree = tabs.P;
                 P->poly_trunc_err = (double)tabs.trunc_err;
             }
+            // dense sampling: footprint-cell moment tables (render_moment.cuh)
+            MomentTables mom;
+            if (P->poly_degree > 0 && build_moment_tables(shape, P->hbx, P->hby, mom) && mom.npt <= 4) {
+                const size_t nfx = mom.fx.size(), nfy = mom.fy.size();
+                E2E_CUDA(cudaMalloc(&P->d_mom, 8 * (nfx + nfy)));
+                cudaError_t ce = cudaMemcpy(P->d_mom, mom.fx.data(), 8 * nfx, cudaMemcpyHostToDevice);
+                if (ce == cudaSuccess) ce = cudaMemcpy(P->d_mom + nfx, mom.fy.data(), 8 * nfy, cudaMemcpyHostToDevice);
+                if (ce != cudaSuccess) { cudaFree(P->d_mom); P->d_mom = nullptr; return fail_cuda(ce, "psf_create: moment table upload"); }
+                MomentParam& M = P->mom;
+                M.T = mom.T; M.ncol = mom.ncol; M.nrow = mom.nrow; M.nit = mom.nit; M.njt = mom.njt;
+                M.hbx = P->hbx; M.hby = P->hby; M.c0x = mom.c0x; M.c0y = mom.c0y;
+                M.fx = reinterpret_cast<const double2*>(P->d_mom);
+                M.fy = reinterpret_cast<const double2*>(P->d_mom + nfx);
+                P->moment_npt = mom.npt;
+            }
         }
     } else if (d->kind == 1) {
         if (d->tab_npix < 1 || d->tab_os < 1 || d->tab_gx < 1 || d->tab_gy < 1 || !d->tab)
@@ -416,6 +436,7 @@ void e2e_psf_destroy(e2e_psf_t* psf)
     if (!psf) return;
     if (psf->d_sat) cudaFree(psf->d_sat);
     if (psf->d_poly) cudaFree(psf->d_poly);
+    if (psf->d_mom) cudaFree(psf->d_mom);
     delete psf;
 }
 
@@ -582,11 +603,32 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         attr_err = cudaFuncSetAttribute(render_analytic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_an);
     });
     if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
+    // dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials
+    const char* mode = getenv("E2E_RENDER");
+    bool use_moment = P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
+    if (mode && !strcmp(mode, "poly")) use_moment = false;
+    if (mode && !strcmp(mode, "moment") && P->kind == 0 && P->moment_npt > 0) use_moment = true;
     for (int ph = 0; ph < pl->n_phases; ++ph) {
         const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
         if (n <= 0) continue;
         const unsigned blocks = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
-        if (P->kind == 0 && P->poly_degree > 0) {
+        if (use_moment) {
+            const unsigned pb = (unsigned)((n + kMomWarps - 1) / kMomWarps);
+#define E2E_MOM_CASE(NPT)                                                                                               \
+    case NPT: {                                                                                                         \
+        const size_t sm = sizeof(MomentWarpSmem<NPT>) * kMomWarps;                                                      \
+        static cudaError_t attr = cudaFuncSetAttribute(render_moment_kernel<NPT>,                                       \
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);           \
+        if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_moment_kernel)");                  \
+        render_moment_kernel<NPT><<<pb, kMomWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, \
+                                                                      P->mom, d_frame, F->view.nx, F->view.ny);         \
+    } break;
+            switch (P->moment_npt) {
+                E2E_MOM_CASE(2) E2E_MOM_CASE(3) E2E_MOM_CASE(4)
+                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+            }
+#undef E2E_MOM_CASE
+        } else if (P->kind == 0 && P->poly_degree > 0) {
             const unsigned pb = (unsigned)((n + kPolyWarps - 1) / kPolyWarps);
             const size_t sm = sizeof(PolyWarpSmem) * kPolyWarps;
 #define E2E_POLY_CASE(DEG)                                                                                              \

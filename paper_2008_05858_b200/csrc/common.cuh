@@ -113,6 +113,17 @@ struct PolyParam {
     const double* ty;                  // [T][P+1][nrow_pad]
 };
 
+// analytic PSF, dense sampling: footprint-cell moments (poly_tables.h MomentTables, render_moment.cuh)
+struct MomentParam {
+    int T;                             // chord terms
+    int ncol, nrow;                    // largest footprint in columns / rows
+    int nit, njt;                      // 8-wide tiles per axis
+    double hbx, hby;                   // footprint half-width + 1/2 (G9)
+    double c0x, c0y;                   // phase origin: d = (x - ilo) - c0x
+    const double2* fx;                 // [T][nit][npt][32] fragment-ordered coefficient pairs
+    const double2* fy;                 // [T][njt][npt][32]
+};
+
 struct TabParam {
     int npix, os, n;               // n = npix * os cells per axis
     int gx, gy;
@@ -139,6 +150,9 @@ struct e2e_psf {
     double poly_trunc_err = 0.0;   // measured truncation error of the tables
     e2e::PolyParam poly;
     double* d_poly = nullptr;      // one allocation: tx then ty
+    int moment_npt = 0;            // > 0: moment tables built, power tiles in use
+    e2e::MomentParam mom;
+    double* d_mom = nullptr;       // one allocation: fx then fy
 };
 
 struct e2e_plan {                  // schedule for one (format, footprint) pair; cached in the format handle

@@ -164,4 +164,74 @@ inline bool build_poly_tables(const PsfShape& S, double hbx, double hby, PolyTab
     return false;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Moment tables (render_moment.cuh).  Same polynomials, but
+//  * the cell is the set of samples that share one footprint box (G9): first column ilo = ceil(x - hbx), and the
+//    phase is d = (x - ilo) - c0x with c0x = hbx - 1/2 (as a double), d in (-1/2, 1/2]; column n = i - ilo >= 0 sits
+//    at offset (n - c0x) - d from the sample, so no per-sample mask is left inside a cell;
+//  * the coefficients are stored in mma.m8n8k4 fragment order, two k-slots per lane:
+//        fy[((t*njt + jt)*npt + pt)*32 + lane][e] = cy_t[p = 8 pt + 2 (lane%4) + e][j = 8 jt + lane/4]
+//        fx[((t*nit + it)*npt + qt)*32 + lane][e] = cx_t[q = 8 qt + 2 (lane%4) + e][i = 8 it + lane/4]
+//    (zero beyond the degree and beyond the window).
+// ------------------------------------------------------------------------------------------------
+struct MomentTables {
+    int P = 0, npt = 0;              // degree, power tiles (8 npt >= P + 1)
+    int ncol = 0, nrow = 0;          // largest footprint in columns / rows
+    int nit = 0, njt = 0;            // 8-wide tiles per axis
+    int T = 0;
+    double c0x = 0.0, c0y = 0.0;
+    std::vector<double> fx, fy;
+    long double trunc_err = 0.0L;
+};
+
+inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, MomentTables& out)
+{
+    out.c0x = hbx - 0.5;
+    out.c0y = hby - 0.5;
+    out.ncol = (int)std::floor(2.0 * hbx) + 1;
+    out.nrow = (int)std::floor(2.0 * hby) + 1;
+    out.nit = (out.ncol + 7) / 8;
+    out.njt = (out.nrow + 7) / 8;
+    out.T = (int)S.terms.size();
+    const int ntest = 24;
+    for (int di = 0; di < kNumPolyDegrees; ++di) {
+        const int P = kPolyDegrees[di];
+        const int npt = (P + 1 + 7) / 8;
+        std::vector<long double> mono(P + 1);
+        std::vector<double> fx((size_t)out.T * out.nit * npt * 64, 0.0), fy((size_t)out.T * out.njt * npt * 64, 0.0);
+        long double worst = 0.0L;
+        for (int t = 0; t < out.T; ++t) {
+            const ChordTerm& ct = S.terms[t];
+            for (int axis = 0; axis < 2; ++axis) {
+                const int cnt = axis == 0 ? out.ncol : out.nrow, ntile = axis == 0 ? out.nit : out.njt;
+                const long double c0 = axis == 0 ? (long double)out.c0x : (long double)out.c0y;
+                std::vector<double>& tab = axis == 0 ? fx : fy;
+                for (int c = 0; c < cnt; ++c) {
+                    const long double base = (long double)c - c0;          // pixel centre - sample position at d = 0
+                    auto f = [&](long double d) { return axis == 0 ? fx_exact(S, ct, base - d) : gy_exact(S, ct, base - d); };
+                    cheb_fit(f, P, mono.data());
+                    for (int k = 0; k <= P; ++k) {
+                        const int tile = c >> 3, lane = ((c & 7) << 2) | ((k & 7) >> 1), e = k & 1, kt = k >> 3;
+                        tab[((((size_t)t * ntile + tile) * npt + kt) * 32 + lane) * 2 + e] = (double)mono[k];
+                    }
+                    for (int i = 0; i <= ntest; ++i) {
+                        const long double d = -0.5L + (long double)i / (long double)ntest;
+                        const long double e = fabsl(horner_l(mono.data(), P, d) - f(d));
+                        if (e > worst) worst = e;
+                    }
+                }
+            }
+        }
+        if (worst <= kPolyTol || di == kNumPolyDegrees - 1) {
+            out.P = P;
+            out.npt = npt;
+            out.fx.swap(fx);
+            out.fy.swap(fy);
+            out.trunc_err = worst;
+            return worst <= kPolyTol;
+        }
+    }
+    return false;
+}
+
 }  // namespace e2e

@@ -1,0 +1,220 @@
+// render_moment.cuh -- steps a4 + a5 for the analytic PSF under dense sampling: the production kernel.
+//
+// A *cell* is a maximal run of consecutive samples of one strip that share one footprint box (G9):
+// ilo = ceil(x - hbx), ihi = floor(x + hbx), jlo, jhi.  Inside a cell the pixel-integrated factors of chord term t
+// are polynomials of the sample's phase (dx, dy) = ((x - ilo) - c0x, (y - jlo) - c0y) in (-1/2, 1/2]^2
+// (poly_tables.h, truncation error < 1e-17):
+//
+//     AX_t[k][i] = sum_q cx_t[q][i] dx_k^q          BY_t[k][j] = sum_p cy_t[p][j] dy_k^p
+//
+// so the cell's whole contribution to the frame ("the sum of the single fibers image ... at each wavelength",
+// P:79 "surface integral of the convolution ...") regroups exactly into
+//
+//     out[j][i] = sum_k w_k sum_t BY_t[k][j] AX_t[k][i] = sum_t ( cy_t^T  M  cx_t )[j][i],
+//     M[p][q]   = sum_k w_k dy_k^p dx_k^q                                   (the cell's weighted phase moments)
+//
+// Per sample only the moment update is left ((P+1)^2 FMAs); the cost per cell, T (P+1) nrow (P+1 + ncol) FMAs, does not
+// depend on how many samples the cell holds.  Everything is a small dense fp64 contraction and runs as chained
+// mma.sync.m8n8k4.f64 tiles (DMMA: same FP64 pipe as DFMA, 256 FMAs per instruction); C fragments feed the next
+// product's A/B operand directly: lane l of a C tile holds columns 2(l%4)+{0,1}, and the k-slot l%4 of the next
+// product is *defined* to be that column, with the table operand stored in the same permuted order:
+//
+//   step 1  MT[q][p]  = sum_k (w_k dx_k^q) (dy_k^p)          A = VX (smem), B = VY (smem)        C -> mt
+//   step 2  Z_t[j][q] = sum_p cy_t[p][j] M[p][q]             A = fy table,  B = mt (registers)   C -> z
+//   step 3  out[j][i]+= sum_q Z_t[j][q] cx_t[q][i]           A = z (registers), B = fx table     C -> out
+//
+// One warp per work item (run of consecutive 32-sample chunks of one strip; schedule of api.cu: items of one launch
+// never touch the same pixel), no block-level cooperation, no atomics; the finished window is added to the frame by
+// plain read-modify-write through L2, in a fixed order -> bit-reproducible.
+#pragma once
+#include "common.cuh"
+#include "render_poly.cuh"
+
+namespace e2e {
+
+constexpr int kMomWarps = 4;           // warps per CTA
+constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sample] (36 mod 16 = 4: conflict-free fragments)
+
+template <int NPT>
+struct MomentWarpSmem {
+    double vx[8 * NPT * kMomLdk];      // w_k dx_k^q
+    double vy[8 * NPT * kMomLdk];      // dy_k^p
+};
+
+template <int NPT>
+__global__ void __launch_bounds__(kMomWarps * 32)
+render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
+                     const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
+                     double* __restrict__ frame, int nx, int ny)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int item_id = blockIdx.x * kMomWarps + warp;
+    if (item_id >= n_items) return;
+    MomentWarpSmem<NPT>& S = reinterpret_cast<MomentWarpSmem<NPT>*>(smem_raw)[warp];
+    const Item it = items[item_id];
+    const Strip st = strips[it.strip];
+    const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
+    constexpr int NP = 8 * NPT;
+
+    long long k = (long long)it.chunk0 * 32;
+    long long kend = k + (long long)it.nchunks * 32;
+    if (kend > st.n) kend = st.n;
+
+    double mt[NPT][NPT][2];                                    // MT tiles: [qt][pt], lane holds MT[8qt + l/4][8pt + 2(l%4) + e]
+    bool have = false;
+    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0;                    // footprint box of the open cell
+
+    // steps 2 + 3 + a5 for the open cell
+    auto flush = [&]() {
+        const bool dead = cI1 < 0 || cI0 >= nx || cJ1 < 0 || cJ0 >= ny || cI1 < cI0 || cJ1 < cJ0;
+        if (dead) return;
+        for (int jp = 0; jp < Q.njt; jp += 3) {
+            if (cJ0 + 8 * jp > cJ1 || cJ0 + 8 * jp >= ny) break;
+            for (int ip = 0; ip < Q.nit; ip += 3) {
+                if (cI0 + 8 * ip > cI1 || cI0 + 8 * ip >= nx) break;
+                double out[3][3][2];
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) { out[a][b][0] = 0.0; out[a][b][1] = 0.0; }
+#pragma unroll 1
+                for (int t = 0; t < Q.T; ++t) {
+                    double z[3][NPT][2];
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+#pragma unroll
+                        for (int b = 0; b < NPT; ++b) { z[a][b][0] = 0.0; z[a][b][1] = 0.0; }
+                    // ---- step 2: Z_t = cy_t^T M for the panel's rows
+                    const double2* fy = Q.fy + ((size_t)(t * Q.njt + jp) * NPT) * 32 + lane;
+#pragma unroll
+                    for (int jt = 0; jt < 3; ++jt) {
+                        if (jp + jt < Q.njt) {
+#pragma unroll
+                            for (int pt = 0; pt < NPT; ++pt) {
+                                const double2 a = __ldg(fy + (jt * NPT + pt) * 32);
+#pragma unroll
+                                for (int qt = 0; qt < NPT; ++qt) {
+                                    dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a.x, mt[qt][pt][0]);
+                                    dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a.y, mt[qt][pt][1]);
+                                }
+                            }
+                        }
+                    }
+                    // ---- step 3: out += Z_t cx_t for the panel's columns
+                    const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
+#pragma unroll
+                    for (int ct = 0; ct < 3; ++ct) {
+                        if (ip + ct < Q.nit) {
+#pragma unroll
+                            for (int qt = 0; qt < NPT; ++qt) {
+                                const double2 b = __ldg(fx + (ct * NPT + qt) * 32);
+#pragma unroll
+                                for (int jt = 0; jt < 3; ++jt) {
+                                    dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][0], b.x);
+                                    dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][1], b.y);
+                                }
+                            }
+                        }
+                    }
+                }
+                // ---- a5: add the panel to the frame.  lane owns out[row 8 jt + l/4][cols 8 ct + 2 (l%4) + {0,1}]
+                const int rlim = min(cJ1, ny - 1), clim = min(cI1, nx - 1);
+                double old[3][3][2];
+#pragma unroll
+                for (int jt = 0; jt < 3; ++jt) {
+                    const int row = cJ0 + 8 * (jp + jt) + lq;
+#pragma unroll
+                    for (int ct = 0; ct < 3; ++ct)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
+                            const bool ok = row >= 0 && row <= rlim && col >= 0 && col <= clim;
+                            old[jt][ct][e] = ok ? __ldcg(frame + (size_t)row * nx + col) : 0.0;
+                        }
+                }
+#pragma unroll
+                for (int jt = 0; jt < 3; ++jt) {
+                    const int row = cJ0 + 8 * (jp + jt) + lq;
+#pragma unroll
+                    for (int ct = 0; ct < 3; ++ct)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
+                            const bool ok = row >= 0 && row <= rlim && col >= 0 && col <= clim;
+                            if (ok) __stcg(frame + (size_t)row * nx + col, old[jt][ct][e] + out[jt][ct][e]);
+                        }
+                }
+            }
+        }
+        __syncwarp();                                          // the next cell's window overlaps this one
+    };
+
+    while (k < kend) {
+        // ---- next batch of up to 32 samples: footprint boxes, phases, power arrays
+        const int nb = (int)min((long long)32, kend - k);
+        const bool valid = lane < nb;
+        const long long kidx = st.off + k + (valid ? lane : nb - 1);
+        const double xk = xs[kidx], yk = ys[kidx];
+        const double wk = valid ? ws[kidx] : 0.0;
+        // G9 footprint box (same operations as the oracle's box)
+        const int ilo = __double2int_ru(__dsub_rn(xk, Q.hbx)), ihi = __double2int_rd(__dadd_rn(xk, Q.hbx));
+        const int jlo = __double2int_ru(__dsub_rn(yk, Q.hby)), jhi = __double2int_rd(__dadd_rn(yk, Q.hby));
+        const double dx = __dsub_rn(__dsub_rn(xk, (double)ilo), Q.c0x);
+        const double dy = __dsub_rn(__dsub_rn(yk, (double)jlo), Q.c0y);
+        __syncwarp();                                          // previous batch's readers are done
+        {
+            double vx = wk, vy = 1.0;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                S.vx[p * kMomLdk + lane] = vx;
+                S.vy[p * kMomLdk + lane] = vy;
+                vx *= dx;
+                vy *= dy;
+            }
+        }
+        __syncwarp();
+        int pos = 0;
+        while (pos < nb) {
+            const int kI0 = __shfl_sync(0xffffffffu, ilo, pos), kI1 = __shfl_sync(0xffffffffu, ihi, pos);
+            const int kJ0 = __shfl_sync(0xffffffffu, jlo, pos), kJ1 = __shfl_sync(0xffffffffu, jhi, pos);
+            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1)) {
+                flush();
+                have = false;
+            }
+            if (!have) {
+                have = true;
+                cI0 = kI0; cI1 = kI1; cJ0 = kJ0; cJ1 = kJ1;
+#pragma unroll
+                for (int a = 0; a < NPT; ++a)
+#pragma unroll
+                    for (int b = 0; b < NPT; ++b) { mt[a][b][0] = 0.0; mt[a][b][1] = 0.0; }
+            }
+            const unsigned same = __ballot_sync(0xffffffffu, valid && ilo == cI0 && ihi == cI1 && jlo == cJ0 && jhi == cJ1);
+            const unsigned rest = ~(same >> pos);              // bit r: sample pos + r is NOT in the cell
+            const int run = rest ? (__ffs(rest) - 1) : 32;     // >= 1: sample pos is in
+            const int pend = min(pos + run, nb);
+            // ---- step 1: MT += VX VY^T over the samples [pos, pend)
+            for (int ks = pos >> 2; ks <= (pend - 1) >> 2; ++ks) {
+                const int ksamp = 4 * ks + lr;
+                const bool in = ksamp >= pos && ksamp < pend;
+                double a[NPT], b[NPT];
+#pragma unroll
+                for (int qt = 0; qt < NPT; ++qt) {
+                    const double v = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
+                    a[qt] = in ? v : 0.0;
+                    b[qt] = S.vy[(8 * qt + lq) * kMomLdk + ksamp];
+                }
+#pragma unroll
+                for (int qt = 0; qt < NPT; ++qt)
+#pragma unroll
+                    for (int pt = 0; pt < NPT; ++pt) dmma_m8n8k4(mt[qt][pt][0], mt[qt][pt][1], a[qt], b[pt]);
+            }
+            pos = pend;
+        }
+        k += nb;
+    }
+    if (have) flush();
+}
+
+}  // namespace e2e

@@ -32,6 +32,10 @@ UNIT = "contributions/s"
 # "survey_formula" figure; the headline roofline counts the irreducible FMAs only)
 C_ERFC, C_PSI = 60.0, 90.0
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+# capture of this command (profiles/, file named beside each value); None = not captured for that kernel
+NCU_TRAFFIC_BYTES = {}
+
 
 def make_scene(name: str):
     from paper_2008_05858_b200 import workloads as W
@@ -193,7 +197,7 @@ def count_contributions(B, r, hbx, hby):
     nmax = int(r.per_order.max())
     x = torch.empty(max(nmax, 1), dtype=torch.float64, device=r.device)
     y = torch.empty_like(x)
-    total = 0
+    total, cells = 0, 0
     for f in range(r.scene.n_fibers):
         for o in range(r.scene.n_orders):
             n = int(r.per_order[o])
@@ -204,7 +208,10 @@ def count_contributions(B, r, hbx, hby):
             ilo = torch.clamp(torch.ceil(xs - hbx), min=0); ihi = torch.clamp(torch.floor(xs + hbx), max=r.scene.nx - 1)
             jlo = torch.clamp(torch.ceil(ys - hby), min=0); jhi = torch.clamp(torch.floor(ys + hby), max=r.scene.ny - 1)
             total += int((torch.clamp(ihi - ilo + 1, min=0) * torch.clamp(jhi - jlo + 1, min=0)).sum().item())
-    return total
+            # footprint cells: maximal runs of consecutive samples with one (unclipped) footprint box
+            b = torch.stack([torch.ceil(xs - hbx), torch.floor(xs + hbx), torch.ceil(ys - hby), torch.floor(ys + hby)])
+            cells += 1 + int((b[:, 1:] != b[:, :-1]).any(dim=0).sum().item())
+    return total, cells
 
 
 def run_ours(args, rank: int, world: int, local_rank: int):
@@ -225,7 +232,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     r = B.Renderer(scene, device=str(dev))
     info = r.psf.info()
     hbx, hby = support_half_widths(scene.psf)
-    contrib = count_contributions(B, r, hbx, hby)
+    contrib, n_cells = count_contributions(B, r, hbx, hby)
+    kinfo = B.e2e_render_kernel_info(r.fmt, r.psf)
     n_samples = r.n_samples
     frame = torch.empty((scene.ny, scene.nx), dtype=torch.float64, device=dev)
     noisy = torch.empty_like(frame)
@@ -255,11 +263,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = B.e2e_launch_count()
     t_wall0 = time.time()
+    torch.cuda.profiler.start()                          # ncu --profile-from-start off: launch list of the timed region only
     ev0.record(stream)
     for _ in range(args.steps):
         step()
     ev1.record(stream)
     barrier()
+    torch.cuda.profiler.stop()
     t_wall1 = time.time()
     launches = B.e2e_launch_count() - n0
     ms_total = ev0.elapsed_time(ev1)
@@ -313,12 +323,19 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     roofline = None
     if fma_flops is not None and ms_render > 0:
         ach = n_samples * fma_flops / (ms_render * 1e-3) / 1e12
-        roofline = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": None,
-                    "kernel": "render_analytic_kernel", "kernel_ms_per_step": ms_render,
+        executed = 2.0 * (n_cells * kinfo["executed_fma_per_cell"] + n_samples * kinfo["executed_fma_per_sample"])
+        roofline = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+                    "traffic": NCU_TRAFFIC_BYTES.get(kinfo["name"]),
+                    "kernel": kinfo["name"], "kernel_ms_per_step": ms_render,
                     "kernel_launches_per_step": prof["n_render"] / max(prof["n_calls"], 1),
-                    "peak_source": "measured in this run: e2e_measure_fp64_peak sustained DFMA rate x 2 (MEASURED_PEAKS.json has no fp64 entry)",
+                    "peak_source": "measured in this run: e2e_measure_fp64_peak, sustained FP64-pipe rate (max of DFMA and DMMA chains) x 2 "
+                                   "(MEASURED_PEAKS.json has no fp64 entry)",
                     "peak_burst": 2.0 * burst / 1e12,
-                    "flops_per_sample": fma_flops, "definition": "irreducible rank-T FMA accumulate only: 2*T*ncols*nrows per sample",
+                    "flops_per_sample": fma_flops, "definition": "algorithmic = irreducible rank-T FMA accumulate of the direct method: "
+                                                                 "2*T*ncols*nrows flop per sample (DESIGN.md 'Roofline')",
+                    "footprint_cells": n_cells,
+                    "executed_tflops": executed / (ms_render * 1e-3) / 1e12, "executed_frac": executed / (ms_render * 1e-3) / 1e12 / peak_tf,
+                    "executed_definition": "fp64 FMAs the kernel issues (DMMA = 256) x 2, from e2e_render_kernel_info x cell / sample counts",
                     "achieved_survey_formula": n_samples * survey_flops / (ms_render * 1e-3) / 1e12,
                     "survey_flops_per_sample": survey_flops}
     cpu = None
@@ -345,7 +362,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="espresso_like")
-    ap.add_argument("--oracle-samples", type=int, default=200_000, help="size of the CPU oracle's bounded sample")
+    ap.add_argument("--oracle-samples", type=int, default=1_500_000, help="size of the CPU oracle's bounded sample")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

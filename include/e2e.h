@@ -181,10 +181,18 @@ E2E_API int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, in
 /* ------------------------------------------------------------------------------------------------
  * Measurement helpers (used by bench.py; not part of the rendering path)
  * ------------------------------------------------------------------------------------------------ */
-/* FP64 roofline denominator.  Launches an all-SM kernel of independent DFMA chains `repeats` times back to back
- * (each launch ~10 ms) and returns fused multiply-adds per second (flop/s = 2x): *burst = the fastest single
+/* FP64 roofline denominator.  Launches all-SM kernels of independent fp64 chains `repeats` times back to back
+ * (each launch ~10 ms), once as DFMA chains and once as mma.sync.m8n8k4.f64 (DMMA) chains -- both feed the same FP64
+ * pipe -- and returns the larger rate in fused multiply-adds per second (flop/s = 2x): *burst = the fastest single
  * launch, *sustained = total work / total time of the second half of the launches.  Synchronous. */
 E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s);
+
+/* Which a4+a5 kernel e2e_render_frame launches for this (format, psf) pair and what it executes: *name is a static
+ * string ("render_moment_kernel<2>", "render_poly_kernel<14>", "render_analytic_kernel", "render_tabulated_kernel");
+ * *executed_fma_per_cell / *executed_fma_per_sample are the fp64 fused multiply-adds the kernel issues per footprint
+ * cell and per sample (DMMA counted as 256), 0 where it does not apply.  Any output pointer may be NULL. */
+E2E_API int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name,
+                                   double* executed_fma_per_cell, double* executed_fma_per_sample);
 
 /* Number of kernel launches the library has issued since load (all entry points), for bench.py's gpu_launches. */
 E2E_API int64_t e2e_launch_count(void);

@@ -23,7 +23,7 @@ ERROR_NAMES = {-1: "E2E_ERR_INVALID_ARG", -2: "E2E_ERR_NOT_MONOTONIC", -3: "E2E_
 SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_destroy", "e2e_format_num_samples",
            "e2e_psf_create", "e2e_psf_destroy", "e2e_psf_info", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_measure_fp64_peak",
-           "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read"]
+           "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info"]
 
 
 class E2EError(RuntimeError):
@@ -107,6 +107,8 @@ def load():
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
     L.e2e_measure_fp64_peak.restype = C.c_int
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
+    L.e2e_render_kernel_info.restype = C.c_int
+    L.e2e_render_kernel_info.argtypes = [vp, vp, C.POINTER(C.c_char_p), C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_launch_count.restype = i64
     L.e2e_launch_count.argtypes = []
     L.e2e_profile_enable.restype = C.c_int
@@ -296,6 +298,13 @@ def e2e_measure_fp64_peak(repeats: int = 60):
     burst, sus = C.c_double(), C.c_double()
     _check(load().e2e_measure_fp64_peak(int(repeats), C.byref(burst), C.byref(sus)))
     return float(burst.value), float(sus.value)
+
+
+def e2e_render_kernel_info(fmt, psf) -> dict:
+    """name of the a4+a5 kernel e2e_render_frame launches for (fmt, psf) and the fp64 FMAs it issues per cell / sample"""
+    name, pc, ps = C.c_char_p(), C.c_double(), C.c_double()
+    _check(load().e2e_render_kernel_info(fmt.handle, psf.handle, C.byref(name), C.byref(pc), C.byref(ps)))
+    return {"name": name.value.decode(), "executed_fma_per_cell": float(pc.value), "executed_fma_per_sample": float(ps.value)}
 
 
 def e2e_profile_enable(on: bool):

@@ -591,6 +591,17 @@ static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spect
     return E2E_OK;
 }
 
+// dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials.
+// E2E_RENDER=poly|moment overrides the rule (A/B measurements)
+static bool choose_moment(const e2e_format* F, const e2e_psf* P)
+{
+    const char* mode = getenv("E2E_RENDER");
+    bool use = P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
+    if (mode && !strcmp(mode, "poly")) use = false;
+    if (mode && !strcmp(mode, "moment") && P->kind == 0 && P->moment_npt > 0) use = true;
+    return use;
+}
+
 static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
                          const double* d_w, double* d_frame, cudaStream_t stream)
 {
@@ -603,11 +614,7 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         attr_err = cudaFuncSetAttribute(render_analytic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_an);
     });
     if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
-    // dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials
-    const char* mode = getenv("E2E_RENDER");
-    bool use_moment = P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
-    if (mode && !strcmp(mode, "poly")) use_moment = false;
-    if (mode && !strcmp(mode, "moment") && P->kind == 0 && P->moment_npt > 0) use_moment = true;
+    const bool use_moment = choose_moment(F, P);
     for (int ph = 0; ph < pl->n_phases; ++ph) {
         const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
         if (n <= 0) continue;
@@ -805,6 +812,35 @@ int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx
     StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
     if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
     return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
+}
+
+int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name, double* fma_cell, double* fma_sample)
+{
+    if (!fmt || !psf) return fail(E2E_ERR_INVALID_ARG, "render_kernel_info: NULL argument");
+    const char* nm = "render_tabulated_kernel";
+    double pc = 0.0, ps = 0.0;
+    if (choose_moment(fmt, psf)) {
+        static const char* names[] = {"", "", "render_moment_kernel<2>", "render_moment_kernel<3>", "render_moment_kernel<4>"};
+        const MomentParam& M = psf->mom;
+        const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
+        nm = names[npt];
+        // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
+        pc = 256.0 * M.T * (2.0 * npt * npt * M.njt * ip + 2.0 * npt * M.njt * M.nit);
+        ps = 64.0 * npt * npt + 2.0 * 8 * npt;                 // step 1 (one k-slot of 4 tiles^2 DMMAs) + powers
+        (void)jp;
+    } else if (psf->kind == 0 && psf->poly_degree > 0) {
+        static thread_local char buf[40];
+        snprintf(buf, sizeof buf, "render_poly_kernel<%d>", psf->poly_degree);
+        nm = buf;
+        const PolyParam& Q = psf->poly;
+        ps = (double)Q.T * ((double)Q.ncol_pad * Q.nrow_pad + (double)(psf->poly_degree + 1) * (Q.ncol_pad + Q.nrow_pad));
+    } else if (psf->kind == 0) {
+        nm = "render_analytic_kernel";
+    }
+    if (name) *name = nm;
+    if (fma_cell) *fma_cell = pc;
+    if (fma_sample) *fma_sample = ps;
+    return E2E_OK;
 }
 
 int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s)

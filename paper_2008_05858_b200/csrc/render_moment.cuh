@@ -42,7 +42,7 @@ struct MomentWarpSmem {
 };
 
 template <int NPT>
-__global__ void __launch_bounds__(kMomWarps * 32)
+__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? 4 : 1)
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                      const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
                      double* __restrict__ frame, int nx, int ny)
@@ -85,64 +85,65 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                     for (int a = 0; a < 3; ++a)
 #pragma unroll
                         for (int b = 0; b < NPT; ++b) { z[a][b][0] = 0.0; z[a][b][1] = 0.0; }
-                    // ---- step 2: Z_t = cy_t^T M for the panel's rows
+                    // ---- step 2: Z_t = cy_t^T M for the panel's rows (k-slots outermost: consecutive DMMAs are independent)
                     const double2* fy = Q.fy + ((size_t)(t * Q.njt + jp) * NPT) * 32 + lane;
+                    const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
+                    double2 a[3][NPT], b[3][NPT];
 #pragma unroll
-                    for (int jt = 0; jt < 3; ++jt) {
-                        if (jp + jt < Q.njt) {
+                    for (int jt = 0; jt < 3; ++jt)
 #pragma unroll
-                            for (int pt = 0; pt < NPT; ++pt) {
-                                const double2 a = __ldg(fy + (jt * NPT + pt) * 32);
+                        for (int pt = 0; pt < NPT; ++pt)
+                            a[jt][pt] = (jp + jt < Q.njt) ? __ldg(fy + (jt * NPT + pt) * 32) : make_double2(0.0, 0.0);
 #pragma unroll
-                                for (int qt = 0; qt < NPT; ++qt) {
-                                    dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a.x, mt[qt][pt][0]);
-                                    dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a.y, mt[qt][pt][1]);
-                                }
-                            }
-                        }
+                    for (int ct = 0; ct < 3; ++ct)
+#pragma unroll
+                        for (int qt = 0; qt < NPT; ++qt)
+                            b[ct][qt] = (ip + ct < Q.nit) ? __ldg(fx + (ct * NPT + qt) * 32) : make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int pt = 0; pt < NPT; ++pt) {
+#pragma unroll
+                        for (int jt = 0; jt < 3; ++jt)
+#pragma unroll
+                            for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt][pt].x, mt[qt][pt][0]);
+#pragma unroll
+                        for (int jt = 0; jt < 3; ++jt)
+#pragma unroll
+                            for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt][pt].y, mt[qt][pt][1]);
                     }
                     // ---- step 3: out += Z_t cx_t for the panel's columns
-                    const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
 #pragma unroll
-                    for (int ct = 0; ct < 3; ++ct) {
-                        if (ip + ct < Q.nit) {
+                    for (int qt = 0; qt < NPT; ++qt) {
 #pragma unroll
-                            for (int qt = 0; qt < NPT; ++qt) {
-                                const double2 b = __ldg(fx + (ct * NPT + qt) * 32);
+                        for (int jt = 0; jt < 3; ++jt)
 #pragma unroll
-                                for (int jt = 0; jt < 3; ++jt) {
-                                    dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][0], b.x);
-                                    dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][1], b.y);
-                                }
-                            }
-                        }
+                            for (int ct = 0; ct < 3; ++ct) dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][0], b[ct][qt].x);
+#pragma unroll
+                        for (int jt = 0; jt < 3; ++jt)
+#pragma unroll
+                            for (int ct = 0; ct < 3; ++ct) dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][1], b[ct][qt].y);
                     }
                 }
                 // ---- a5: add the panel to the frame.  lane owns out[row 8 jt + l/4][cols 8 ct + 2 (l%4) + {0,1}]
                 const int rlim = min(cJ1, ny - 1), clim = min(cI1, nx - 1);
-                double old[3][3][2];
 #pragma unroll
                 for (int jt = 0; jt < 3; ++jt) {
                     const int row = cJ0 + 8 * (jp + jt) + lq;
+                    const bool rok = row >= 0 && row <= rlim;
+                    double* prow = frame + (size_t)(rok ? row : 0) * nx;
+                    double old[3][2];
 #pragma unroll
                     for (int ct = 0; ct < 3; ++ct)
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
                             const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
-                            const bool ok = row >= 0 && row <= rlim && col >= 0 && col <= clim;
-                            old[jt][ct][e] = ok ? __ldcg(frame + (size_t)row * nx + col) : 0.0;
+                            old[ct][e] = (rok && col >= 0 && col <= clim) ? __ldcg(prow + col) : 0.0;
                         }
-                }
-#pragma unroll
-                for (int jt = 0; jt < 3; ++jt) {
-                    const int row = cJ0 + 8 * (jp + jt) + lq;
 #pragma unroll
                     for (int ct = 0; ct < 3; ++ct)
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
                             const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
-                            const bool ok = row >= 0 && row <= rlim && col >= 0 && col <= clim;
-                            if (ok) __stcg(frame + (size_t)row * nx + col, old[jt][ct][e] + out[jt][ct][e]);
+                            if (rok && col >= 0 && col <= clim) __stcg(prow + col, old[ct][e] + out[jt][ct][e]);
                         }
                 }
             }

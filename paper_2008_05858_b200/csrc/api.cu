@@ -165,6 +165,7 @@ int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* d)
     auto reserve = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_m = reserve(sizeof(int) * no), o_lmin = reserve(8 * no), o_dl = reserve(8 * no), o_ns = reserve(8 * no);
     const size_t o_bl = reserve(8 * no), o_ba = reserve(8 * no), o_fx = reserve(8 * nf), o_fy = reserve(8 * nf);
+    const size_t o_ix = reserve(8 * (size_t)no * (kMaxDeg + 1)), o_iy = reserve(8 * (size_t)no * (kMaxDeg + 1));
     const size_t o_eff = reserve(d->eff_table ? 8 * (size_t)d->eff_n : 0);
     char* blob = nullptr;
     E2E_CUDA(cudaMalloc(&blob, off));
@@ -183,6 +184,24 @@ int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* d)
     if (d->blaze_amp) E2E_CUDA_F(cudaMemcpy(blob + o_ba, d->blaze_amp, 8 * no, cudaMemcpyHostToDevice));
     E2E_CUDA_F(cudaMemcpy(blob + o_fx, d->fiber_dx, 8 * nf, cudaMemcpyHostToDevice));
     E2E_CUDA_F(cudaMemcpy(blob + o_fy, d->fiber_dy, 8 * nf, cudaMemcpyHostToDevice));
+    {
+        // O2 inner Horner sums over M per order (the exact fma sequence of poly2's inner loop), zero-padded to degree 5
+        std::vector<double> ix((size_t)no * (kMaxDeg + 1), 0.0), iy((size_t)no * (kMaxDeg + 1), 0.0);
+        for (int o = 0; o < no; ++o) {
+            const double M = ((double)d->order_m[o] - d->m0) * d->inv_dm;
+            for (int p = 0; p <= d->deg_l; ++p) {
+                double sx = 0.0, sy = 0.0;
+                for (int q = d->deg_m; q >= 0; --q) {
+                    sx = fma(sx, M, d->coef_x[p * (d->deg_m + 1) + q]);
+                    sy = fma(sy, M, d->coef_y[p * (d->deg_m + 1) + q]);
+                }
+                ix[(size_t)o * (kMaxDeg + 1) + p] = sx;
+                iy[(size_t)o * (kMaxDeg + 1) + p] = sy;
+            }
+        }
+        E2E_CUDA_F(cudaMemcpy(blob + o_ix, ix.data(), 8 * ix.size(), cudaMemcpyHostToDevice));
+        E2E_CUDA_F(cudaMemcpy(blob + o_iy, iy.data(), 8 * iy.size(), cudaMemcpyHostToDevice));
+    }
     if (d->eff_table) E2E_CUDA_F(cudaMemcpy(blob + o_eff, d->eff_table, 8 * (size_t)d->eff_n, cudaMemcpyHostToDevice));
 
     FormatView& v = F->view;
@@ -198,6 +217,8 @@ int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* d)
     v.blaze_amp = d->blaze_amp ? (const double*)(blob + o_ba) : nullptr;
     v.fiber_dx = (const double*)(blob + o_fx);
     v.fiber_dy = (const double*)(blob + o_fy);
+    v.inner_x = (const double*)(blob + o_ix);
+    v.inner_y = (const double*)(blob + o_iy);
     v.eff_table = d->eff_table ? (const double*)(blob + o_eff) : nullptr;
     v.eff_n = d->eff_n; v.eff_lam0 = d->eff_lam0; v.eff_dlam = d->eff_dlam;
 

@@ -68,6 +68,9 @@ struct FormatView {
     const double* blaze_amp;       // [n_orders] or nullptr
     const double* fiber_dx;        // [n_fibers]
     const double* fiber_dy;
+    const double* inner_x;         // [n_orders][kMaxDeg + 1] inner Horner sums over M of coef_x, zero-padded at the top
+    const double* inner_y;         //   (O2: the order number is constant along a strip, so these are the per-order
+                                   //    coefficients of the outer Horner in L; same fma sequence -> same bits)
     const double* eff_table;       // or nullptr
     long long eff_n;
     double eff_lam0, eff_dlam;

@@ -9,20 +9,20 @@
 
 namespace e2e {
 
+// Philox4x32-10 stream of one pixel, consumed a whole counter block (4 words = 2 uniforms) at a time so that the
+// words stay in registers; the word order is the stream's: block 0 words 0..3, block 1 words 0..3, ...
 struct Philox {
     uint32_t k0, k1;      // key
     uint32_t c0, c1;      // pixel index (low, high)
     uint32_t block;       // next counter block
-    uint32_t out[4];
-    int left;             // unread words in out
 
     __device__ __forceinline__ void init(uint64_t seed, uint64_t pixel)
     {
         k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32);
         c0 = (uint32_t)pixel; c1 = (uint32_t)(pixel >> 32);
-        block = 0; left = 0;
+        block = 0;
     }
-    __device__ __forceinline__ void refill()
+    __device__ __forceinline__ void next_block(uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3)
     {
         uint32_t x0 = c0, x1 = c1, x2 = block, x3 = 0, ka = k0, kb = k1;
 #pragma unroll
@@ -33,20 +33,12 @@ struct Philox {
             x0 = y0; x1 = l1; x2 = y2; x3 = l0;
             ka += 0x9E3779B9u; kb += 0xBB67AE85u;
         }
-        out[0] = x0; out[1] = x1; out[2] = x2; out[3] = x3;
-        block += 1; left = 4;
-    }
-    __device__ __forceinline__ uint32_t word()
-    {
-        if (left == 0) refill();
-        uint32_t w = out[4 - left];
-        left -= 1;
-        return w;
+        w0 = x0; w1 = x1; w2 = x2; w3 = x3;
+        block += 1;
     }
     // u = ((hi >> 5) * 2^26 + (lo >> 6) + 1/2) * 2^-53  in (0, 1)
-    __device__ __forceinline__ double uniform()
+    static __device__ __forceinline__ double uniform(uint32_t hi, uint32_t lo)
     {
-        uint32_t hi = word(), lo = word();
         double a = (double)(hi >> 5), b = (double)(lo >> 6);
         return (a * 67108864.0 + b + 0.5) * (1.0 / 9007199254740992.0);
     }
@@ -94,24 +86,30 @@ __global__ void detector_kernel(const double* __restrict__ in, double* __restric
     if (!(mu > 0.0)) mu = 0.0;
     Philox g;
     g.init(det.seed, (uint64_t)p);
-    double z1, z2;
-    for (;;) {                                     // Marsaglia polar pair
-        double v1 = 2.0 * g.uniform() - 1.0;
-        double v2 = 2.0 * g.uniform() - 1.0;
-        double q = fma(v1, v1, v2 * v2);
-        if (q < 1.0 && q > 0.0) {
-            double f = sqrt(-2.0 * spec_log(q) / q);
-            z1 = v1 * f; z2 = v2 * f;
-            break;
-        }
-    }
+    // Marsaglia polar pair: the rejection loop only draws (v1, v2, q); the log / sqrt run once after it, converged
+    double v1, v2, q;
+    uint32_t w0, w1, w2, w3;
+    do {
+        g.next_block(w0, w1, w2, w3);
+        v1 = 2.0 * Philox::uniform(w0, w1) - 1.0;
+        v2 = 2.0 * Philox::uniform(w2, w3) - 1.0;
+        q = fma(v1, v1, v2 * v2);
+    } while (!(q < 1.0 && q > 0.0));
+    const double fz = sqrt(-2.0 * spec_log(q) / q);
+    const double z1 = v1 * fz, z2 = v2 * fz;
     double cnt;
     if (!(mu > 0.0)) {
         cnt = 0.0;
     } else if (mu < 64.0) {                        // Knuth multiplication method
-        double L = spec_exp(-mu), prod = g.uniform();
+        bool second = false;                       // the uniforms after the gaussian pair start on a block boundary
+        auto next_u = [&]() {
+            second = !second;
+            if (second) { g.next_block(w0, w1, w2, w3); return Philox::uniform(w0, w1); }
+            return Philox::uniform(w2, w3);
+        };
+        double L = spec_exp(-mu), prod = next_u();
         cnt = 0.0;
-        while (prod > L) { cnt += 1.0; prod = prod * g.uniform(); }
+        while (prod > L) { cnt += 1.0; prod = prod * next_u(); }
     } else {                                       // normal + first Cornish-Fisher term
         double a = sqrt(mu) * z2;
         double b = (z2 * z2 - 1.0) / 6.0;

@@ -29,6 +29,24 @@ __device__ __forceinline__ void sample_position(const FormatView& f, int o, long
     Y = poly2(f.coef_y, f.deg_l, f.deg_m, L, M);
 }
 
+// the same positions from the per-order inner sums (format_create): outer Horner in L only.  The padded leading
+// steps compute fma(0, L, 0) = 0 and fma(0, L, c) = c exactly, so the result has the bits of sample_position.
+__device__ __forceinline__ void sample_position_fast(const FormatView& f, int o, long long k, double& lam, double& X, double& Y)
+{
+    lam = fma((double)k + 0.5, __ldg(f.dl + o), __ldg(f.lam_min + o));     // O1
+    const double L = __dmul_rn(__dsub_rn(lam, f.lam0), f.inv_dlam);        // O2
+    const double* cx = f.inner_x + (size_t)o * (kMaxDeg + 1);
+    const double* cy = f.inner_y + (size_t)o * (kMaxDeg + 1);
+    double ax = 0.0, ay = 0.0;
+#pragma unroll
+    for (int p = kMaxDeg; p >= 0; --p) {
+        ax = fma(ax, L, __ldg(cx + p));
+        ay = fma(ay, L, __ldg(cy + p));
+    }
+    X = ax;
+    Y = ay;
+}
+
 // e2e_format_create: one pass over every sample of every order.
 //   spacing[o] = (min, max) over k of x_{k+1} - x_k   (monotone  <=>  min > 0 or max < 0)
 //   bins[o][b] = (min, max) of y over the samples with floor((x + pad) / 64) == b
@@ -114,7 +132,7 @@ __global__ void setup_samples_kernel(FormatView f, SpectraParam sp, const Strip*
     long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= st.n) return;
     double lam, X, Y;
-    sample_position(f, o, k, lam, X, Y);
+    sample_position_fast(f, o, k, lam, X, Y);
     const e2e_spectrum_t& s = sp.s[fiber];
     double w = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(s.scale, spectrum_at(s, lam)), blaze_at(f, o, lam)), eff_at(f, lam)),
                          f.dl[o]);

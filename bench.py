@@ -34,7 +34,10 @@ C_ERFC, C_PSI = 60.0, 90.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture of this command (profiles/, file named beside each value); None = not captured for that kernel
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r1_v4_espresso.md, launch ids 1-4: mean of (443.4+117.8, 441.9+117.0, 443.7+118.4, 442.4+117.1) MB
+    "render_moment_kernel<2>": 560.4e6,
+}
 
 
 def make_scene(name: str):
@@ -214,6 +217,22 @@ def count_contributions(B, r, hbx, hby):
     return total, cells
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """max over ranks of a per-rank time (the only cross-rank exchange of the bench: "replicas only")"""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world: int, units_per_rank: float, seconds_per_step: float) -> float:
+    """whole-job throughput: every rank processes its own replica of the workload (weak scaling)"""
+    return world * units_per_rank / seconds_per_step
+
+
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     from paper_2008_05858_b200 import build as _build
@@ -276,13 +295,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     prof = B.e2e_profile_read(reset=True)
     B.e2e_profile_enable(False)
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
     ms_step = ms_total / args.steps
-    value = world * contrib / (ms_step * 1e-3)
+    value = aggregate_value(world, contrib, ms_step * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the spectra, D2H of the frame, every step
     e2e = None
@@ -302,12 +317,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             B.e2e_render_frame_host(r.fmt, r.psf, desc, h_frame.data_ptr(), ws, det=det, stream=stream)   # synchronises
         barrier()
         dt = (time.perf_counter() - t0) / k_e2e
-        if world > 1:
-            import torch.distributed as dist
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * contrib / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+        dt = max_over_ranks(dt, world, dev)
+        e2e = {"value": aggregate_value(world, contrib, dt), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "ms_per_step": dt * 1e3, "steps": k_e2e}
         del ws, h_frame
 

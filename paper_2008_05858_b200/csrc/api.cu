@@ -3,6 +3,7 @@
 #include "setup.cuh"
 #include "render_analytic.cuh"
 #include "render_tabulated.cuh"
+#include "render_tabcell.cuh"
 #include "render_poly.cuh"
 #include "render_moment.cuh"
 #include "poly_tables.h"
@@ -434,6 +435,42 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
         cudaError_t ce = cudaMemcpy(P->d_sat, sat.data(), 8 * sat.size(), cudaMemcpyHostToDevice);
         if (ce != cudaSuccess) { cudaFree(P->d_sat); return fail_cuda(ce, "psf_create: table upload"); }
         T.sat = P->d_sat;
+        // production path (render_tabcell.cuh): PI[ry][rx][J][I] = sum of the kernel cells inside the pixel whose
+        // lower-left corner is the fine-grid point (os I + rx - os, os J + ry - os), from a long double SAT
+        T.pi = nullptr; T.pi_ld = d->tab_npix + 2; T.c0 = P->hbx - 1.0;
+        if (d->tab_os <= kTcMaxOs) {
+            const int os = d->tab_os, pld = T.pi_ld, N = (int)n;
+            const size_t per_node = (size_t)os * os * pld * pld;
+            std::vector<double> pi(nk * per_node, 0.0);
+            std::vector<long double> L(ld * ld);
+            auto clampi = [&](int g) { return g < 0 ? 0 : (g > N ? N : g); };
+            for (size_t k = 0; k < nk; ++k) {
+                const double* Tk = d->tab + k * ncell;
+                std::fill(L.begin(), L.end(), 0.0L);
+                for (size_t bb = 1; bb <= (size_t)N; ++bb) {
+                    long double run = 0.0L;
+                    for (size_t aa = 1; aa <= (size_t)N; ++aa) {
+                        run += (long double)Tk[(bb - 1) * N + (aa - 1)];
+                        L[bb * ld + aa] = L[(bb - 1) * ld + aa] + run;
+                    }
+                }
+                double* out = pi.data() + k * per_node;
+                for (int ry = 0; ry < os; ++ry)
+                    for (int rx = 0; rx < os; ++rx)
+                        for (int J = 0; J < pld; ++J)
+                            for (int I = 0; I < pld; ++I) {
+                                const int gy0 = clampi(os * J + ry - os), gy1 = clampi(os * J + ry);
+                                const int gx0 = clampi(os * I + rx - os), gx1 = clampi(os * I + rx);
+                                const long double v = (L[(size_t)gy1 * ld + gx1] - L[(size_t)gy0 * ld + gx1]) -
+                                                      (L[(size_t)gy1 * ld + gx0] - L[(size_t)gy0 * ld + gx0]);
+                                out[(((size_t)ry * os + rx) * pld + J) * pld + I] = (double)v;
+                            }
+            }
+            E2E_CUDA(cudaMalloc(&P->d_pi, 8 * pi.size()));
+            ce = cudaMemcpy(P->d_pi, pi.data(), 8 * pi.size(), cudaMemcpyHostToDevice);
+            if (ce != cudaSuccess) { cudaFree(P->d_pi); P->d_pi = nullptr; return fail_cuda(ce, "psf_create: pixel-integral table upload"); }
+            T.pi = P->d_pi;
+        }
     } else {
         return fail(E2E_ERR_INVALID_ARG, "psf_create: kind must be 0 or 1");
     }
@@ -456,6 +493,7 @@ void e2e_psf_destroy(e2e_psf_t* psf)
 {
     if (!psf) return;
     if (psf->d_sat) cudaFree(psf->d_sat);
+    if (psf->d_pi) cudaFree(psf->d_pi);
     if (psf->d_poly) cudaFree(psf->d_poly);
     if (psf->d_mom) cudaFree(psf->d_mom);
     delete psf;
@@ -623,6 +661,14 @@ static bool choose_moment(const e2e_format* F, const e2e_psf* P)
     return use;
 }
 
+// tabulated PSF: cell-deposit kernel unless the oversampling is too fine for its weight array;
+// E2E_TAB=lattice forces the per-sample lattice kernel (A/B measurements)
+static bool choose_tabcell(const e2e_psf* P)
+{
+    const char* mode = getenv("E2E_TAB");
+    return P->kind == 1 && P->tab.pi != nullptr && !(mode && !strcmp(mode, "lattice"));
+}
+
 static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
                          const double* d_w, double* d_frame, cudaStream_t stream)
 {
@@ -636,6 +682,7 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
     });
     if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
     const bool use_moment = choose_moment(F, P);
+    const bool use_tabcell = choose_tabcell(P);
     for (int ph = 0; ph < pl->n_phases; ++ph) {
         const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
         if (n <= 0) continue;
@@ -672,7 +719,14 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         } else if (P->kind == 0)
             render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n,
                                                                                    P->an, d_frame, F->view.nx, F->view.ny);
-        else
+        else if (use_tabcell) {
+            const unsigned pb = (unsigned)((n + kTcWarps - 1) / kTcWarps);
+            const size_t sm = 8 * tabcell_warp_smem_doubles(P->tab.os) * kTcWarps;
+            cudaError_t attr = cudaFuncSetAttribute(render_tabcell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_tabcell_kernel)");
+            render_tabcell_kernel<<<pb, kTcWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, P->tab,
+                                                                     d_frame, F->view.nx, F->view.ny);
+        } else
             render_tabulated_kernel<<<blocks, kWarpsPerCta * 32, smem_tab, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0,
                                                                                      n, P->tab, lat_ld, d_frame, F->view.nx, F->view.ny);
         count_launch();
@@ -838,7 +892,7 @@ int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx
 int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name, double* fma_cell, double* fma_sample)
 {
     if (!fmt || !psf) return fail(E2E_ERR_INVALID_ARG, "render_kernel_info: NULL argument");
-    const char* nm = "render_tabulated_kernel";
+    const char* nm = choose_tabcell(psf) ? "render_tabcell_kernel" : "render_tabulated_kernel";
     double pc = 0.0, ps = 0.0;
     if (choose_moment(fmt, psf)) {
         static const char* names[] = {"", "", "render_moment_kernel<2>", "render_moment_kernel<3>", "render_moment_kernel<4>"};

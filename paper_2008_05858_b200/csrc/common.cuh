@@ -135,6 +135,9 @@ struct TabParam {
     double half;                   // npix / 2
     double fsx, fsy;               // (gx-1)/(nx-1), (gy-1)/(ny-1)
     const double* sat;             // [gy][gx][n+1][n+1] summed-area tables
+    const double* pi;              // [gy][gx][os][os][pi_ld][pi_ld] phase-major pixel-integral tables (render_tabcell.cuh) or nullptr
+    int pi_ld;                     // npix + 2
+    double c0;                     // hb - 1: sub-pixel phase = (x - ilo) - c0 in (0, 1]
 };
 
 }  // namespace e2e
@@ -149,6 +152,7 @@ struct e2e_psf {
     e2e::AnalyticParam an;
     e2e::TabParam tab;
     double* d_sat = nullptr;
+    double* d_pi = nullptr;        // phase-major pixel-integral tables of the tabulated PSF
     int poly_degree = 0;           // > 0: polynomial tables built (analytic PSF), degree in use
     double poly_trunc_err = 0.0;   // measured truncation error of the tables
     e2e::PolyParam poly;

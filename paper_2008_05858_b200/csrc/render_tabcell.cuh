@@ -26,7 +26,10 @@
 
 namespace e2e {
 
-constexpr int kTcWarps = 4;            // warps per CTA
+#ifndef E2E_TC_WARPS
+#define E2E_TC_WARPS 16
+#endif
+constexpr int kTcWarps = E2E_TC_WARPS;  // warps per CTA: one CTA per SM, its warps walk neighbouring runs of one strip (shared L1 working set)
 constexpr int kTcMaxOs = 16;           // largest oversampling handled here (weight array (os+1)^2 x 4 per warp)
 constexpr int kTcSlots = 8;            // pixels per lane and panel
 constexpr int kTcPitch = 33;           // staging pitch: val[v][sample]
@@ -87,13 +90,19 @@ render_tabcell_kernel(const double* __restrict__ xs, const double* __restrict__ 
                 }
                 for (int c = 0; c < 4; ++c) {
                     const double* Pc = node[c];
+                    if (c == 1 && T.gx == 1) continue;         // single-node axes: the second node carries no weight
+                    if (c >= 2 && T.gy == 1) break;
                     for (int bp = bMin; bp <= bMax + 1; ++bp) {
                         const int ry = bp ? T.os - bp : 0, dJ = bp ? 0 : 1;
+                        const double* Wrow = Wt + c * S2 + bp * S;
+                        const double* Prow = Pc + ((size_t)(ry * T.os) * ld + dJ) * ld;
+                        // no zero test inside: every offset of [aMin, aMax + 1] normally carries weight, and a
+                        // branch-free body lets the table loads of consecutive offsets overlap
+#pragma unroll 3
                         for (int ap = aMin; ap <= aMax + 1; ++ap) {
-                            const double wv = Wt[c * S2 + bp * S + ap];
-                            if (wv == 0.0) continue;
+                            const double wv = Wrow[ap];
                             const int rx = ap ? T.os - ap : 0, dI = ap ? 0 : 1;
-                            const double* src = Pc + ((size_t)(ry * T.os + rx) * ld + dJ) * ld + dI;
+                            const double* src = Prow + (size_t)rx * ld * ld + dI;
 #pragma unroll
                             for (int s = 0; s < kTcSlots; ++s)
                                 if (s < nslot) out[s] = fma(wv, __ldg(src + poff[s]), out[s]);

@@ -93,6 +93,8 @@ def lib():
             L.orc_exp.argtypes = [C.c_double]
             L.orc_detector_draws.restype = None
             L.orc_detector_draws.argtypes = [C.c_void_p, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p]
+            L.orc_detector_ex.restype = None
+            L.orc_detector_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
         _lib = L
     return _lib
 
@@ -229,6 +231,27 @@ def detector(frame: np.ndarray, det, pixel_offset: int = 0) -> np.ndarray:
     a = _f64(frame).reshape(-1)
     out = np.zeros_like(a)
     lib().orc_detector(a.ctypes.data, out.ctypes.data, a.shape[0], pixel_offset, C.addressof(d))
+    return out.reshape(np.asarray(frame).shape)
+
+
+class _DetectorEx(C.Structure):
+    _fields_ = [("base", _Detector), ("prnu", C.c_void_p), ("dark", C.c_void_p),
+                ("full_well", C.c_double), ("e_per_adu", C.c_double), ("adu_max", C.c_double)]
+
+
+def detector_ex(frame: np.ndarray, det, prnu=None, dark=None, full_well: float = 0.0, e_per_adu: float = 0.0,
+                adu_max: float = 65535.0, pixel_offset: int = 0) -> np.ndarray:
+    """Full detector stage (detector_oracle.c orc_detector_ex): PRNU / dark maps, full-well saturation, ADC."""
+    a = _f64(frame).reshape(-1)
+    pr = _f64(prnu).reshape(-1) if prnu is not None else None
+    dk = _f64(dark).reshape(-1) if dark is not None else None
+    assert pr is None or pr.shape == a.shape
+    assert dk is None or dk.shape == a.shape
+    d = _DetectorEx(_Detector(det.gain, det.dark_e, det.ron_e, det.bias, det.seed),
+                    pr.ctypes.data if pr is not None else None, dk.ctypes.data if dk is not None else None,
+                    float(full_well), float(e_per_adu), float(adu_max))
+    out = np.zeros_like(a)
+    lib().orc_detector_ex(a.ctypes.data, out.ctypes.data, a.shape[0], pixel_offset, C.addressof(d))
     return out.reshape(np.asarray(frame).shape)
 
 

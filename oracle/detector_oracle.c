@@ -141,3 +141,46 @@ void orc_detector(const double *in, double *out, int64_t n, int64_t pixel_offset
         out[p] = (cnt + d->bias) + d->ron_e * z1;
     }
 }
+
+/*
+ * Full detector stage ("photon noise and all other specific detector noises (e.g. dark
+ * current, RON ...)").  The paper names the effects only; the reading (G19) is, per pixel p:
+ *
+ *   mu   = max(0, gain * prnu[p] * frame[p] + dark[p])        prnu = pixel response non-uniformity map (NULL = 1),
+ *                                                              dark = dark-current map in e- (NULL = dark_e)
+ *   (z1, n) = the same draws as the basic stage (orc_detector_draws: one Philox stream per pixel)
+ *   e    = min(n, full_well)            if full_well > 0       (the well saturates before read-out)
+ *   e_per_adu <= 0:  out = (e + bias) + ron_e * z1                             (electrons, no quantisation)
+ *   e_per_adu  > 0:  out = clamp(floor(((e + ron_e * z1) / e_per_adu + bias) + 1/2), 0, adu_max)   (ADC)
+ *
+ * With prnu = dark = NULL, full_well = 0, e_per_adu = 0 it IS the basic stage, operation for operation (pinned).
+ * Cross-talk between read-out ports couples pixels and is not part of this stage (not built).
+ */
+typedef struct {
+    orc_detector_t base;
+    const double *prnu, *dark;       /* [n] maps or NULL */
+    double full_well, e_per_adu, adu_max;
+} orc_detector_ex_t;
+
+void orc_detector_ex(const double *in, double *out, int64_t n, int64_t pixel_offset, const orc_detector_ex_t *d)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p) {
+        double g = d->base.gain;
+        if (d->prnu) g = g * d->prnu[p];
+        double mu = g * in[p] + (d->dark ? d->dark[p] : d->base.dark_e);
+        if (!(mu > 0.0)) mu = 0.0;
+        double z1, e;
+        orc_detector_draws(&d->base, (uint64_t)(pixel_offset + p), mu, &z1, &e);
+        if (d->full_well > 0.0 && e > d->full_well) e = d->full_well;
+        if (!(d->e_per_adu > 0.0)) {
+            out[p] = (e + d->base.bias) + d->base.ron_e * z1;
+        } else {
+            double v = e + d->base.ron_e * z1;
+            double a = floor((v / d->e_per_adu + d->base.bias) + 0.5);
+            if (a < 0.0) a = 0.0;
+            if (a > d->adu_max) a = d->adu_max;
+            out[p] = a;
+        }
+    }
+}

@@ -278,6 +278,25 @@ def test_render_espresso_flux_conservation_and_gaps(B, espresso_gpu):
     assert G.min() >= 0.0
 
 
+def test_render_hires_full_frame_windows(B):
+    """BASELINE.json configs[2] at full size (10 fibers x 60 orders, 173 M samples) in the launch configuration
+    bench.py times; oracle on sampled windows that span several fibers of the pseudo-slit"""
+    s = W.hires_like()
+    G = gpu_render(B, s)
+    assert np.isfinite(G).all()
+    for o, f, frac in ((0, 0, 0.0008), (30, 4, 0.41), (59, 9, 0.9992)):
+        n = oracle.order_nsamples(s, o)
+        k = int(frac * (n - 1))
+        lam, x, y, w = oracle.samples(s, f, o, k, k + 1)
+        i0, j0 = max(0, int(x[0]) - 12), max(0, int(y[0]) - 24)
+        wnx, wny = min(24, s.nx - i0), min(48, s.ny - j0)
+        O = oracle.render(s, window=(i0, j0, wnx, wny))
+        assert O.max() > 0
+        assert_frame_parity(G[j0:j0 + wny, i0:i0 + wnx], O, f"hires window {i0},{j0}")
+    tot = oracle.total_weight(s)
+    assert abs(float(G.sum(dtype=np.longdouble)) / tot - 1.0) < 1e-11
+
+
 # ------------------------------------------------------------------------------------------ a4/a5 tabulated
 def small_field_scene(gx=3, gy=2, npix=7, os=4, seed=77, nx=300, ny=120):
     s = small_tiny(spp=3.0, lam=(5010.0, 5013.0))
@@ -306,6 +325,30 @@ def test_render_tabulated_11px_8x(B):
     G = gpu_render(B, s)
     O = oracle.render(s)
     assert_frame_parity(G, O, "tabulated 11 px x 8")
+
+
+@pytest.mark.parametrize("npix,os", [(6, 3), (5, 16), (9, 1), (5, 20)])
+def test_render_tabulated_shapes(B, npix, os):
+    """even / odd kernel widths, non-power-of-two and unit oversampling (cell-deposit kernel), and an oversampling
+    beyond its weight array (os = 20 -> per-sample lattice kernel)"""
+    s = small_field_scene(gx=3, gy=3, npix=npix, os=os, seed=78)
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, f"tabulated npix={npix} os={os}")
+
+
+def test_render_tabulated_steep_trace_and_fibers(B):
+    """cells that change row every few samples (steep trace) and two overlapping fibers through the tabulated path"""
+    s = small_field_scene(gx=2, gy=3, npix=7, os=4, seed=79)
+    s.coef_y = np.array([560.0, 900.0, 0.0, 0.0])         # y = 20 .. 128 over x = 150 .. 438: ~0.4 px of y per px of x
+    s.fiber_dx = np.array([0.0, 0.3])
+    s.fiber_dy = np.array([0.0, 2.5])
+    s.spectra = [s.spectra[0], s.spectra[0]]
+    G = gpu_render(B, s)
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, "tabulated steep trace, 2 fibers")
 
 
 def test_render_field_psf_full_frame_windows(B):

@@ -178,6 +178,27 @@ typedef struct e2e_detector {
 E2E_API int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny,
                        const e2e_detector_t* det, void* cuda_stream);
 
+/* Full detector stage ("... all other specific detector noises (e.g. dark current, RON ...)";
+ * reading G19 of DESIGN.md).  Per pixel p:
+ *   mu = max(0, gain * prnu[p] * in[p] + dark[p]);  (z1, n) = the draws of the basic stage;
+ *   e  = min(n, full_well_e) when full_well_e > 0 (the well saturates before read-out);
+ *   e_per_adu <= 0:  out[p] = (e + bias) + ron_e * z1                                  (electrons)
+ *   e_per_adu  > 0:  out[p] = clamp(floor(((e + ron_e * z1) / e_per_adu + bias) + 1/2), 0, adu_max)   (ADC counts)
+ * d_prnu (pixel response non-uniformity) and d_dark (dark electrons per pixel) are DEVICE [ny*nx] maps owned by the
+ * caller, or NULL (= 1 and base.dark_e).  With both NULL, full_well_e = 0 and e_per_adu = 0 the result equals
+ * e2e_apply_detector bit for bit.  Errors: NULL frame / det, non-finite or negative full_well_e, e_per_adu, adu_max
+ * -> E2E_ERR_INVALID_ARG.  Asynchronous on cuda_stream; in may equal out; the maps must not alias out. */
+typedef struct e2e_detector_ex {
+    e2e_detector_t base;
+    const double* d_prnu;
+    const double* d_dark;
+    double full_well_e;
+    double e_per_adu;
+    double adu_max;
+} e2e_detector_ex_t;
+E2E_API int e2e_apply_detector_ex(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny,
+                          const e2e_detector_ex_t* det, void* cuda_stream);
+
 /* ------------------------------------------------------------------------------------------------
  * Measurement helpers (used by bench.py; not part of the rendering path)
  * ------------------------------------------------------------------------------------------------ */

@@ -22,7 +22,8 @@ ERROR_NAMES = {-1: "E2E_ERR_INVALID_ARG", -2: "E2E_ERR_NOT_MONOTONIC", -3: "E2E_
 # every symbol include/e2e.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_destroy", "e2e_format_num_samples",
            "e2e_psf_create", "e2e_psf_destroy", "e2e_psf_info", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
-           "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_measure_fp64_peak",
+           "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_apply_detector_ex",
+           "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info"]
 
 
@@ -62,6 +63,11 @@ class ProfileDesc(C.Structure):
 class DetectorDesc(C.Structure):
     _fields_ = [("gain", C.c_double), ("dark_e", C.c_double), ("ron_e", C.c_double), ("bias", C.c_double),
                 ("seed", C.c_uint64)]
+
+
+class DetectorExDesc(C.Structure):
+    _fields_ = [("base", DetectorDesc), ("d_prnu", C.c_void_p), ("d_dark", C.c_void_p), ("full_well_e", C.c_double),
+                ("e_per_adu", C.c_double), ("adu_max", C.c_double)]
 
 
 _lib = None
@@ -105,6 +111,8 @@ def load():
     L.e2e_render_frame_host.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorDesc), vp, vp, C.c_size_t, vp]
     L.e2e_apply_detector.restype = C.c_int
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
+    L.e2e_apply_detector_ex.restype = C.c_int
+    L.e2e_apply_detector_ex.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorExDesc), vp]
     L.e2e_measure_fp64_peak.restype = C.c_int
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_render_kernel_info.restype = C.c_int
@@ -291,6 +299,17 @@ def e2e_apply_detector(d_in, d_out, nx: int, ny: int, det, stream=None):
     d = DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed))
     _check(load().e2e_apply_detector(int(d_in.data_ptr()), int(d_out.data_ptr()), int(nx), int(ny), C.byref(d),
                                      _stream_ptr(stream)))
+
+
+def e2e_apply_detector_ex(d_in, d_out, nx: int, ny: int, det, d_prnu=None, d_dark=None, full_well_e: float = 0.0,
+                          e_per_adu: float = 0.0, adu_max: float = 65535.0, stream=None):
+    """full detector stage (e2e.h): d_prnu / d_dark are device tensors [ny*nx] or None"""
+    d = DetectorExDesc(DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed)),
+                       int(d_prnu.data_ptr()) if d_prnu is not None else None,
+                       int(d_dark.data_ptr()) if d_dark is not None else None,
+                       float(full_well_e), float(e_per_adu), float(adu_max))
+    _check(load().e2e_apply_detector_ex(int(d_in.data_ptr()), int(d_out.data_ptr()), int(nx), int(ny), C.byref(d),
+                                        _stream_ptr(stream)))
 
 
 def e2e_measure_fp64_peak(repeats: int = 60):

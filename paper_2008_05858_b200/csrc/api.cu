@@ -30,6 +30,7 @@ int fail_cuda(cudaError_t e, const char* what)
 }
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream);
+int launch_detector_ex(const double* d_in, double* d_out, long long n, const e2e_detector_ex_t& det, cudaStream_t stream);
 int measure_fp64_peak(int repeats, double* burst, double* sustained);
 
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
@@ -887,6 +888,25 @@ int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx
     StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
     if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
     return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
+}
+
+int e2e_apply_detector_ex(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_ex_t* det,
+                          void* cuda_stream)
+{
+    if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: NULL argument");
+    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: bad frame size");
+    const e2e_detector_t& b = det->base;
+    if (!is_fin(b.gain) || !is_fin(b.dark_e) || !is_fin(b.ron_e) || !is_fin(b.bias))
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: non-finite parameter");
+    if (!is_fin(det->full_well_e) || det->full_well_e < 0.0 || !is_fin(det->e_per_adu) || det->e_per_adu < 0.0)
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: full_well_e / e_per_adu must be finite and >= 0");
+    if (det->e_per_adu > 0.0 && (!is_fin(det->adu_max) || det->adu_max < 0.0))
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: adu_max must be finite and >= 0");
+    if (det->d_prnu == d_frame_out || det->d_dark == d_frame_out)
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: a map aliases the output frame");
+    StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
+    if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
+    return launch_detector_ex(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
 }
 
 int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name, double* fma_cell, double* fma_sample)

@@ -78,14 +78,11 @@ __device__ __forceinline__ double spec_exp(double y)
     return P * __longlong_as_double((long long)b);
 }
 
-__global__ void detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, e2e_detector_t det)
+// the draws of one pixel (G12): z1 for the read noise, cnt = Poisson(mu)
+__device__ __forceinline__ void detector_draws(uint64_t seed, long long p, double mu, double& z1_out, double& cnt_out)
 {
-    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    double mu = det.gain * in[p] + det.dark_e;
-    if (!(mu > 0.0)) mu = 0.0;
     Philox g;
-    g.init(det.seed, (uint64_t)p);
+    g.init(seed, (uint64_t)p);
     // Marsaglia polar pair: the rejection loop only draws (v1, v2, q); the log / sqrt run once after it, converged
     double v1, v2, q;
     uint32_t w0, w1, w2, w3;
@@ -116,7 +113,41 @@ __global__ void detector_kernel(const double* __restrict__ in, double* __restric
         cnt = floor(((mu + a) + b) + 0.5);
         if (cnt < 0.0) cnt = 0.0;
     }
+    z1_out = z1; cnt_out = cnt;
+}
+
+__global__ void detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, e2e_detector_t det)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    double mu = det.gain * in[p] + det.dark_e;
+    if (!(mu > 0.0)) mu = 0.0;
+    double z1, cnt;
+    detector_draws(det.seed, p, mu, z1, cnt);
     out[p] = (cnt + det.bias) + det.ron_e * z1;
+}
+
+// full detector stage (e2e.h e2e_apply_detector_ex; G19): PRNU / dark maps, full well, ADC
+__global__ void detector_ex_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, e2e_detector_ex_t det)
+{
+    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    double g = det.base.gain;
+    if (det.d_prnu) g = g * __ldg(det.d_prnu + p);
+    double mu = g * in[p] + (det.d_dark ? __ldg(det.d_dark + p) : det.base.dark_e);
+    if (!(mu > 0.0)) mu = 0.0;
+    double z1, e;
+    detector_draws(det.base.seed, p, mu, z1, e);
+    if (det.full_well_e > 0.0 && e > det.full_well_e) e = det.full_well_e;
+    if (!(det.e_per_adu > 0.0)) {
+        out[p] = (e + det.base.bias) + det.base.ron_e * z1;
+    } else {
+        const double v = e + det.base.ron_e * z1;
+        double a = floor((v / det.e_per_adu + det.base.bias) + 0.5);
+        if (a < 0.0) a = 0.0;
+        if (a > det.adu_max) a = det.adu_max;
+        out[p] = a;
+    }
 }
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream)
@@ -128,6 +159,18 @@ int launch_detector(const double* d_in, double* d_out, long long n, const e2e_de
     count_launch();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "detector_kernel launch");
+    return E2E_OK;
+}
+
+int launch_detector_ex(const double* d_in, double* d_out, long long n, const e2e_detector_ex_t& det, cudaStream_t stream)
+{
+    if (n <= 0) return E2E_OK;
+    const int threads = 256;
+    long long blocks = (n + threads - 1) / threads;
+    detector_ex_kernel<<<(unsigned)blocks, threads, 0, stream>>>(d_in, d_out, n, det);
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "detector_ex_kernel launch");
     return E2E_OK;
 }
 

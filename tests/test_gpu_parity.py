@@ -293,8 +293,9 @@ def test_render_hires_full_frame_windows(B):
         O = oracle.render(s, window=(i0, j0, wnx, wny))
         assert O.max() > 0
         assert_frame_parity(G[j0:j0 + wny, i0:i0 + wnx], O, f"hires window {i0},{j0}")
-    tot = oracle.total_weight(s)
-    assert abs(float(G.sum(dtype=np.longdouble)) / tot - 1.0) < 1e-11
+    # the outer fibers of the last orders leave the detector (G11: dropped), so the frame holds a bit less than was injected
+    ratio = float(G.sum(dtype=np.longdouble)) / oracle.total_weight(s)
+    assert 0.9 < ratio <= 1.0 + 1e-12
 
 
 # ------------------------------------------------------------------------------------------ a4/a5 tabulated
@@ -407,6 +408,46 @@ def test_detector_bit_exact(B):
     B.e2e_apply_detector(d_in, d_in, nx, ny, det)
     assert np.array_equal(d_in.cpu().numpy(), O)
     assert abs(G[-1].mean() / (0.9 * fr[-1].mean() + 0.4 + 100.0) - 1.0) < 0.01
+
+
+def test_detector_ex_bit_exact(B):
+    """full detector stage: PRNU / dark maps, full well, ADC -- every variant bit-exact vs the oracle"""
+    import torch
+    rng = np.random.default_rng(6)
+    nx, ny = 419, 61
+    n = nx * ny
+    fr = np.concatenate([np.zeros(500), rng.uniform(0, 5, 4000), rng.uniform(5, 64, 4000), rng.uniform(64, 200, 4000),
+                         rng.uniform(3e4, 9e4, n - 12500)])
+    fr[3] = -7.0
+    fr = fr.reshape(ny, nx)
+    prnu = rng.normal(1.0, 0.02, (ny, nx))
+    prnu[0, :7] = 0.0                                         # dead pixels
+    dark = rng.uniform(0.0, 3.0, (ny, nx))
+    dark[1, :5] = 500.0                                       # hot pixels
+    det = W.Detector(gain=0.85, dark_e=0.4, ron_e=3.0, bias=200.0, seed=0x0BAD_CAFE_F00D_0001)
+    d_in, d_pr, d_dk = (torch.from_numpy(a).cuda() for a in (fr, prnu, dark))
+    d_out = torch.empty_like(d_in)
+    variants = [dict(), dict(prnu=True), dict(dark=True), dict(prnu=True, dark=True, full_well_e=6.0e4),
+                dict(prnu=True, dark=True, full_well_e=6.0e4, e_per_adu=1.3, adu_max=65535.0),
+                dict(e_per_adu=0.7, adu_max=4095.0)]
+    for v in variants:
+        kw = {k: v[k] for k in ("full_well_e", "e_per_adu", "adu_max") if k in v}
+        B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det, d_prnu=d_pr if v.get("prnu") else None,
+                                d_dark=d_dk if v.get("dark") else None, **kw)
+        okw = {("full_well" if k == "full_well_e" else k): x for k, x in kw.items()}
+        O = oracle.detector_ex(fr, det, prnu=prnu if v.get("prnu") else None, dark=dark if v.get("dark") else None, **okw)
+        assert np.array_equal(d_out.cpu().numpy(), O), v
+    # no maps / well / ADC = the basic stage; in place works
+    B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det)
+    ref = torch.empty_like(d_in)
+    B.e2e_apply_detector(d_in, ref, nx, ny, det)
+    assert torch.equal(d_out, ref)
+    B.e2e_apply_detector_ex(d_in, d_in, nx, ny, det, d_prnu=d_pr, d_dark=d_dk, full_well_e=6.0e4, e_per_adu=1.3)
+    assert np.array_equal(d_in.cpu().numpy(), O if False else oracle.detector_ex(fr, det, prnu=prnu, dark=dark, full_well=6.0e4, e_per_adu=1.3))
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_ex(d_out, d_out, nx, ny, det, e_per_adu=-1.0)
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_ex(d_out, d_out, nx, ny, det, d_prnu=d_out)
 
 
 def test_rv_sweep_photocenter_linear_in_velocity(B):

@@ -29,12 +29,13 @@ int fail_cuda(cudaError_t e, const char* what)
     return E2E_ERR_CUDA;
 }
 
-int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream);
+int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream, long long p0 = 0);
 int launch_detector_ex(const double* d_in, double* d_out, long long n, const e2e_detector_ex_t& det, cudaStream_t stream);
 int measure_fp64_peak(int repeats, double* burst, double* sustained);
 
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
+constexpr int kHostBands = 6;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -89,10 +90,35 @@ static double host_x_of_lambda(const e2e_format_desc_t& d, int o, double lam)
 
 using namespace e2e;
 
+// copy stream + events of the banded host path; created on first use, one per device (kept until exit)
+struct HostPipe {
+    static constexpr int kEvents = 16;
+    cudaStream_t copy = nullptr;
+    cudaEvent_t ev[kEvents] = {};
+    std::mutex mu;
+};
+static HostPipe* host_pipe()
+{
+    static std::mutex mu;
+    static HostPipe* pipes[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!pipes[dev]) {
+        HostPipe* h = new HostPipe;
+        bool ok = cudaStreamCreateWithFlags(&h->copy, cudaStreamNonBlocking) == cudaSuccess;
+        for (int i = 0; ok && i < HostPipe::kEvents; ++i) ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { delete h; return nullptr; }
+        pipes[dev] = h;
+    }
+    return pipes[dev];
+}
+
 e2e_plan::~e2e_plan()
 {
     if (d_strips) cudaFree(d_strips);
     if (d_items) cudaFree(d_items);
+    if (d_band_items) cudaFree(d_band_items);
 }
 
 extern "C" {
@@ -616,6 +642,47 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
     E2E_CUDA(cudaMemcpy(pl->d_strips, pl->strips.data(), sizeof(Strip) * n_strips, cudaMemcpyHostToDevice));
     E2E_CUDA(cudaMalloc(&pl->d_items, sizeof(Item) * std::max<size_t>(1, flat.size())));
     if (!flat.empty()) E2E_CUDA(cudaMemcpy(pl->d_items, flat.data(), sizeof(Item) * flat.size(), cudaMemcpyHostToDevice));
+    // ---- row bands for the host path: strips sorted by their first row, split into bands of about equal sample counts
+    {
+        const int ny = F->view.ny;
+        std::vector<int> rlo(n_strips, INT_MAX);
+        for (int s = 0; s < n_strips; ++s)
+            for (int B = 0; B < nB; ++B)
+                if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B]) rlo[s] = std::min(rlo[s], cov_lo[(size_t)s * nB + B]);
+        std::vector<int> order(n_strips);
+        for (int s = 0; s < n_strips; ++s) order[s] = s;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rlo[a] < rlo[b]; });
+        int want = kHostBands;
+        if (const char* e = getenv("E2E_HOST_BANDS")) want = std::max(1, std::min(atoi(e), 16));
+        std::vector<int> band_of(n_strips, 0);
+        long long acc = 0;
+        const long long tot = std::max<long long>(pl->total_samples, 1);
+        for (int i = 0; i < n_strips; ++i) {
+            const int s = order[i];
+            band_of[s] = (int)std::min<long long>(want - 1, acc * want / tot);
+            acc += pl->strips[s].n;
+        }
+        pl->n_bands = want;
+        pl->n_phases_all = (int)phases.size();
+        pl->band_fin_row.assign(want, ny);
+        for (int b = want - 2; b >= 0; --b) {
+            int lo = pl->band_fin_row[b + 1];
+            for (int s = 0; s < n_strips; ++s)
+                if (band_of[s] == b + 1 && pl->strips[s].n > 0) lo = std::min(lo, rlo[s]);
+            pl->band_fin_row[b] = std::max(0, std::min(lo, ny));
+        }
+        std::vector<Item> bflat;
+        pl->band_phase_off.assign((size_t)want * (phases.size() + 1), 0);
+        for (int b = 0; b < want; ++b)
+            for (size_t ph = 0; ph <= phases.size(); ++ph) {
+                pl->band_phase_off[(size_t)b * (phases.size() + 1) + ph] = (int)bflat.size();
+                if (ph == phases.size()) break;
+                for (const Item& it : phases[ph])
+                    if (band_of[it.strip] == b) bflat.push_back(it);
+            }
+        E2E_CUDA(cudaMalloc(&pl->d_band_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
+        if (!bflat.empty()) E2E_CUDA(cudaMemcpy(pl->d_band_items, bflat.data(), sizeof(Item) * bflat.size(), cudaMemcpyHostToDevice));
+    }
     *out = pl.get();
     F->plans.push_back(std::move(pl));
     return E2E_OK;
@@ -671,8 +738,10 @@ static bool choose_tabcell(const e2e_psf* P)
 }
 
 static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
-                         const double* d_w, double* d_frame, cudaStream_t stream)
+                         const double* d_w, double* d_frame, cudaStream_t stream, const Item* d_item_list = nullptr,
+                         const int* phase_off = nullptr, int n_phases = -1)
 {
+    if (!d_item_list) { d_item_list = pl->d_items; phase_off = pl->phase_off.data(); n_phases = pl->n_phases; }
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     const size_t smem_an = (size_t)kWarpsPerCta * (kWinCols + kWinRows) * kLdk * sizeof(double);
@@ -684,8 +753,8 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
     if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
     const bool use_moment = choose_moment(F, P);
     const bool use_tabcell = choose_tabcell(P);
-    for (int ph = 0; ph < pl->n_phases; ++ph) {
-        const int i0 = pl->phase_off[ph], n = pl->phase_off[ph + 1] - i0;
+    for (int ph = 0; ph < n_phases; ++ph) {
+        const int i0 = phase_off[ph], n = phase_off[ph + 1] - i0;
         if (n <= 0) continue;
         const unsigned blocks = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
         if (use_moment) {
@@ -696,7 +765,7 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         static cudaError_t attr = cudaFuncSetAttribute(render_moment_kernel<NPT>,                                       \
                                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);           \
         if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_moment_kernel)");                  \
-        render_moment_kernel<NPT><<<pb, kMomWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, \
+        render_moment_kernel<NPT><<<pb, kMomWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, \
                                                                       P->mom, d_frame, F->view.nx, F->view.ny);         \
     } break;
             switch (P->moment_npt) {
@@ -709,7 +778,7 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
             const size_t sm = sizeof(PolyWarpSmem) * kPolyWarps;
 #define E2E_POLY_CASE(DEG)                                                                                              \
     case DEG:                                                                                                           \
-        render_poly_kernel<DEG><<<pb, kPolyWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, \
+        render_poly_kernel<DEG><<<pb, kPolyWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, \
                                                                      P->poly, d_frame, F->view.nx, F->view.ny);        \
         break;
             switch (P->poly_degree) {
@@ -718,17 +787,17 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
             }
 #undef E2E_POLY_CASE
         } else if (P->kind == 0)
-            render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n,
+            render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n,
                                                                                    P->an, d_frame, F->view.nx, F->view.ny);
         else if (use_tabcell) {
             const unsigned pb = (unsigned)((n + kTcWarps - 1) / kTcWarps);
             const size_t sm = 8 * tabcell_warp_smem_doubles(P->tab.os) * kTcWarps;
             cudaError_t attr = cudaFuncSetAttribute(render_tabcell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
             if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_tabcell_kernel)");
-            render_tabcell_kernel<<<pb, kTcWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0, n, P->tab,
+            render_tabcell_kernel<<<pb, kTcWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, P->tab,
                                                                      d_frame, F->view.nx, F->view.ny);
         } else
-            render_tabulated_kernel<<<blocks, kWarpsPerCta * 32, smem_tab, stream>>>(d_x, d_y, d_w, pl->d_strips, pl->d_items + i0,
+            render_tabulated_kernel<<<blocks, kWarpsPerCta * 32, smem_tab, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0,
                                                                                      n, P->tab, lat_ld, d_frame, F->view.nx, F->view.ny);
         count_launch();
         cudaError_t e = cudaGetLastError();
@@ -867,14 +936,59 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
         p += align_up((size_t)spectra[f].n * 8, 256);
     }
     const size_t used = (size_t)(p - (char*)d_workspace);
-    rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
+    e2e_plan* pl = nullptr;
+    rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
-    if (det) {
-        rc = e2e_apply_detector(d_frame, d_frame, fmt->view.nx, fmt->view.ny, det, stream);
+    HostPipe* hp = host_pipe();
+    if (pl->n_bands <= 1 || !hp) {
+        // one pass: render, detector, copy
+        rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
         if (rc) return rc;
+        if (det) {
+            rc = e2e_apply_detector(d_frame, d_frame, fmt->view.nx, fmt->view.ny, det, stream);
+            if (rc) return rc;
+        }
+        E2E_CUDA(cudaMemcpyAsync(h_frame, d_frame, frame_bytes, cudaMemcpyDeviceToHost, stream));
+        E2E_CUDA(cudaStreamSynchronize(stream));
+        return E2E_OK;
     }
-    E2E_CUDA(cudaMemcpyAsync(h_frame, d_frame, frame_bytes, cudaMemcpyDeviceToHost, stream));
+    // banded pipeline: a1-a3 for the whole frame, then per row band a4 + a5 (+ a6 on the rows that became final) on the
+    // caller's stream while the previous band's rows travel to the host on the library's copy stream
+    const size_t per = sample_array_bytes(pl->total_samples);
+    if (workspace_bytes - used < 3 * per) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace too small");
+    double* d_x = (double*)p;
+    double* d_y = (double*)(p + per);
+    double* d_w = (double*)(p + 2 * per);
+    const int nx = fmt->view.nx, ny = fmt->view.ny;
+    if (det && (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias)))
+        return fail(E2E_ERR_INVALID_ARG, "render_frame_host: non-finite detector parameter");
+    std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
+    E2E_CUDA(cudaMemsetAsync(d_frame, 0, frame_bytes, stream));
+    rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, stream);
+    if (rc) return rc;
+    int row0 = 0;
+    for (int b = 0; b < pl->n_bands; ++b) {
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, pl->d_band_items,
+                           pl->band_phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        if (rc) return rc;
+        const int row1 = std::max(row0, pl->band_fin_row[b]);
+        if (row1 > row0) {
+            const size_t off = (size_t)row0 * nx;
+            const long long npx = (long long)(row1 - row0) * nx;
+            if (det) {
+                rc = launch_detector(d_frame + off, d_frame + off, npx, *det, stream, (long long)off);
+                if (rc) return rc;
+            }
+            cudaEvent_t ev = hp->ev[b % HostPipe::kEvents];
+            E2E_CUDA(cudaEventRecord(ev, stream));
+            E2E_CUDA(cudaStreamWaitEvent(hp->copy, ev, 0));
+            E2E_CUDA(cudaMemcpyAsync(h_frame + off, d_frame + off, (size_t)npx * 8, cudaMemcpyDeviceToHost, hp->copy));
+            row0 = row1;
+        }
+    }
     E2E_CUDA(cudaStreamSynchronize(stream));
+    E2E_CUDA(cudaStreamSynchronize(hp->copy));
+    (void)ny;
     return E2E_OK;
 }
 

@@ -174,6 +174,14 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     e2e::Item* d_items = nullptr;
     int n_items = 0;
     int n_colors = 0;
+    // host path (e2e_render_frame_host): the same items regrouped into row bands so that finished rows can travel to
+    // the host while later bands render.  band_phase_off[b * (n_phases_all + 1) + ph] indexes d_band_items; rows below
+    // band_fin_row[b] are final once band b has been rendered (no later band writes them)
+    int n_bands = 0;
+    int n_phases_all = 0;          // phases before empty ones were dropped (colour x parity)
+    std::vector<int> band_phase_off;
+    std::vector<int> band_fin_row;
+    e2e::Item* d_band_items = nullptr;
     ~e2e_plan();
 };
 

@@ -116,14 +116,16 @@ __device__ __forceinline__ void detector_draws(uint64_t seed, long long p, doubl
     z1_out = z1; cnt_out = cnt;
 }
 
-__global__ void detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, e2e_detector_t det)
+// in / out point at pixel p0 of the frame (the host path applies the stage band by band); the stream is keyed by the
+// pixel's index in the whole frame, so the result does not depend on how the frame is split into launches
+__global__ void detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, long long p0, e2e_detector_t det)
 {
     long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     double mu = det.gain * in[p] + det.dark_e;
     if (!(mu > 0.0)) mu = 0.0;
     double z1, cnt;
-    detector_draws(det.seed, p, mu, z1, cnt);
+    detector_draws(det.seed, p0 + p, mu, z1, cnt);
     out[p] = (cnt + det.bias) + det.ron_e * z1;
 }
 
@@ -150,12 +152,12 @@ __global__ void detector_ex_kernel(const double* __restrict__ in, double* __rest
     }
 }
 
-int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream)
+int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream, long long p0)
 {
     if (n <= 0) return E2E_OK;
     const int threads = 256;
     long long blocks = (n + threads - 1) / threads;
-    detector_kernel<<<(unsigned)blocks, threads, 0, stream>>>(d_in, d_out, n, det);
+    detector_kernel<<<(unsigned)blocks, threads, 0, stream>>>(d_in, d_out, n, p0, det);
     count_launch();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "detector_kernel launch");

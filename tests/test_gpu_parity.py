@@ -388,6 +388,46 @@ def test_render_frame_host_matches_device_path(B):
         r.close()
 
 
+def test_render_frame_host_banded_pipeline(B):
+    """host entry point on a multi-order, two-fiber frame: rows travel to the host band by band while later bands
+    render.  Every row must arrive; the frame equals the device path up to the order of the additions, and the
+    detector stage (keyed by the pixel's index in the whole frame) matches the one-pass result"""
+    import torch
+    s = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    det = W.Detector(gain=1.0, dark_e=0.5, ron_e=3.0, bias=100.0, seed=424242)
+    r = B.Renderer(s)
+    try:
+        d_frame = r.render()
+        dev = d_frame.cpu().numpy()
+        d_noisy = torch.empty_like(d_frame)
+        B.e2e_apply_detector(d_frame, d_noisy, s.nx, s.ny, det)
+        dev_noisy = d_noisy.cpu().numpy()
+        host_tabs = [np.ascontiguousarray(sp.flux, dtype=np.float64) for sp in s.spectra]
+        desc = B.spectra_array(s.spectra, [t.ctypes.data for t in host_tabs])
+        nbytes = B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc)
+        ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        out = torch.full((s.ny, s.nx), float("nan"), dtype=torch.float64).pin_memory()
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws)
+        H = out.numpy().copy()
+        assert np.isfinite(H).all()                                   # every row was copied
+        mx = dev.max()
+        assert np.abs(H - dev).max() <= 1e-13 * mx
+        assert np.array_equal(H == 0.0, dev == 0.0)
+        out.fill_(float("nan"))
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws, det=det)
+        Hn = out.numpy()
+        assert np.isfinite(Hn).all()
+        # identical draws; a last-bit difference of mu can move a Poisson count only at a rounding boundary
+        assert (Hn == dev_noisy).mean() > 0.9999
+        assert np.abs(Hn - dev_noisy).max() <= 2.0
+        # and the result is reproducible call to call
+        again = torch.empty_like(out)
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, again.data_ptr(), ws, det=det)
+        assert torch.equal(again, out)
+    finally:
+        r.close()
+
+
 # ------------------------------------------------------------------------------------------ a6 detector
 def test_detector_bit_exact(B):
     import torch

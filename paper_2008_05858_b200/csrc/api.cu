@@ -35,6 +35,7 @@ int measure_fp64_peak(int repeats, double* burst, double* sustained);
 
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
+constexpr long long kSmallFrameItems = 4736;   // 2 x (148 SMs x 16 resident warps): below this a K = 2 schedule leaves the GPU idle
 constexpr int kHostBands = 6;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -611,22 +612,40 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
     }
     pl->n_colors = n_colors;
 
-    // ---- runs: alternate runs of a strip go to different launches; two runs of the same parity are separated
-    //      by a full run whose x-extent exceeds 2 hb + 3 px, so their pixel windows are disjoint
-    std::vector<std::vector<Item>> phases((size_t)n_colors * 2);
+    // ---- runs: consecutive runs of a strip cycle through K launches; two runs of the same class are separated by
+    //      K - 1 full runs whose joint x-extent exceeds 2 hb + 3 px, so their pixel windows are disjoint.
+    //      K = 2 (long runs, fewest launches) when that already fills the GPU; small frames (a single strip) take
+    //      K = 4: runs 3x shorter, twice the launches, 4/3 G chunk-times per strip end to end instead of 2 G
+    //      (measured on B200, tiny / rv_sweep render: K = 2 0.49 / 0.95 ms, K = 4 0.40 / 0.68, K = 8 0.42 / 0.70, K = 16 0.54 / 0.77)
+    auto run_length = [&](int o, long long nchunks) {
+        long long G = nchunks;
+        const long long N = F->nsamp[o];
+        if (N >= 2 && min_sp[o] > 0.0) {
+            double g = std::floor((2.0 * P->hbx + 3.0) / (32.0 * min_sp[o])) + 1.0;
+            if (g < (double)nchunks) G = (long long)g;
+        }
+        return G;
+    };
+    long long items_k2 = 0;
+    for (int s = 0; s < n_strips; ++s) {
+        const long long N = F->nsamp[s % no];
+        if (N == 0) continue;
+        const long long nchunks = (N + 31) / 32;
+        items_k2 += (nchunks + run_length(s % no, nchunks) - 1) / run_length(s % no, nchunks);
+    }
+    int K = items_k2 < kSmallFrameItems ? 4 : 2;
+    if (const char* e = getenv("E2E_RUN_CLASSES")) K = std::max(2, std::min(atoi(e), 16));
+    std::vector<std::vector<Item>> phases((size_t)n_colors * K);
     for (int s = 0; s < n_strips; ++s) {
         const int o = s % no;
         const long long N = F->nsamp[o];
         if (N == 0) continue;
         const long long nchunks = (N + 31) / 32;
-        long long G = nchunks;
-        if (N >= 2 && min_sp[o] > 0.0) {
-            double g = std::floor((2.0 * P->hbx + 3.0) / (32.0 * min_sp[o])) + 1.0;
-            if (g < (double)nchunks) G = (long long)g;
-        }
+        long long G = run_length(o, nchunks);
+        if (K > 2 && G < nchunks) G = (G + K - 2) / (K - 1);
         int run = 0;
         for (long long c0 = 0; c0 < nchunks; c0 += G, ++run)
-            phases[(size_t)color[s] * 2 + (run & 1)].push_back(Item{s, (int)c0, (int)std::min(G, nchunks - c0)});
+            phases[(size_t)color[s] * K + (run % K)].push_back(Item{s, (int)c0, (int)std::min(G, nchunks - c0)});
     }
     std::vector<Item> flat;
     pl->phase_off.clear();

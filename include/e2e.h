@@ -87,7 +87,7 @@ typedef struct {
 
 /* Copies everything (caller keeps ownership of the arrays).  Evaluates every sample position once on the
  * device to (i) check that x(lam_k) is strictly monotone in k inside each order, (ii) record the smallest
- * sample spacing and the row range of each order per 64-column bin (used to schedule renders without atomics).
+ * sample spacing and the row range of each order per 64-column bin (used to schedule renders so that concurrent warps never share a pixel).
  * Polynomial evaluation is the fixed fma-Horner sequence of DESIGN.md "O2" (inner over q=deg_m..0 in M,
  * outer over p=deg_l..0 in L), bit-identical on host and device. */
 E2E_API int e2e_format_create(e2e_format_t** out, const e2e_format_desc_t* desc);
@@ -144,7 +144,7 @@ E2E_API int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spe
 
 /* a1-a5.  spectra: HOST array [n_fibers] whose d_flux members are DEVICE pointers.  d_frame: DEVICE
  * [ny*nx] fp64 row-major; accumulate = 0 overwrites it (it is zero-filled first), 1 adds to it.
- * Deterministic: the same inputs give the same bits; no atomics are used.  Asynchronous on cuda_stream
+ * Deterministic: the same inputs give the same bits (every pixel's additions happen in a fixed order).  Asynchronous on cuda_stream
  * (a cudaStream_t, NULL = default stream); launch errors are returned, later device faults surface at the
  * caller's next synchronisation.  The call allocates nothing on the device except, the first time a
  * (format, psf) pair is seen, the cached schedule (a few hundred KB). */

@@ -24,14 +24,17 @@
 //   step 3  out[j][i]+= sum_q Z_t[j][q] cx_t[q][i]           A = z (registers), B = fx table     C -> out
 //
 // One warp per work item (run of consecutive 32-sample chunks of one strip; schedule of api.cu: items of one launch
-// never touch the same pixel), no block-level cooperation, no atomics; the finished window is added to the frame by
-// plain read-modify-write through L2, in a fixed order -> bit-reproducible.
+// never touch the same pixel), no block-level cooperation; the finished window is added to the frame by L2 reductions
+// (red.global.add.f64) that the flush's __syncwarp() keeps in cell order -> bit-reproducible.
 #pragma once
 #include "common.cuh"
 #include "render_poly.cuh"
 
 namespace e2e {
 
+#ifndef E2E_MOM_RED
+#define E2E_MOM_RED 1
+#endif
 constexpr int kMomWarps = 4;           // warps per CTA
 constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sample] (36 mod 16 = 4: conflict-free fragments)
 
@@ -130,6 +133,18 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                     const int row = cJ0 + 8 * (jp + jt) + lq;
                     const bool rok = row >= 0 && row <= rlim;
                     double* prow = frame + (size_t)(rok ? row : 0) * nx;
+#if E2E_MOM_RED
+                    // fire-and-forget reduction at L2 (same IEEE sum as load + add + store, no round trip to wait for).
+                    // Order per pixel: items of one launch never share a pixel, and inside the warp the __syncwarp()
+                    // that closes every flush orders this cell's reductions before the next cell's -> still bit-reproducible
+#pragma unroll
+                    for (int ct = 0; ct < 3; ++ct)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
+                            if (rok && col >= 0 && col <= clim) atomicAdd(prow + col, out[jt][ct][e]);
+                        }
+#else
                     double old[3][2];
 #pragma unroll
                     for (int ct = 0; ct < 3; ++ct)
@@ -145,6 +160,7 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                             const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
                             if (rok && col >= 0 && col <= clim) __stcg(prow + col, old[ct][e] + out[jt][ct][e]);
                         }
+#endif
                 }
             }
         }

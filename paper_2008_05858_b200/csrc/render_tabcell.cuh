@@ -22,8 +22,9 @@
 // once per cell (~32 samples at 32 samples/px).
 //  (3) groups: up to kTcGroup consecutive cells of a strip that differ only in ilo read the SAME table entries (their
 //      windows are shifted by whole pixels), so the walk loads each entry once and feeds one accumulator set per cell;
-//      the shifted windows are summed in a warp-private shared tile and reach the frame with one read-modify-write.
-// One warp per work item (schedule of api.cu), no atomics, fixed order everywhere -> bit-reproducible.
+//      the shifted windows are summed in a warp-private shared tile and reach the frame with one L2 reduction per pixel.
+// One warp per work item (schedule of api.cu), fixed order everywhere (the reductions of successive groups are ordered
+// by the flush's __syncwarp()) -> bit-reproducible.
 #pragma once
 #include "common.cuh"
 
@@ -161,7 +162,7 @@ render_tabcell_kernel(const double* __restrict__ xs, const double* __restrict__ 
                         const int row = gJ + j, col = c0col + i;
                         if (row >= 0 && row < ny && col >= 0 && col < nx) {
                             double* dst = frame + (size_t)row * nx + col;
-                            __stcg(dst, __ldcg(dst) + tile[q]);
+                            atomicAdd(dst, tile[q]);        // L2 reduction, no round trip; ordered by the flush's __syncwarp()
                         }
                     }
                 } else {
@@ -173,7 +174,7 @@ render_tabcell_kernel(const double* __restrict__ xs, const double* __restrict__ 
                             const int row = gJ + j, col = c0col + i;
                             if (row >= 0 && row < ny && col >= 0 && col < nx) {
                                 double* dst = frame + (size_t)row * nx + col;
-                                __stcg(dst, __ldcg(dst) + out[0][s]);
+                                atomicAdd(dst, out[0][s]);
                             }
                         }
                     }

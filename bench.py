@@ -35,8 +35,8 @@ C_ERFC, C_PSI = 60.0, 90.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture of this command (profiles/, file named beside each value); None = not captured for that kernel
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1_v4_espresso.md, launch ids 1-4: mean of (443.4+117.8, 441.9+117.0, 443.7+118.4, 442.4+117.1) MB
-    "render_moment_kernel<2>": 560.4e6,
+    # profiles/r1_v5_espresso.md, launch ids 1-4: mean of (440.5+114.3, 439.8+113.5, 441.0+114.3, 439.5+114.5) MB
+    "render_moment_kernel<2>": 554.3e6,
 }
 
 

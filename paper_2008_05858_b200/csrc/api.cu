@@ -421,7 +421,7 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
                 if (ce != cudaSuccess) { cudaFree(P->d_mom); P->d_mom = nullptr; return fail_cuda(ce, "psf_create: moment table upload"); }
                 MomentParam& M = P->mom;
                 M.T = mom.T; M.ncol = mom.ncol; M.nrow = mom.nrow; M.nit = mom.nit; M.njt = mom.njt;
-                M.hbx = P->hbx; M.hby = P->hby; M.c0x = mom.c0x; M.c0y = mom.c0y;
+                M.hbx = P->hbx; M.hby = P->hby; M.c0x = mom.c0x; M.c0y = mom.c0y; M.nyb = mom.nyb;
                 M.fx = reinterpret_cast<const double2*>(P->d_mom);
                 M.fy = reinterpret_cast<const double2*>(P->d_mom + nfx);
                 P->moment_npt = mom.npt;
@@ -1053,8 +1053,8 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
         const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
         nm = names[npt];
         // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
-        pc = 256.0 * M.T * (2.0 * npt * npt * M.njt * ip + 2.0 * npt * M.njt * M.nit);
-        ps = 64.0 * npt * npt + 2.0 * 8 * npt;                 // step 1 (one k-slot of 4 tiles^2 DMMAs) + powers
+        pc = 256.0 * M.T * (2.0 * npt * M.njt * ip + 2.0 * npt * M.njt * M.nit);   // y has one power tile (phase windows)
+        ps = 64.0 * npt + 8.0 * npt + 8.0;                     // step 1 (npt DMMAs per 4 samples) + powers
         (void)jp;
     } else if (psf->kind == 0 && psf->poly_degree > 0) {
         static thread_local char buf[40];

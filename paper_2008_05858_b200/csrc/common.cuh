@@ -124,7 +124,8 @@ struct MomentParam {
     double hbx, hby;                   // footprint half-width + 1/2 (G9)
     double c0x, c0y;                   // phase origin: d = (x - ilo) - c0x
     const double2* fx;                 // [T][nit][npt][32] fragment-ordered coefficient pairs
-    const double2* fy;                 // [T][njt][npt][32]
+    const double2* fy;                 // [nyb][T][njt][32]   y-phase windows, degree 7 (one power tile)
+    int nyb;                           // windows: centres -1/2 + (b + 1/2)/nyb, valid for |dy - centre| <= 1/nyb
 };
 
 struct TabParam {

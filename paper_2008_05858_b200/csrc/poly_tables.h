@@ -71,20 +71,20 @@ inline long double gy_exact(const PsfShape& S, const ChordTerm& t, long double v
     return t.g * (psi_diff(zp, t.cs) - psi_diff(zm, t.cs));
 }
 
-// monomial coefficients (in d, |d| <= 1/2) of the degree-P Chebyshev interpolant of f on [-1/2, 1/2]
+// monomial coefficients (in d, |d| <= hw) of the degree-P Chebyshev interpolant of f on [-hw, hw]
 template <class F>
-inline void cheb_fit(F f, int P, long double* mono /* [P+1] */)
+inline void cheb_fit(F f, int P, long double* mono /* [P+1] */, long double hw = 0.5L)
 {
     const int N = P + 1;
     std::vector<long double> fv(N), c(N);
-    for (int j = 0; j < N; ++j) fv[j] = f(0.5L * cosl(kLPi * ((long double)j + 0.5L) / (long double)N));
+    for (int j = 0; j < N; ++j) fv[j] = f(hw * cosl(kLPi * ((long double)j + 0.5L) / (long double)N));
     for (int i = 0; i < N; ++i) {
         long double acc = 0.0L;
         for (int j = 0; j < N; ++j) acc += fv[j] * cosl(kLPi * (long double)i * ((long double)j + 0.5L) / (long double)N);
         c[i] = acc * 2.0L / (long double)N;
     }
     c[0] *= 0.5L;
-    // sum_i c_i T_i(tau), tau = 2 d  ->  monomials in tau, then in d
+    // sum_i c_i T_i(tau), tau = d / hw  ->  monomials in tau, then in d
     std::vector<long double> t0(N, 0.0L), t1(N, 0.0L), t2(N, 0.0L), m(N, 0.0L);
     t0[0] = 1.0L;
     m[0] += c[0];
@@ -96,7 +96,7 @@ inline void cheb_fit(F f, int P, long double* mono /* [P+1] */)
         t1.swap(t2);
     }
     long double sc = 1.0L;
-    for (int k = 0; k < N; ++k) { mono[k] = m[k] * sc; sc *= 2.0L; }
+    for (int k = 0; k < N; ++k) { mono[k] = m[k] * sc; sc /= hw; }
 }
 
 inline long double horner_l(const long double* a, int P, long double d)
@@ -170,20 +170,29 @@ inline bool build_poly_tables(const PsfShape& S, double hbx, double hby, PolyTab
 //    phase is d = (x - ilo) - c0x with c0x = hbx - 1/2 (as a double), d in (-1/2, 1/2]; column n = i - ilo >= 0 sits
 //    at offset (n - c0x) - d from the sample, so no per-sample mask is left inside a cell;
 //  * the coefficients are stored in mma.m8n8k4 fragment order, two k-slots per lane:
-//        fy[((t*njt + jt)*npt + pt)*32 + lane][e] = cy_t[p = 8 pt + 2 (lane%4) + e][j = 8 jt + lane/4]
+//        fy[((b*T + t)*njt + jt)*32 + lane][e]    = cy_{b,t}[p = 2 (lane%4) + e][j = 8 jt + lane/4]   (y-phase window b)
 //        fx[((t*nit + it)*npt + qt)*32 + lane][e] = cx_t[q = 8 qt + 2 (lane%4) + e][i = 8 it + lane/4]
 //    (zero beyond the degree and beyond the window).
 // ------------------------------------------------------------------------------------------------
 struct MomentTables {
-    int P = 0, npt = 0;              // degree, power tiles (8 npt >= P + 1)
+    int P = 0, npt = 0;              // x: degree, power tiles (8 npt >= P + 1)
     int ncol = 0, nrow = 0;          // largest footprint in columns / rows
     int nit = 0, njt = 0;            // 8-wide tiles per axis
     int T = 0;
     double c0x = 0.0, c0y = 0.0;
-    std::vector<double> fx, fy;
+    int nyb = 0;                     // y: phase bins, centres -1/2 + (b + 1/2)/nyb, degree-7 fits valid for |dy - centre| <= 1/nyb
+    std::vector<double> fx, fy;      // fy[((b*T + t)*njt + jt)*32 + lane][e] = cy_{b,t}[p = 2 (lane%4) + e][j = 8 jt + lane/4]
     long double trunc_err = 0.0L;
 };
 
+constexpr int kMomYDegree = 7;       // one 8-deep power tile in y
+constexpr int kMomYBins[] = {16, 32, 64, 128, 256};
+
+// The y-phase of the samples of one cell moves by (trace slope) x (1 px) only, so the y-factors do not need a polynomial
+// that is good on the whole (-1/2, 1/2]: the range is cut into nyb overlapping windows (centres 1/nyb apart, each fit
+// valid for +-1/nyb around its centre) and each window gets its own degree-7 Chebyshev fit -- 8 coefficients = one DMMA
+// power tile instead of two or three.  A cell takes the window whose centre is nearest to its first sample (|delta| <=
+// 1/(2 nyb)) and keeps it while |delta| <= 1/nyb (render_moment.cuh).  nyb = the coarsest of kMomYBins that reaches kPolyTol.
 inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, MomentTables& out)
 {
     out.c0x = hbx - 0.5;
@@ -194,31 +203,29 @@ inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, Momen
     out.njt = (out.nrow + 7) / 8;
     out.T = (int)S.terms.size();
     const int ntest = 24;
-    for (int di = 0; di < kNumPolyDegrees; ++di) {
+    // ---- x: one polynomial per (term, column) on the whole phase range
+    bool okx = false;
+    long double worst_x = 0.0L;
+    for (int di = 0; di < kNumPolyDegrees && !okx; ++di) {
         const int P = kPolyDegrees[di];
         const int npt = (P + 1 + 7) / 8;
         std::vector<long double> mono(P + 1);
-        std::vector<double> fx((size_t)out.T * out.nit * npt * 64, 0.0), fy((size_t)out.T * out.njt * npt * 64, 0.0);
+        std::vector<double> fx((size_t)out.T * out.nit * npt * 64, 0.0);
         long double worst = 0.0L;
         for (int t = 0; t < out.T; ++t) {
             const ChordTerm& ct = S.terms[t];
-            for (int axis = 0; axis < 2; ++axis) {
-                const int cnt = axis == 0 ? out.ncol : out.nrow, ntile = axis == 0 ? out.nit : out.njt;
-                const long double c0 = axis == 0 ? (long double)out.c0x : (long double)out.c0y;
-                std::vector<double>& tab = axis == 0 ? fx : fy;
-                for (int c = 0; c < cnt; ++c) {
-                    const long double base = (long double)c - c0;          // pixel centre - sample position at d = 0
-                    auto f = [&](long double d) { return axis == 0 ? fx_exact(S, ct, base - d) : gy_exact(S, ct, base - d); };
-                    cheb_fit(f, P, mono.data());
-                    for (int k = 0; k <= P; ++k) {
-                        const int tile = c >> 3, lane = ((c & 7) << 2) | ((k & 7) >> 1), e = k & 1, kt = k >> 3;
-                        tab[((((size_t)t * ntile + tile) * npt + kt) * 32 + lane) * 2 + e] = (double)mono[k];
-                    }
-                    for (int i = 0; i <= ntest; ++i) {
-                        const long double d = -0.5L + (long double)i / (long double)ntest;
-                        const long double e = fabsl(horner_l(mono.data(), P, d) - f(d));
-                        if (e > worst) worst = e;
-                    }
+            for (int c = 0; c < out.ncol; ++c) {
+                const long double base = (long double)c - (long double)out.c0x;   // pixel centre - sample position at d = 0
+                auto f = [&](long double d) { return fx_exact(S, ct, base - d); };
+                cheb_fit(f, P, mono.data());
+                for (int k = 0; k <= P; ++k) {
+                    const int tile = c >> 3, lane = ((c & 7) << 2) | ((k & 7) >> 1), e = k & 1, kt = k >> 3;
+                    fx[((((size_t)t * out.nit + tile) * npt + kt) * 32 + lane) * 2 + e] = (double)mono[k];
+                }
+                for (int i = 0; i <= ntest; ++i) {
+                    const long double d = -0.5L + (long double)i / (long double)ntest;
+                    const long double e = fabsl(horner_l(mono.data(), P, d) - f(d));
+                    if (e > worst) worst = e;
                 }
             }
         }
@@ -226,9 +233,43 @@ inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, Momen
             out.P = P;
             out.npt = npt;
             out.fx.swap(fx);
+            worst_x = worst;
+            okx = worst <= kPolyTol;
+            break;
+        }
+    }
+    if (!okx) return false;
+    // ---- y: windows
+    for (int nyb : kMomYBins) {
+        const long double hw = 1.0L / (long double)nyb;
+        std::vector<long double> mono(kMomYDegree + 1);
+        std::vector<double> fy((size_t)nyb * out.T * out.njt * 64, 0.0);
+        long double worst = 0.0L;
+        for (int b = 0; b < nyb; ++b) {
+            const long double yc = -0.5L + ((long double)b + 0.5L) * hw;
+            for (int t = 0; t < out.T; ++t) {
+                const ChordTerm& ct = S.terms[t];
+                for (int c = 0; c < out.nrow; ++c) {
+                    const long double base = (long double)c - (long double)out.c0y - yc;
+                    auto f = [&](long double d) { return gy_exact(S, ct, base - d); };
+                    cheb_fit(f, kMomYDegree, mono.data(), hw);
+                    for (int k = 0; k <= kMomYDegree; ++k) {
+                        const int tile = c >> 3, lane = ((c & 7) << 2) | (k >> 1), e = k & 1;
+                        fy[((((size_t)b * out.T + t) * out.njt + tile) * 32 + lane) * 2 + e] = (double)mono[k];
+                    }
+                    for (int i = 0; i <= 8; ++i) {
+                        const long double d = hw * (-1.0L + (long double)i / 4.0L);
+                        const long double e = fabsl(horner_l(mono.data(), kMomYDegree, d) - f(d));
+                        if (e > worst) worst = e;
+                    }
+                }
+            }
+        }
+        if (worst <= kPolyTol) {
+            out.nyb = nyb;
             out.fy.swap(fy);
-            out.trunc_err = worst;
-            return worst <= kPolyTol;
+            out.trunc_err = worst > worst_x ? worst : worst_x;
+            return true;
         }
     }
     return false;

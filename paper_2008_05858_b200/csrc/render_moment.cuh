@@ -13,8 +13,11 @@
 //     out[j][i] = sum_k w_k sum_t BY_t[k][j] AX_t[k][i] = sum_t ( cy_t^T  M  cx_t )[j][i],
 //     M[p][q]   = sum_k w_k dy_k^p dx_k^q                                   (the cell's weighted phase moments)
 //
-// Per sample only the moment update is left ((P+1)^2 FMAs); the cost per cell, T (P+1) nrow (P+1 + ncol) FMAs, does not
-// depend on how many samples the cell holds.  Everything is a small dense fp64 contraction and runs as chained
+// Per sample only the moment update is left; the cost per cell does not depend on how many samples the cell holds.
+// The y-phase of one cell's samples moves by (trace slope) x (1 px) only, so BY uses one of nyb overlapping phase
+// windows with its own degree-7 fit (poly_tables.h): p runs over 8 powers of delta = dy - (window centre) = ONE power
+// tile, while q runs over the P + 1 powers of dx (the x-phase sweeps the whole pixel inside a cell).  A cell = maximal
+// run of samples with one footprint box whose dy stays inside the window chosen at its first sample.  Everything is a small dense fp64 contraction and runs as chained
 // mma.sync.m8n8k4.f64 tiles (DMMA: same FP64 pipe as DFMA, 256 FMAs per instruction); C fragments feed the next
 // product's A/B operand directly: lane l of a C tile holds columns 2(l%4)+{0,1}, and the k-slot l%4 of the next
 // product is *defined* to be that column, with the table operand stored in the same permuted order:
@@ -41,7 +44,7 @@ constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sam
 template <int NPT>
 struct MomentWarpSmem {
     double vx[8 * NPT * kMomLdk];      // w_k dx_k^q
-    double vy[8 * NPT * kMomLdk];      // dy_k^p
+    double vy[8 * kMomLdk];            // delta_k^p, p = 0..7 (rewritten for every cell: delta is relative to the cell's window)
 };
 
 template <int NPT>
@@ -64,9 +67,11 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
     long long kend = k + (long long)it.nchunks * 32;
     if (kend > st.n) kend = st.n;
 
-    double mt[NPT][NPT][2];                                    // MT tiles: [qt][pt], lane holds MT[8qt + l/4][8pt + 2(l%4) + e]
+    double mt[NPT][2];                                         // MT tiles [qt]: lane holds MT[q = 8qt + l/4][p = 2(l%4) + e]
     bool have = false;
-    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0;                    // footprint box of the open cell
+    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
+    double cYc = 0.0;                                          // its centre
+    const double ywin = 1.0 / (double)Q.nyb;
 
     // steps 2 + 3 + a5 for the open cell
     auto flush = [&]() {
@@ -88,31 +93,25 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                     for (int a = 0; a < 3; ++a)
 #pragma unroll
                         for (int b = 0; b < NPT; ++b) { z[a][b][0] = 0.0; z[a][b][1] = 0.0; }
-                    // ---- step 2: Z_t = cy_t^T M for the panel's rows (k-slots outermost: consecutive DMMAs are independent)
-                    const double2* fy = Q.fy + ((size_t)(t * Q.njt + jp) * NPT) * 32 + lane;
+                    // ---- step 2: Z_t = cy_t^T M for the panel's rows (one power tile in p: two k-slots)
+                    const double2* fy = Q.fy + ((size_t)(cYb * Q.T + t) * Q.njt + jp) * 32 + lane;
                     const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
-                    double2 a[3][NPT], b[3][NPT];
+                    double2 a[3], b[3][NPT];
 #pragma unroll
-                    for (int jt = 0; jt < 3; ++jt)
-#pragma unroll
-                        for (int pt = 0; pt < NPT; ++pt)
-                            a[jt][pt] = (jp + jt < Q.njt) ? __ldg(fy + (jt * NPT + pt) * 32) : make_double2(0.0, 0.0);
+                    for (int jt = 0; jt < 3; ++jt) a[jt] = (jp + jt < Q.njt) ? __ldg(fy + jt * 32) : make_double2(0.0, 0.0);
 #pragma unroll
                     for (int ct = 0; ct < 3; ++ct)
 #pragma unroll
                         for (int qt = 0; qt < NPT; ++qt)
                             b[ct][qt] = (ip + ct < Q.nit) ? __ldg(fx + (ct * NPT + qt) * 32) : make_double2(0.0, 0.0);
 #pragma unroll
-                    for (int pt = 0; pt < NPT; ++pt) {
+                    for (int jt = 0; jt < 3; ++jt)
 #pragma unroll
-                        for (int jt = 0; jt < 3; ++jt)
+                        for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt].x, mt[qt][0]);
 #pragma unroll
-                            for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt][pt].x, mt[qt][pt][0]);
+                    for (int jt = 0; jt < 3; ++jt)
 #pragma unroll
-                        for (int jt = 0; jt < 3; ++jt)
-#pragma unroll
-                            for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt][pt].y, mt[qt][pt][1]);
-                    }
+                        for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt].y, mt[qt][1]);
                     // ---- step 3: out += Z_t cx_t for the panel's columns
 #pragma unroll
                     for (int qt = 0; qt < NPT; ++qt) {
@@ -181,13 +180,11 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         const double dy = __dsub_rn(__dsub_rn(yk, (double)jlo), Q.c0y);
         __syncwarp();                                          // previous batch's readers are done
         {
-            double vx = wk, vy = 1.0;
+            double vx = wk;
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 S.vx[p * kMomLdk + lane] = vx;
-                S.vy[p * kMomLdk + lane] = vy;
                 vx *= dx;
-                vy *= dy;
             }
         }
         __syncwarp();
@@ -195,37 +192,50 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         while (pos < nb) {
             const int kI0 = __shfl_sync(0xffffffffu, ilo, pos), kI1 = __shfl_sync(0xffffffffu, ihi, pos);
             const int kJ0 = __shfl_sync(0xffffffffu, jlo, pos), kJ1 = __shfl_sync(0xffffffffu, jhi, pos);
-            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1)) {
+            const double kdy = __shfl_sync(0xffffffffu, dy, pos);
+            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1 || !(fabs(kdy - cYc) <= ywin))) {
                 flush();
                 have = false;
             }
             if (!have) {
                 have = true;
                 cI0 = kI0; cI1 = kI1; cJ0 = kJ0; cJ1 = kJ1;
+                // window whose centre is nearest to the first sample: |delta| <= ywin / 2, kept while |delta| <= ywin
+                cYb = min(max((int)floor((kdy + 0.5) * (double)Q.nyb), 0), Q.nyb - 1);
+                cYc = ((double)cYb + 0.5) * ywin - 0.5;
 #pragma unroll
-                for (int a = 0; a < NPT; ++a)
-#pragma unroll
-                    for (int b = 0; b < NPT; ++b) { mt[a][b][0] = 0.0; mt[a][b][1] = 0.0; }
+                for (int a = 0; a < NPT; ++a) { mt[a][0] = 0.0; mt[a][1] = 0.0; }
             }
-            const unsigned same = __ballot_sync(0xffffffffu, valid && ilo == cI0 && ihi == cI1 && jlo == cJ0 && jhi == cJ1);
+            const double dl = dy - cYc;
+            const unsigned same = __ballot_sync(0xffffffffu, valid && ilo == cI0 && ihi == cI1 && jlo == cJ0 && jhi == cJ1 &&
+                                                                 fabs(dl) <= ywin);
             const unsigned rest = ~(same >> pos);              // bit r: sample pos + r is NOT in the cell
             const int run = rest ? (__ffs(rest) - 1) : 32;     // >= 1: sample pos is in
             const int pend = min(pos + run, nb);
+            // powers of delta for this run (delta is relative to the cell's window, so they are staged per run)
+            __syncwarp();                                      // the previous run's step-1 reads of vy are done
+            {
+                double vy = 1.0;
+#pragma unroll
+                for (int p = 0; p < 8; ++p) {
+                    S.vy[p * kMomLdk + lane] = vy;
+                    vy *= dl;
+                }
+            }
+            __syncwarp();
             // ---- step 1: MT += VX VY^T over the samples [pos, pend)
             for (int ks = pos >> 2; ks <= (pend - 1) >> 2; ++ks) {
                 const int ksamp = 4 * ks + lr;
                 const bool in = ksamp >= pos && ksamp < pend;
-                double a[NPT], b[NPT];
+                const double b = S.vy[lq * kMomLdk + ksamp];
+                double a[NPT];
 #pragma unroll
                 for (int qt = 0; qt < NPT; ++qt) {
                     const double v = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
                     a[qt] = in ? v : 0.0;
-                    b[qt] = S.vy[(8 * qt + lq) * kMomLdk + ksamp];
                 }
 #pragma unroll
-                for (int qt = 0; qt < NPT; ++qt)
-#pragma unroll
-                    for (int pt = 0; pt < NPT; ++pt) dmma_m8n8k4(mt[qt][pt][0], mt[qt][pt][1], a[qt], b[pt]);
+                for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[qt][0], mt[qt][1], a[qt], b);
             }
             pos = pend;
         }

@@ -1053,9 +1053,9 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
         const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
         nm = names[npt];
         // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
-        pc = 256.0 * M.T * (2.0 * npt * M.njt * ip + 2.0 * npt * M.njt * M.nit);   // y has one power tile (phase windows)
+        pc = 256.0 * M.T * (2.0 * npt * M.nit * jp + 2.0 * M.nit * M.njt);         // step 2 (redone per row panel) + step 3
         ps = 64.0 * npt + 8.0 * npt + 8.0;                     // step 1 (npt DMMAs per 4 samples) + powers
-        (void)jp;
+        (void)ip;
     } else if (psf->kind == 0 && psf->poly_degree > 0) {
         static thread_local char buf[40];
         snprintf(buf, sizeof buf, "render_poly_kernel<%d>", psf->poly_degree);

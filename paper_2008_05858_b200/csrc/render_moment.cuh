@@ -17,14 +17,20 @@
 // The y-phase of one cell's samples moves by (trace slope) x (1 px) only, so BY uses one of nyb overlapping phase
 // windows with its own degree-7 fit (poly_tables.h): p runs over 8 powers of delta = dy - (window centre) = ONE power
 // tile, while q runs over the P + 1 powers of dx (the x-phase sweeps the whole pixel inside a cell).  A cell = maximal
-// run of samples with one footprint box whose dy stays inside the window chosen at its first sample.  Everything is a small dense fp64 contraction and runs as chained
-// mma.sync.m8n8k4.f64 tiles (DMMA: same FP64 pipe as DFMA, 256 FMAs per instruction); C fragments feed the next
-// product's A/B operand directly: lane l of a C tile holds columns 2(l%4)+{0,1}, and the k-slot l%4 of the next
-// product is *defined* to be that column, with the table operand stored in the same permuted order:
+// run of samples with one footprint box whose dy stays inside the window chosen at its first sample.
 //
-//   step 1  MT[q][p]  = sum_k (w_k dx_k^q) (dy_k^p)          A = VX (smem), B = VY (smem)        C -> mt
-//   step 2  Z_t[j][q] = sum_p cy_t[p][j] M[p][q]             A = fy table,  B = mt (registers)   C -> z
-//   step 3  out[j][i]+= sum_q Z_t[j][q] cx_t[q][i]           A = z (registers), B = fx table     C -> out
+// Everything is a small dense fp64 contraction and runs as chained mma.sync.m8n8k4.f64 tiles (DMMA: same FP64 pipe as
+// DFMA, 256 FMAs per instruction).  The products are ordered so that the short dimension (8 powers of delta) is the
+// contraction index of the LARGE product, and transposed so that every C fragment feeds the next product's A operand
+// directly from registers: lane l of a C tile holds columns 2(l%4)+{0,1}, and the k-slot l%4 of the next product is
+// *defined* to be that column, with the table operand stored in the same permuted order:
+//
+//   step 1  M[p][q]      = sum_k dy_k^p (w_k dx_k^q)          A = VY (smem),      B = VX (smem)    C -> mt   NPT DMMAs / 4 samples
+//   step 2  Y_t^T[i][p]  = sum_q cx_t[q][i] M[p][q]           A = fx table,       B = mt (regs)    C -> yt   ncol/8 * 2 NPT DMMAs
+//   step 3  out^T[i][j] += sum_p Y_t^T[i][p] cy_t[p][j]       A = yt (regs),      B = fy table     C -> out  ncol/8 * nrow/8 * 2 DMMAs
+//
+// ESPRESSO-like PSF (24 x 24 window, T = 6, NPT = 2): 30 DMMAs per term, 180 per cell (the first version of this kernel,
+// with both phases on the full range and the contraction over q last, needed 360).
 //
 // One warp per work item (run of consecutive 32-sample chunks of one strip; schedule of api.cu: items of one launch
 // never touch the same pixel), no block-level cooperation; the finished window is added to the frame by L2 reductions
@@ -67,7 +73,7 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
     long long kend = k + (long long)it.nchunks * 32;
     if (kend > st.n) kend = st.n;
 
-    double mt[NPT][2];                                         // MT tiles [qt]: lane holds MT[q = 8qt + l/4][p = 2(l%4) + e]
+    double mt[NPT][2];                                         // M tiles [qt]: lane holds M[p = l/4][q = 8qt + 2(l%4) + e]
     bool have = false;
     int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
     double cYc = 0.0;                                          // its centre
@@ -81,85 +87,60 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
             if (cJ0 + 8 * jp > cJ1 || cJ0 + 8 * jp >= ny) break;
             for (int ip = 0; ip < Q.nit; ip += 3) {
                 if (cI0 + 8 * ip > cI1 || cI0 + 8 * ip >= nx) break;
-                double out[3][3][2];
+                double out[3][3][2];                           // [it][jt]: lane owns col 8 it + l/4, rows 8 jt + 2 (l%4) + {0,1}
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
                     for (int b = 0; b < 3; ++b) { out[a][b][0] = 0.0; out[a][b][1] = 0.0; }
 #pragma unroll 1
                 for (int t = 0; t < Q.T; ++t) {
-                    double z[3][NPT][2];
-#pragma unroll
-                    for (int a = 0; a < 3; ++a)
-#pragma unroll
-                        for (int b = 0; b < NPT; ++b) { z[a][b][0] = 0.0; z[a][b][1] = 0.0; }
-                    // ---- step 2: Z_t = cy_t^T M for the panel's rows (one power tile in p: two k-slots)
                     const double2* fy = Q.fy + ((size_t)(cYb * Q.T + t) * Q.njt + jp) * 32 + lane;
                     const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
-                    double2 a[3], b[3][NPT];
+                    double2 cy[3], cx[3][NPT];
 #pragma unroll
-                    for (int jt = 0; jt < 3; ++jt) a[jt] = (jp + jt < Q.njt) ? __ldg(fy + jt * 32) : make_double2(0.0, 0.0);
+                    for (int jt = 0; jt < 3; ++jt) cy[jt] = (jp + jt < Q.njt) ? __ldg(fy + jt * 32) : make_double2(0.0, 0.0);
 #pragma unroll
-                    for (int ct = 0; ct < 3; ++ct)
+                    for (int it = 0; it < 3; ++it)
 #pragma unroll
                         for (int qt = 0; qt < NPT; ++qt)
-                            b[ct][qt] = (ip + ct < Q.nit) ? __ldg(fx + (ct * NPT + qt) * 32) : make_double2(0.0, 0.0);
+                            cx[it][qt] = (ip + it < Q.nit) ? __ldg(fx + (it * NPT + qt) * 32) : make_double2(0.0, 0.0);
+                    // ---- step 2: Y_t^T = cx_t^T M^T  (columns x 8 powers of delta; contraction over the powers of dx)
+                    double yt[3][2];
 #pragma unroll
-                    for (int jt = 0; jt < 3; ++jt)
-#pragma unroll
-                        for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt].x, mt[qt][0]);
-#pragma unroll
-                    for (int jt = 0; jt < 3; ++jt)
-#pragma unroll
-                        for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(z[jt][qt][0], z[jt][qt][1], a[jt].y, mt[qt][1]);
-                    // ---- step 3: out += Z_t cx_t for the panel's columns
+                    for (int it = 0; it < 3; ++it) { yt[it][0] = 0.0; yt[it][1] = 0.0; }
 #pragma unroll
                     for (int qt = 0; qt < NPT; ++qt) {
 #pragma unroll
-                        for (int jt = 0; jt < 3; ++jt)
+                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].x, mt[qt][0]);
 #pragma unroll
-                            for (int ct = 0; ct < 3; ++ct) dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][0], b[ct][qt].x);
-#pragma unroll
-                        for (int jt = 0; jt < 3; ++jt)
-#pragma unroll
-                            for (int ct = 0; ct < 3; ++ct) dmma_m8n8k4(out[jt][ct][0], out[jt][ct][1], z[jt][qt][1], b[ct][qt].y);
+                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].y, mt[qt][1]);
                     }
+                    // ---- step 3: out^T += Y_t^T cy_t  (contraction over the 8 powers of delta: two k-slots)
+#pragma unroll
+                    for (int it = 0; it < 3; ++it)
+#pragma unroll
+                        for (int jt = 0; jt < 3; ++jt) dmma_m8n8k4(out[it][jt][0], out[it][jt][1], yt[it][0], cy[jt].x);
+#pragma unroll
+                    for (int it = 0; it < 3; ++it)
+#pragma unroll
+                        for (int jt = 0; jt < 3; ++jt) dmma_m8n8k4(out[it][jt][0], out[it][jt][1], yt[it][1], cy[jt].y);
                 }
-                // ---- a5: add the panel to the frame.  lane owns out[row 8 jt + l/4][cols 8 ct + 2 (l%4) + {0,1}]
+                // ---- a5: add the panel to the frame by L2 reductions (red.global.add.f64): the same IEEE sum as load + add +
+                // store without a round trip to wait for.  Order per pixel: items of one launch never share a pixel, and
+                // inside the warp the __syncwarp() that closes every flush orders this cell's reductions before the next
+                // cell's -> bit-reproducible
                 const int rlim = min(cJ1, ny - 1), clim = min(cI1, nx - 1);
 #pragma unroll
-                for (int jt = 0; jt < 3; ++jt) {
-                    const int row = cJ0 + 8 * (jp + jt) + lq;
-                    const bool rok = row >= 0 && row <= rlim;
-                    double* prow = frame + (size_t)(rok ? row : 0) * nx;
-#if E2E_MOM_RED
-                    // fire-and-forget reduction at L2 (same IEEE sum as load + add + store, no round trip to wait for).
-                    // Order per pixel: items of one launch never share a pixel, and inside the warp the __syncwarp()
-                    // that closes every flush orders this cell's reductions before the next cell's -> still bit-reproducible
+                for (int it = 0; it < 3; ++it) {
+                    const int col = cI0 + 8 * (ip + it) + lq;
+                    const bool cok = col >= 0 && col <= clim;
 #pragma unroll
-                    for (int ct = 0; ct < 3; ++ct)
+                    for (int jt = 0; jt < 3; ++jt)
 #pragma unroll
                         for (int e = 0; e < 2; ++e) {
-                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
-                            if (rok && col >= 0 && col <= clim) atomicAdd(prow + col, out[jt][ct][e]);
+                            const int row = cJ0 + 8 * (jp + jt) + 2 * lr + e;
+                            if (cok && row >= 0 && row <= rlim) atomicAdd(frame + (size_t)row * nx + col, out[it][jt][e]);
                         }
-#else
-                    double old[3][2];
-#pragma unroll
-                    for (int ct = 0; ct < 3; ++ct)
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
-                            old[ct][e] = (rok && col >= 0 && col <= clim) ? __ldcg(prow + col) : 0.0;
-                        }
-#pragma unroll
-                    for (int ct = 0; ct < 3; ++ct)
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            const int col = cI0 + 8 * (ip + ct) + 2 * lr + e;
-                            if (rok && col >= 0 && col <= clim) __stcg(prow + col, old[ct][e] + out[jt][ct][e]);
-                        }
-#endif
                 }
             }
         }
@@ -227,15 +208,13 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
             for (int ks = pos >> 2; ks <= (pend - 1) >> 2; ++ks) {
                 const int ksamp = 4 * ks + lr;
                 const bool in = ksamp >= pos && ksamp < pend;
-                const double b = S.vy[lq * kMomLdk + ksamp];
-                double a[NPT];
+                const double v = S.vy[lq * kMomLdk + ksamp];
+                const double a = in ? v : 0.0;                 // A = VY: row p = l/4, k-slot = sample
+                double b[NPT];                                 // B = VX^T: k-slot = sample, column q = 8 qt + l/4
 #pragma unroll
-                for (int qt = 0; qt < NPT; ++qt) {
-                    const double v = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
-                    a[qt] = in ? v : 0.0;
-                }
+                for (int qt = 0; qt < NPT; ++qt) b[qt] = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
 #pragma unroll
-                for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[qt][0], mt[qt][1], a[qt], b);
+                for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[qt][0], mt[qt][1], a, b[qt]);
             }
             pos = pend;
         }

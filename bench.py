@@ -35,8 +35,8 @@ C_ERFC, C_PSI = 60.0, 90.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture of this command (profiles/, file named beside each value); None = not captured for that kernel
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1_v5_espresso.md, launch ids 1-4: mean of (440.5+114.3, 439.8+113.5, 441.0+114.3, 439.5+114.5) MB
-    "render_moment_kernel<2>": 554.3e6,
+    # profiles/r1_v6_espresso.md, launch ids 1-4 (dram__bytes_read.sum + dram__bytes_write.sum, mean)
+    "render_moment_kernel<2>": 549.0e6,
 }
 
 
@@ -333,8 +333,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     ms_render = prof["ms_render"] / max(prof["n_calls"], 1)
     roofline = None
     if fma_flops is not None and ms_render > 0:
-        ach = n_samples * fma_flops / (ms_render * 1e-3) / 1e12
+        alg = B.e2e_render_algorithmic_fma(r.fmt, r.psf)
+        alg_flops = 2.0 * (n_cells * alg["fma_per_cell"] + n_samples * alg["fma_per_sample"])
         executed = 2.0 * (n_cells * kinfo["executed_fma_per_cell"] + n_samples * kinfo["executed_fma_per_sample"])
+        sec = ms_render * 1e-3
+        if alg_flops <= 0:                                   # kernels that do not work cell by cell: the direct method's accumulate
+            alg_flops = n_samples * fma_flops
+        ach = alg_flops / sec / 1e12
         roofline = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
                     "traffic": NCU_TRAFFIC_BYTES.get(kinfo["name"]),
                     "kernel": kinfo["name"], "kernel_ms_per_step": ms_render,
@@ -342,13 +347,18 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                     "peak_source": "measured in this run: e2e_measure_fp64_peak, sustained FP64-pipe rate (max of DFMA and DMMA chains) x 2 "
                                    "(MEASURED_PEAKS.json has no fp64 entry)",
                     "peak_burst": 2.0 * burst / 1e12,
-                    "flops_per_sample": fma_flops, "definition": "algorithmic = irreducible rank-T FMA accumulate of the direct method: "
-                                                                 "2*T*ncols*nrows flop per sample (DESIGN.md 'Roofline')",
+                    "flops_per_sample": alg_flops / n_samples,
+                    "definition": "algorithmic = un-padded fp64 flops of the cell-moment method (DESIGN.md 5.3 'Roofline'): per cell "
+                                  "2 T (8 (P+1) w + 8 w h), per sample 2 * 8 (P+1); x measured cell / sample counts of the workload",
                     "footprint_cells": n_cells,
-                    "executed_tflops": executed / (ms_render * 1e-3) / 1e12, "executed_frac": executed / (ms_render * 1e-3) / 1e12 / peak_tf,
-                    "executed_definition": "fp64 FMAs the kernel issues (DMMA = 256) x 2, from e2e_render_kernel_info x cell / sample counts",
-                    "achieved_survey_formula": n_samples * survey_flops / (ms_render * 1e-3) / 1e12,
-                    "survey_flops_per_sample": survey_flops}
+                    "executed_tflops": executed / sec / 1e12, "executed_frac": executed / sec / 1e12 / peak_tf,
+                    "executed_definition": "fp64 FMAs the kernel issues (DMMA = 256, padded tiles) x 2, from e2e_render_kernel_info x cell / sample counts",
+                    "direct_method_flops_per_sample": fma_flops,
+                    "direct_method_tflops_equivalent": n_samples * fma_flops / sec / 1e12,
+                    "direct_method_definition": "bare rank-T accumulate of the per-sample method, 2*T*w*h flop per sample: what this kernel would "
+                                                "have to sustain if it evaluated every (sample, pixel) product (it does not: context only)",
+                    "survey_flops_per_sample": survey_flops,
+                    "survey_formula_tflops_equivalent": n_samples * survey_flops / sec / 1e12}
     cpu = None
     if not args.no_cpu:
         c = time_oracle(scene, args.oracle_samples)

@@ -219,6 +219,13 @@ E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, dou
 E2E_API int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name,
                                    double* executed_fma_per_cell, double* executed_fma_per_sample);
 
+/* Algorithmic work of the a4+a5 method e2e_render_frame uses for this pair (DESIGN.md 5.3 "Roofline"), without the
+ * padding of the DMMA tiles: fp64 fused multiply-adds per footprint cell, T (8 (P+1) w + 8 w h) with w x h the nominal
+ * footprint (2 H + 1 pixels per axis, G9), P the x-phase degree, T the chord terms, and per sample, 8 (P+1) (moment update).
+ * 0 for the kernels that do not work cell by cell.  Output pointers may be NULL. */
+E2E_API int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, double* fma_per_cell,
+                                       double* fma_per_sample);
+
 /* Number of kernel launches the library has issued since load (all entry points), for bench.py's gpu_launches. */
 E2E_API int64_t e2e_launch_count(void);
 

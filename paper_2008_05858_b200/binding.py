@@ -24,7 +24,8 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_psf_create", "e2e_psf_destroy", "e2e_psf_info", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_apply_detector_ex",
            "e2e_measure_fp64_peak",
-           "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info"]
+           "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
+           "e2e_render_algorithmic_fma"]
 
 
 class E2EError(RuntimeError):
@@ -117,6 +118,8 @@ def load():
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_render_kernel_info.restype = C.c_int
     L.e2e_render_kernel_info.argtypes = [vp, vp, C.POINTER(C.c_char_p), C.POINTER(dbl), C.POINTER(dbl)]
+    L.e2e_render_algorithmic_fma.restype = C.c_int
+    L.e2e_render_algorithmic_fma.argtypes = [vp, vp, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_launch_count.restype = i64
     L.e2e_launch_count.argtypes = []
     L.e2e_profile_enable.restype = C.c_int
@@ -324,6 +327,13 @@ def e2e_render_kernel_info(fmt, psf) -> dict:
     name, pc, ps = C.c_char_p(), C.c_double(), C.c_double()
     _check(load().e2e_render_kernel_info(fmt.handle, psf.handle, C.byref(name), C.byref(pc), C.byref(ps)))
     return {"name": name.value.decode(), "executed_fma_per_cell": float(pc.value), "executed_fma_per_sample": float(ps.value)}
+
+
+def e2e_render_algorithmic_fma(fmt, psf) -> dict:
+    """un-padded fp64 FMAs of the cell-moment method per footprint cell / per sample (0 for the other kernels)"""
+    pc, ps = C.c_double(), C.c_double()
+    _check(load().e2e_render_algorithmic_fma(fmt.handle, psf.handle, C.byref(pc), C.byref(ps)))
+    return {"fma_per_cell": float(pc.value), "fma_per_sample": float(ps.value)}
 
 
 def e2e_profile_enable(on: bool):

@@ -425,6 +425,7 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
                 M.fx = reinterpret_cast<const double2*>(P->d_mom);
                 M.fy = reinterpret_cast<const double2*>(P->d_mom + nfx);
                 P->moment_npt = mom.npt;
+                P->moment_degree = mom.P;
             }
         }
     } else if (d->kind == 1) {
@@ -1066,6 +1067,21 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
         nm = "render_analytic_kernel";
     }
     if (name) *name = nm;
+    if (fma_cell) *fma_cell = pc;
+    if (fma_sample) *fma_sample = ps;
+    return E2E_OK;
+}
+
+int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, double* fma_cell, double* fma_sample)
+{
+    if (!fmt || !psf) return fail(E2E_ERR_INVALID_ARG, "render_algorithmic_fma: NULL argument");
+    double pc = 0.0, ps = 0.0;
+    if (choose_moment(fmt, psf)) {
+        const double w = std::floor(2.0 * psf->hbx), h = std::floor(2.0 * psf->hby);   // nominal footprint (2 H + 1 per axis, G9)
+        const double np1 = (double)psf->moment_degree + 1.0;
+        pc = (double)psf->mom.T * (8.0 * np1 * w + 8.0 * w * h);
+        ps = 8.0 * np1;
+    }
     if (fma_cell) *fma_cell = pc;
     if (fma_sample) *fma_sample = ps;
     return E2E_OK;

@@ -159,6 +159,7 @@ struct e2e_psf {
     e2e::PolyParam poly;
     double* d_poly = nullptr;      // one allocation: tx then ty
     int moment_npt = 0;            // > 0: moment tables built, power tiles in use
+    int moment_degree = 0;         // x-phase degree of the moment tables
     e2e::MomentParam mom;
     double* d_mom = nullptr;       // one allocation: fx then fy
 };

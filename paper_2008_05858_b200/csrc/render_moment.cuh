@@ -44,6 +44,9 @@ namespace e2e {
 #ifndef E2E_MOM_RED
 #define E2E_MOM_RED 1
 #endif
+#ifndef E2E_MOM_MINB
+#define E2E_MOM_MINB 4
+#endif
 constexpr int kMomWarps = 4;           // warps per CTA
 constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sample] (36 mod 16 = 4: conflict-free fragments)
 
@@ -54,7 +57,7 @@ struct MomentWarpSmem {
 };
 
 template <int NPT>
-__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? 4 : 1)
+__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB : 1)
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                      const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
                      double* __restrict__ frame, int nx, int ny)

@@ -25,7 +25,7 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_apply_detector_ex",
            "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
-           "e2e_render_algorithmic_fma"]
+           "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames"]
 
 
 class E2EError(RuntimeError):
@@ -118,6 +118,10 @@ def load():
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_render_kernel_info.restype = C.c_int
     L.e2e_render_kernel_info.argtypes = [vp, vp, C.POINTER(C.c_char_p), C.POINTER(dbl), C.POINTER(dbl)]
+    L.e2e_render_frames_workspace_bytes.restype = C.c_int
+    L.e2e_render_frames_workspace_bytes.argtypes = [vp, vp, i32, C.POINTER(C.c_size_t)]
+    L.e2e_render_frames.restype = C.c_int
+    L.e2e_render_frames.argtypes = [vp, vp, i32, vp, vp, i32, vp, C.c_size_t, vp]
     L.e2e_render_algorithmic_fma.restype = C.c_int
     L.e2e_render_algorithmic_fma.argtypes = [vp, vp, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_launch_count.restype = i64
@@ -281,6 +285,26 @@ def e2e_render_frame(fmt: Format, psf: Psf, spectra_desc, d_frame, accumulate: b
     _check(load().e2e_render_frame(fmt.handle, psf.handle, spectra_desc, int(d_frame.data_ptr()), int(bool(accumulate)),
                                    int(d_workspace.data_ptr()), int(d_workspace.numel() * d_workspace.element_size()),
                                    _stream_ptr(stream)))
+
+
+def e2e_render_frames_workspace_bytes(fmt: Format, psf: Psf, n_frames: int) -> int:
+    n = C.c_size_t()
+    _check(load().e2e_render_frames_workspace_bytes(fmt.handle, psf.handle, int(n_frames), C.byref(n)))
+    return int(n.value)
+
+
+def e2e_render_frames(fmt: Format, psf: Psf, spectra_descs: Sequence, d_frames: Sequence, accumulate: bool, d_workspace, stream=None):
+    """batch render on fixed geometry: spectra_descs = one spectra_array per frame, d_frames = one CUDA tensor per frame"""
+    nfr = len(d_frames)
+    nfib = len(spectra_descs[0])
+    flat = (SpectrumDesc * (nfr * nfib))()
+    for b, desc in enumerate(spectra_descs):
+        for f in range(nfib):
+            C.memmove(C.byref(flat, (b * nfib + f) * C.sizeof(SpectrumDesc)), C.byref(desc, f * C.sizeof(SpectrumDesc)),
+                      C.sizeof(SpectrumDesc))
+    ptrs = (C.c_void_p * nfr)(*[int(t.data_ptr()) for t in d_frames])
+    _check(load().e2e_render_frames(fmt.handle, psf.handle, nfr, flat, ptrs, int(bool(accumulate)), int(d_workspace.data_ptr()),
+                                    int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
 
 
 def e2e_render_host_workspace_bytes(fmt: Format, psf: Psf, spectra_desc) -> int:

@@ -759,8 +759,18 @@ static bool choose_tabcell(const e2e_psf* P)
 
 static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
                          const double* d_w, double* d_frame, cudaStream_t stream, const Item* d_item_list = nullptr,
-                         const int* phase_off = nullptr, int n_phases = -1)
+                         const int* phase_off = nullptr, int n_phases = -1, int n_frames = 1, long long w_stride = 0,
+                         double* const* d_frames = nullptr, double* const* h_frames = nullptr)
 {
+    // batch (e2e_render_frames): the production kernel takes the frame index from blockIdx.y; the other kernels
+    // render frame after frame
+    if (n_frames > 1 && !choose_moment(F, P)) {
+        for (int b = 0; b < n_frames; ++b) {
+            int rc = launch_render(F, P, pl, d_x, d_y, d_w + (size_t)b * w_stride, h_frames[b], stream, d_item_list, phase_off, n_phases);
+            if (rc) return rc;
+        }
+        return E2E_OK;
+    }
     if (!d_item_list) { d_item_list = pl->d_items; phase_off = pl->phase_off.data(); n_phases = pl->n_phases; }
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
@@ -785,8 +795,9 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         static cudaError_t attr = cudaFuncSetAttribute(render_moment_kernel<NPT>,                                       \
                                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);           \
         if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_moment_kernel)");                  \
-        render_moment_kernel<NPT><<<pb, kMomWarps * 32, sm, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, \
-                                                                      P->mom, d_frame, F->view.nx, F->view.ny);         \
+        render_moment_kernel<NPT><<<dim3(pb, n_frames), kMomWarps * 32, sm, stream>>>(                                  \
+            d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, P->mom, d_frame, F->view.nx, F->view.ny, w_stride,        \
+            n_frames > 1 ? d_frames : nullptr);                                                                          \
     } break;
             switch (P->moment_npt) {
                 E2E_MOM_CASE(2) E2E_MOM_CASE(3) E2E_MOM_CASE(4)
@@ -907,6 +918,69 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
         StageTimer tm(kStageRender, stream);
         const long long before = g_launches.load();
         rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+        if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
+    }
+    return rc;
+}
+
+int e2e_render_frames_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_frames, size_t* bytes)
+{
+    if (n_frames < 1 || n_frames > 65535) return fail(E2E_ERR_INVALID_ARG, "render_frames_workspace_bytes: n_frames must be 1..65535");
+    size_t one = 0;
+    int rc = e2e_render_workspace_bytes(fmt, psf, &one);
+    if (rc) return rc;
+    *bytes = one / 3 * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256);
+    return E2E_OK;
+}
+
+int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_frames, const e2e_spectrum_t* spectra,
+                      double* const* d_frames, int32_t accumulate, void* d_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!fmt || !psf || !d_frames) return fail(E2E_ERR_INVALID_ARG, "render_frames: NULL argument");
+    if (n_frames < 1 || n_frames > 65535) return fail(E2E_ERR_INVALID_ARG, "render_frames: n_frames must be 1..65535");
+    if (psf->nx != fmt->view.nx || psf->ny != fmt->view.ny)
+        return fail(E2E_ERR_INVALID_ARG, "render_frames: psf was created for another detector size");
+    const int nf = fmt->view.n_fibers;
+    for (int b = 0; b < n_frames; ++b) {
+        if (!d_frames[b]) return fail(E2E_ERR_INVALID_ARG, "render_frames: NULL frame pointer");
+        for (int c = 0; c < b; ++c)
+            if (d_frames[c] == d_frames[b]) return fail(E2E_ERR_INVALID_ARG, "render_frames: two frames share one buffer");
+        int rc = check_spectra(fmt, spectra ? spectra + (size_t)b * nf : nullptr, "render_frames");
+        if (rc) return rc;
+    }
+    e2e_plan* pl = nullptr;
+    int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    const size_t per = sample_array_bytes(pl->total_samples);
+    const size_t need = per * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256);
+    if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace NULL or not 256-byte aligned");
+    if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace too small");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    double* d_x = (double*)d_workspace;
+    double* d_y = (double*)((char*)d_workspace + per);
+    double* d_w = (double*)((char*)d_workspace + 2 * per);
+    double** d_ptrs = (double**)((char*)d_workspace + per * (2 + (size_t)n_frames));
+    // pageable source: the copy is staged before the call returns, so the caller's array need not outlive it
+    E2E_CUDA(cudaMemcpyAsync(d_ptrs, d_frames, sizeof(double*) * (size_t)n_frames, cudaMemcpyHostToDevice, stream));
+    if (!accumulate) {
+        StageTimer tm(kStageZero, stream);
+        for (int b = 0; b < n_frames; ++b)
+            E2E_CUDA(cudaMemsetAsync(d_frames[b], 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
+    }
+    {
+        StageTimer tm(kStageSetup, stream);
+        const long long before = g_launches.load();
+        for (int b = 0; b < n_frames && !rc; ++b)               // a1-a3 once (frame 0 writes x, y), a2 per frame
+            rc = launch_setup(fmt, pl, spectra + (size_t)b * nf, b == 0 ? d_x : nullptr, b == 0 ? d_y : nullptr,
+                              d_w + (size_t)b * (per / 8), stream);
+        if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
+        if (rc) return rc;
+    }
+    {
+        StageTimer tm(kStageRender, stream);
+        const long long before = g_launches.load();
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frames[0], stream, nullptr, nullptr, -1, n_frames, (long long)(per / 8),
+                           d_ptrs, d_frames);
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
     }
     return rc;

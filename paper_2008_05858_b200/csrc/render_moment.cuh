@@ -60,12 +60,16 @@ template <int NPT>
 __global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB : 1)
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                      const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
-                     double* __restrict__ frame, int nx, int ny)
+                     double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int item_id = blockIdx.x * kMomWarps + warp;
     if (item_id >= n_items) return;
+    if (frames) {                                             // batch render (e2e_render_frames): blockIdx.y = frame,
+        frame = frames[blockIdx.y];                           // same geometry, its own weights and target
+        ws += (long long)blockIdx.y * w_stride;
+    }
     MomentWarpSmem<NPT>& S = reinterpret_cast<MomentWarpSmem<NPT>*>(smem_raw)[warp];
     const Item it = items[item_id];
     const Strip st = strips[it.strip];

@@ -496,6 +496,53 @@ def test_detector_ex_bit_exact(B):
         B.e2e_apply_detector_ex(d_out, d_out, nx, ny, det, d_prnu=d_out)
 
 
+def test_render_frames_batch_equals_single_renders(B):
+    """batch render on fixed geometry.  The five Doppler-shifted frames of the RV sweep in one call are,
+    frame by frame, the bits of five single renders (and frame 0 passes the oracle parity of the other tests);
+    the sparse-sampling scene takes the frame-after-frame route of the non-production kernels"""
+    import torch
+    for make in (lambda v: W.rv_sweep(v), lambda v: _sparse_rv(v)):
+        scenes = [make(v) for v in (0.0, 0.01, 0.1, 1.0, 10.0)]
+        r = B.Renderer(scenes[0])
+        try:
+            singles = []
+            descs = []
+            keep = []
+            for sc in scenes:
+                flux = [torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).cuda() for sp in sc.spectra]
+                keep.append(flux)
+                d = B.spectra_array(sc.spectra, [t.data_ptr() for t in flux])
+                descs.append(d)
+                fr = torch.empty((sc.ny, sc.nx), dtype=torch.float64, device="cuda")
+                B.e2e_render_frame(r.fmt, r.psf, d, fr, False, r.workspace)
+                singles.append(fr.clone())
+            nbytes = B.e2e_render_frames_workspace_bytes(r.fmt, r.psf, len(scenes))
+            ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            frames = [torch.full((scenes[0].ny, scenes[0].nx), float("nan"), dtype=torch.float64, device="cuda") for _ in scenes]
+            B.e2e_render_frames(r.fmt, r.psf, descs, frames, False, ws)
+            torch.cuda.synchronize()
+            for a, b in zip(frames, singles):
+                assert torch.equal(a, b)
+            assert not torch.equal(frames[0], frames[4])            # the shift is there
+            # accumulate = 1 adds on top
+            B.e2e_render_frames(r.fmt, r.psf, descs, frames, True, ws)
+            torch.cuda.synchronize()
+            assert torch.allclose(frames[2], 2.0 * singles[2], rtol=1e-15, atol=0.0)
+            with pytest.raises(B.E2EError):
+                B.e2e_render_frames(r.fmt, r.psf, descs[:2], [frames[0], frames[0]], False, ws)
+            with pytest.raises(B.E2EError):
+                B.e2e_render_frames(r.fmt, r.psf, descs, frames, False, ws[:4096])
+        finally:
+            r.close()
+
+
+def _sparse_rv(v):
+    s = W.rv_sweep(v)
+    s.samples_per_px = 3.0
+    s.lam_max = np.array([s.lam_min[0] + 4.0])
+    return s
+
+
 def test_rv_sweep_photocenter_linear_in_velocity(B):
     """BASELINE.json configs[4]: 5 Doppler-shifted frames; global photocenter shift vs the analytic slope and
     per-line centroid residual against a straight line in v < 1e-6 px; GPU == oracle on the v = 10 m/s frame;

@@ -41,11 +41,8 @@
 
 namespace e2e {
 
-#ifndef E2E_MOM_RED
-#define E2E_MOM_RED 1
-#endif
 #ifndef E2E_MOM_MINB
-#define E2E_MOM_MINB 4
+#define E2E_MOM_MINB 4           // CTAs per SM for NPT = 2 (3 / 5 / 6 measured slower)
 #endif
 constexpr int kMomWarps = 4;           // warps per CTA
 constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sample] (36 mod 16 = 4: conflict-free fragments)

@@ -118,7 +118,7 @@ __device__ __forceinline__ void detector_draws(uint64_t seed, long long p, doubl
 
 // in / out point at pixel p0 of the frame (the host path applies the stage band by band); the stream is keyed by the
 // pixel's index in the whole frame, so the result does not depend on how the frame is split into launches
-__global__ void detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, long long p0, e2e_detector_t det)
+__global__ void __launch_bounds__(256, 6) detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, long long p0, e2e_detector_t det)
 {
     long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;

@@ -36,7 +36,7 @@ int measure_fp64_peak(int repeats, double* burst, double* sustained);
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
 constexpr long long kSmallFrameItems = 4736;   // 2 x (148 SMs x 16 resident warps): below this a K = 2 schedule leaves the GPU idle
-constexpr int kHostBands = 6;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
+constexpr int kHostBands = 8;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -674,12 +674,28 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rlo[a] < rlo[b]; });
         int want = kHostBands;
         if (const char* e = getenv("E2E_HOST_BANDS")) want = std::max(1, std::min(atoi(e), 16));
+        // band b takes the share wgt[b] of the samples: the first bands are small, so that the copy engine starts early,
+        // the later ones up to 3x larger (the copy is the slower side and must only never run dry); E2E_HOST_BAND_RAMP=0:
+        // equal shares
+        std::vector<double> cum(want + 1, 0.0);
+        {
+            const char* ramp = getenv("E2E_HOST_BAND_RAMP");
+            std::vector<double> wgt(want, 1.0);
+            if (!(ramp && ramp[0] == '0'))
+                for (int b = 0; b < want; ++b) wgt[b] = 1.0 + 2.0 * (double)b / (double)std::max(1, want - 1);
+            double sum = 0.0;
+            for (double w : wgt) sum += w;
+            for (int b = 0; b < want; ++b) cum[b + 1] = cum[b] + wgt[b] / sum;
+        }
         std::vector<int> band_of(n_strips, 0);
         long long acc = 0;
         const long long tot = std::max<long long>(pl->total_samples, 1);
         for (int i = 0; i < n_strips; ++i) {
             const int s = order[i];
-            band_of[s] = (int)std::min<long long>(want - 1, acc * want / tot);
+            const double frac = (double)acc / (double)tot;
+            int b = 0;
+            while (b < want - 1 && frac >= cum[b + 1]) ++b;
+            band_of[s] = b;
             acc += pl->strips[s].n;
         }
         pl->n_bands = want;

@@ -120,6 +120,7 @@ e2e_plan::~e2e_plan()
     if (d_strips) cudaFree(d_strips);
     if (d_items) cudaFree(d_items);
     if (d_band_items) cudaFree(d_band_items);
+    if (d_band_strips) cudaFree(d_band_strips);
 }
 
 extern "C" {
@@ -716,6 +717,15 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
                 for (const Item& it : phases[ph])
                     if (band_of[it.strip] == b) bflat.push_back(it);
             }
+        std::vector<int> bstrips;
+        pl->band_strip_off.assign(want + 1, 0);
+        for (int b = 0; b < want; ++b) {
+            for (int s = 0; s < n_strips; ++s)
+                if (band_of[s] == b && pl->strips[s].n > 0) bstrips.push_back(s);
+            pl->band_strip_off[b + 1] = (int)bstrips.size();
+        }
+        E2E_CUDA(cudaMalloc(&pl->d_band_strips, sizeof(int) * std::max<size_t>(1, bstrips.size())));
+        if (!bstrips.empty()) E2E_CUDA(cudaMemcpy(pl->d_band_strips, bstrips.data(), sizeof(int) * bstrips.size(), cudaMemcpyHostToDevice));
         E2E_CUDA(cudaMalloc(&pl->d_band_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
         if (!bflat.empty()) E2E_CUDA(cudaMemcpy(pl->d_band_items, bflat.data(), sizeof(Item) * bflat.size(), cudaMemcpyHostToDevice));
     }
@@ -738,7 +748,7 @@ static int check_spectra(const e2e_format* F, const e2e_spectrum_t* spectra, con
 }
 
 static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spectrum_t* spectra, double* d_x, double* d_y,
-                        double* d_w, cudaStream_t stream)
+                        double* d_w, cudaStream_t stream, int band = -1)
 {
     SpectraParam sp;
     memset(&sp, 0, sizeof(sp));
@@ -746,8 +756,15 @@ static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spect
     long long nmax = 0;
     for (long long n : F->nsamp) nmax = std::max(nmax, n);
     if (nmax == 0) return E2E_OK;
-    dim3 grid((unsigned)((nmax + 255) / 256), (unsigned)pl->n_strips);
-    setup_samples_kernel<<<grid, 256, 0, stream>>>(F->view, sp, pl->d_strips, 0, nullptr, d_x, d_y, d_w);
+    const int* ids = nullptr;
+    int ny_grid = pl->n_strips;
+    if (band >= 0) {                                            // one row band of the host path
+        ids = pl->d_band_strips + pl->band_strip_off[band];
+        ny_grid = pl->band_strip_off[band + 1] - pl->band_strip_off[band];
+        if (ny_grid == 0) return E2E_OK;
+    }
+    dim3 grid((unsigned)((nmax + 255) / 256), (unsigned)ny_grid);
+    setup_samples_kernel<<<grid, 256, 0, stream>>>(F->view, sp, pl->d_strips, 0, nullptr, d_x, d_y, d_w, ids);
     count_launch();
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "setup_samples_kernel launch");
@@ -1074,10 +1091,10 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
         return fail(E2E_ERR_INVALID_ARG, "render_frame_host: non-finite detector parameter");
     std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
     E2E_CUDA(cudaMemsetAsync(d_frame, 0, frame_bytes, stream));
-    rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, stream);
-    if (rc) return rc;
     int row0 = 0;
     for (int b = 0; b < pl->n_bands; ++b) {
+        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, stream, b);          // a1-a3 of this band's strips only
+        if (rc) return rc;
         rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, pl->d_band_items,
                            pl->band_phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
         if (rc) return rc;

@@ -184,6 +184,8 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     std::vector<int> band_phase_off;
     std::vector<int> band_fin_row;
     e2e::Item* d_band_items = nullptr;
+    std::vector<int> band_strip_off;   // [n_bands + 1] into d_band_strips: the strips of each band
+    int* d_band_strips = nullptr;
     ~e2e_plan();
 };
 

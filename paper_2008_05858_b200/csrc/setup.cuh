@@ -122,13 +122,16 @@ __device__ __forceinline__ double eff_at(const FormatView& f, double lam)
 
 // a1-a3 for every strip (fiber, order) of a render: blockIdx.y = strip = fiber * n_orders + order.
 // Coalesced: thread <-> sample, structure-of-arrays output.
+// strip_ids (optional): the strips of this launch (the host path sets up one row band at a time); strips is then the
+// whole strip table.
 __global__ void setup_samples_kernel(FormatView f, SpectraParam sp, const Strip* __restrict__ strips,
                                      int strip0, double* __restrict__ out_lam, double* __restrict__ out_x,
-                                     double* __restrict__ out_y, double* __restrict__ out_w)
+                                     double* __restrict__ out_y, double* __restrict__ out_w,
+                                     const int* __restrict__ strip_ids = nullptr)
 {
-    int sidx = strip0 + blockIdx.y;
+    int sidx = strip_ids ? strip_ids[blockIdx.y] : strip0 + blockIdx.y;
     int fiber = sidx / f.n_orders, o = sidx - fiber * f.n_orders;
-    Strip st = strips[blockIdx.y];
+    Strip st = strips[strip_ids ? sidx : blockIdx.y];
     long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= st.n) return;
     double lam, X, Y;

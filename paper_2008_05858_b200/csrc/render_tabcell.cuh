@@ -120,7 +120,7 @@ render_tabcell_kernel(const double* __restrict__ xs, const double* __restrict__ 
                         const double* Wrow = Wt + c * SR + rb * S;
                         const double* Prow = Pc + ((size_t)(ry * T.os) * ld + dJ) * ld;
                         // branch-free body: the table loads of consecutive offsets overlap
-#pragma unroll 2
+#pragma unroll 9
                         for (int ap = aMin; ap <= aMax + 1; ++ap) {
                             double wv[kTcGroup];
 #pragma unroll

@@ -673,7 +673,10 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         std::vector<int> order(n_strips);
         for (int s = 0; s < n_strips; ++s) order[s] = s;
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rlo[a] < rlo[b]; });
-        int want = kHostBands;
+        // 8 bands of growing size when a band's launches are few (2 colours x 2 classes); frames with many colours (10
+        // fibers per order: 10 launches per band) measured better with 6 equal bands
+        const bool many_phases = phases.size() > 4;
+        int want = many_phases ? 6 : kHostBands;
         if (const char* e = getenv("E2E_HOST_BANDS")) want = std::max(1, std::min(atoi(e), 16));
         // band b takes the share wgt[b] of the samples: the first bands are small, so that the copy engine starts early,
         // the later ones up to 3x larger (the copy is the slower side and must only never run dry); E2E_HOST_BAND_RAMP=0:
@@ -682,7 +685,7 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         {
             const char* ramp = getenv("E2E_HOST_BAND_RAMP");
             std::vector<double> wgt(want, 1.0);
-            if (!(ramp && ramp[0] == '0'))
+            if (ramp ? ramp[0] != '0' : !many_phases)
                 for (int b = 0; b < want; ++b) wgt[b] = 1.0 + 2.0 * (double)b / (double)std::max(1, want - 1);
             double sum = 0.0;
             for (double w : wgt) sum += w;

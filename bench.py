@@ -325,7 +325,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the spectra, D2H of the frame, every step
     e2e = None
     if not args.no_e2e:
-        host_tabs = [torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).pin_memory() for sp in scene.spectra]
+        pinned = {}                                          # fibers that share one table share one pinned copy (and one H2D)
+        for sp in scene.spectra:
+            if id(sp.flux) not in pinned:
+                pinned[id(sp.flux)] = torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).pin_memory()
+        host_tabs = [pinned[id(sp.flux)] for sp in scene.spectra]
         desc = B.spectra_array(scene.spectra, [t.data_ptr() for t in host_tabs])
         nbytes = B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc)
         ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)

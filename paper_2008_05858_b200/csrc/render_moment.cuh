@@ -42,7 +42,8 @@
 namespace e2e {
 
 #ifndef E2E_MOM_MINB
-#define E2E_MOM_MINB 4           // 4-warp CTA equivalents per SM for NPT = 2, i.e. 16 warps (12 / 20 / 24 measured slower)
+#define E2E_MOM_MINB 18          // single-warp CTAs per SM asked of ptxas for NPT = 2: 96 registers, no spills, 21 resident
+                                 // (16 -> 114 registers: 6.13 ms; 17-19 -> 96: 6.00; 22-24 -> 80 with spills: 6.38)
 #endif
 constexpr int kMomWarps = 1;           // warps per CTA: one item per CTA, so a slow item never holds three finished warps' resources
                                        // (4 / 2 / 1 warps per CTA: 6.18 / 6.17 / 6.13 ms)
@@ -55,7 +56,7 @@ struct MomentWarpSmem {
 };
 
 template <int NPT>
-__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB * 4 / kMomWarps : 1)
+__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB : 1)
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                      const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
                      double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)

@@ -169,10 +169,12 @@ E2E_API int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int
  * [ny*nx] array (pinned memory gives full PCIe speed).  The call copies the tables to the device, renders,
  * applies the detector stage a6 when det != NULL, copies the frame back and synchronises the stream before
  * returning.  Device scratch is taken from d_workspace, which must hold e2e_render_host_workspace_bytes() bytes.
- * The (fiber, order) strips are rendered in 8 row bands of growing size (E2E_HOST_BANDS overrides, 1..16): as soon as no later band
- * can write a row, a6 runs on it and it travels to the host on a copy stream owned by the library while the next band
- * renders.  The frame is bit-reproducible call to call; against e2e_render_frame it can differ in the last bit where
- * strips of different bands overlap (the additions happen in band order).  Calls on one device are serialised. */
+ * The (fiber, order) strips are rendered in up to 8 row bands (E2E_HOST_BANDS overrides, 1..16) that share no pixel
+ * (a band starts only where a strip's first row lies above every row of the strips before it): even bands run on
+ * cuda_stream, odd bands on a second stream owned by the library, and as soon as a band is done a6 runs on its rows
+ * and they travel to the host on the library's copy stream.  The frame is bit-reproducible call to call; against
+ * e2e_render_frame it can differ in the last bit where strips overlap (the additions happen band by band).  Calls
+ * on one device are serialised. */
 E2E_API int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                                     size_t* bytes);
 struct e2e_detector;

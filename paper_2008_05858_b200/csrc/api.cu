@@ -95,7 +95,9 @@ using namespace e2e;
 struct HostPipe {
     static constexpr int kEvents = 16;
     cudaStream_t copy = nullptr;
+    cudaStream_t aux = nullptr;        // second compute stream: odd bands render here while even bands render on the caller's
     cudaEvent_t ev[kEvents] = {};
+    cudaEvent_t ev_start = nullptr, ev_aux_done = nullptr;
     std::mutex mu;
 };
 static HostPipe* host_pipe()
@@ -107,7 +109,10 @@ static HostPipe* host_pipe()
     std::lock_guard<std::mutex> lk(mu);
     if (!pipes[dev]) {
         HostPipe* h = new HostPipe;
-        bool ok = cudaStreamCreateWithFlags(&h->copy, cudaStreamNonBlocking) == cudaSuccess;
+        bool ok = cudaStreamCreateWithFlags(&h->copy, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&h->aux, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&h->ev_aux_done, cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; ok && i < HostPipe::kEvents; ++i) ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { delete h; return nullptr; }
         pipes[dev] = h;
@@ -694,14 +699,27 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         std::vector<int> band_of(n_strips, 0);
         long long acc = 0;
         const long long tot = std::max<long long>(pl->total_samples, 1);
+        // A band may only start at a GAP -- a strip whose first row lies above every row of the strips before it -- so that
+        // no pixel belongs to two bands: bands can then be rendered concurrently (two streams) and the rows of a band are
+        // final as soon as that band alone is done.  Without enough gaps (orders that overlap everywhere) there are fewer
+        // bands, down to one.
+        std::vector<int> rhi(n_strips, INT_MIN);
+        for (int s = 0; s < n_strips; ++s)
+            for (int B = 0; B < nB; ++B)
+                if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B]) rhi[s] = std::max(rhi[s], cov_hi[(size_t)s * nB + B]);
+        int cur_band = 0, top = INT_MIN;
         for (int i = 0; i < n_strips; ++i) {
             const int s = order[i];
+            if (pl->strips[s].n == 0) { band_of[s] = cur_band; continue; }
             const double frac = (double)acc / (double)tot;
             int b = 0;
             while (b < want - 1 && frac >= cum[b + 1]) ++b;
-            band_of[s] = b;
+            if (b > cur_band && rlo[s] > top) cur_band = std::min(b, cur_band + 1);
+            band_of[s] = cur_band;
+            top = std::max(top, rhi[s]);
             acc += pl->strips[s].n;
         }
+        want = cur_band + 1;
         pl->n_bands = want;
         pl->n_phases_all = (int)phases.size();
         pl->band_fin_row.assign(want, ny);
@@ -1094,11 +1112,15 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
         return fail(E2E_ERR_INVALID_ARG, "render_frame_host: non-finite detector parameter");
     std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
     E2E_CUDA(cudaMemsetAsync(d_frame, 0, frame_bytes, stream));
+    // bands share no pixel (build_plan): even bands on the caller's stream, odd bands on the library's second stream
+    E2E_CUDA(cudaEventRecord(hp->ev_start, stream));
+    E2E_CUDA(cudaStreamWaitEvent(hp->aux, hp->ev_start, 0));
     int row0 = 0;
     for (int b = 0; b < pl->n_bands; ++b) {
-        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, stream, b);          // a1-a3 of this band's strips only
+        cudaStream_t cs = (b & 1) ? hp->aux : stream;
+        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, b);              // a1-a3 of this band's strips only
         if (rc) return rc;
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, pl->d_band_items,
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, pl->d_band_items,
                            pl->band_phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
         if (rc) return rc;
         const int row1 = std::max(row0, pl->band_fin_row[b]);
@@ -1106,16 +1128,18 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
             const size_t off = (size_t)row0 * nx;
             const long long npx = (long long)(row1 - row0) * nx;
             if (det) {
-                rc = launch_detector(d_frame + off, d_frame + off, npx, *det, stream, (long long)off);
+                rc = launch_detector(d_frame + off, d_frame + off, npx, *det, cs, (long long)off);
                 if (rc) return rc;
             }
             cudaEvent_t ev = hp->ev[b % HostPipe::kEvents];
-            E2E_CUDA(cudaEventRecord(ev, stream));
+            E2E_CUDA(cudaEventRecord(ev, cs));
             E2E_CUDA(cudaStreamWaitEvent(hp->copy, ev, 0));
             E2E_CUDA(cudaMemcpyAsync(h_frame + off, d_frame + off, (size_t)npx * 8, cudaMemcpyDeviceToHost, hp->copy));
             row0 = row1;
         }
     }
+    E2E_CUDA(cudaEventRecord(hp->ev_aux_done, hp->aux));
+    E2E_CUDA(cudaStreamWaitEvent(stream, hp->ev_aux_done, 0));
     E2E_CUDA(cudaStreamSynchronize(stream));
     E2E_CUDA(cudaStreamSynchronize(hp->copy));
     (void)ny;

@@ -147,7 +147,9 @@ E2E_API int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spe
  * Deterministic: the same inputs give the same bits (every pixel's additions happen in a fixed order).  Asynchronous on cuda_stream
  * (a cudaStream_t, NULL = default stream); launch errors are returned, later device faults surface at the
  * caller's next synchronisation.  The call allocates nothing on the device except, the first time a
- * (format, psf) pair is seen, the cached schedule (a few hundred KB). */
+ * (format, psf) pair is seen, the cached schedule (a few hundred KB). 
+ * Part of the work is enqueued on a stream owned by the library that forks from and joins cuda_stream (two row bands
+ * that share no pixel are rendered concurrently); to the caller the call is ordered on cuda_stream as a whole. */
 E2E_API int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                      double* d_frame, int32_t accumulate, void* d_workspace, size_t workspace_bytes,
                      void* cuda_stream);

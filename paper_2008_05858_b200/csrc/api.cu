@@ -36,6 +36,7 @@ int measure_fp64_peak(int repeats, double* burst, double* sustained);
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
 constexpr long long kSmallFrameItems = 4736;   // 2 x (148 SMs x 16 resident warps): below this a K = 2 schedule leaves the GPU idle
+constexpr int kDeviceParts = 2;        // row bands e2e_render_frame renders concurrently (they share no pixel)
 constexpr int kHostBands = 8;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -96,6 +97,8 @@ struct HostPipe {
     static constexpr int kEvents = 16;
     cudaStream_t copy = nullptr;
     cudaStream_t aux = nullptr;        // second compute stream: odd bands render here while even bands render on the caller's
+    cudaStream_t aux2[2] = {};         // device path with 3 / 4 concurrent parts
+    cudaEvent_t ev_aux2_done[2] = {};
     cudaEvent_t ev[kEvents] = {};
     cudaEvent_t ev_start = nullptr, ev_aux_done = nullptr;
     std::mutex mu;
@@ -113,6 +116,9 @@ static HostPipe* host_pipe()
                   cudaStreamCreateWithFlags(&h->aux, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) == cudaSuccess &&
                   cudaEventCreateWithFlags(&h->ev_aux_done, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; ok && i < 2; ++i)
+            ok = cudaStreamCreateWithFlags(&h->aux2[i], cudaStreamNonBlocking) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&h->ev_aux2_done[i], cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; ok && i < HostPipe::kEvents; ++i) ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { delete h; return nullptr; }
         pipes[dev] = h;
@@ -124,8 +130,10 @@ e2e_plan::~e2e_plan()
 {
     if (d_strips) cudaFree(d_strips);
     if (d_items) cudaFree(d_items);
-    if (d_band_items) cudaFree(d_band_items);
-    if (d_band_strips) cudaFree(d_band_strips);
+    for (BandPart* bp : {&host, &halves}) {
+        if (bp->d_items) cudaFree(bp->d_items);
+        if (bp->d_strips) cudaFree(bp->d_strips);
+    }
 }
 
 extern "C" {
@@ -668,87 +676,94 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
     E2E_CUDA(cudaMemcpy(pl->d_strips, pl->strips.data(), sizeof(Strip) * n_strips, cudaMemcpyHostToDevice));
     E2E_CUDA(cudaMalloc(&pl->d_items, sizeof(Item) * std::max<size_t>(1, flat.size())));
     if (!flat.empty()) E2E_CUDA(cudaMemcpy(pl->d_items, flat.data(), sizeof(Item) * flat.size(), cudaMemcpyHostToDevice));
-    // ---- row bands for the host path: strips sorted by their first row, split into bands of about equal sample counts
+    // ---- row bands: strips sorted by their first row, split into bands by sample count, bands starting only at gaps
     {
         const int ny = F->view.ny;
-        std::vector<int> rlo(n_strips, INT_MAX);
+        std::vector<int> rlo(n_strips, INT_MAX), rhi(n_strips, INT_MIN);
         for (int s = 0; s < n_strips; ++s)
             for (int B = 0; B < nB; ++B)
-                if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B]) rlo[s] = std::min(rlo[s], cov_lo[(size_t)s * nB + B]);
+                if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B]) {
+                    rlo[s] = std::min(rlo[s], cov_lo[(size_t)s * nB + B]);
+                    rhi[s] = std::max(rhi[s], cov_hi[(size_t)s * nB + B]);
+                }
         std::vector<int> order(n_strips);
         for (int s = 0; s < n_strips; ++s) order[s] = s;
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rlo[a] < rlo[b]; });
-        // 8 bands of growing size when a band's launches are few (2 colours x 2 classes); frames with many colours (10
-        // fibers per order: 10 launches per band) measured better with 6 equal bands
+        pl->n_phases_all = (int)phases.size();
+        const long long tot = std::max<long long>(pl->total_samples, 1);
+        auto build_part = [&](int want, bool ramp, e2e_plan::BandPart& part) -> int {
+            // band b takes the share wgt[b] of the samples; ramp: the first bands are small, so that the copy engine starts
+            // early, the later ones up to 3x larger (the copy is the slower side and must only never run dry)
+            std::vector<double> cum(want + 1, 0.0);
+            {
+                std::vector<double> wgt(want, 1.0);
+                if (ramp)
+                    for (int b = 0; b < want; ++b) wgt[b] = 1.0 + 2.0 * (double)b / (double)std::max(1, want - 1);
+                double sum = 0.0;
+                for (double w : wgt) sum += w;
+                for (int b = 0; b < want; ++b) cum[b + 1] = cum[b] + wgt[b] / sum;
+            }
+            // A band may only start at a GAP -- a strip whose first row lies above every row of the strips before it -- so
+            // that no pixel belongs to two bands: bands can be rendered concurrently (two streams) and the rows of a band
+            // are final as soon as that band alone is done.  Without enough gaps (orders that overlap everywhere) there are
+            // fewer bands, down to one.
+            std::vector<int> band_of(n_strips, 0);
+            long long acc = 0;
+            int cur_band = 0, top = INT_MIN;
+            for (int i = 0; i < n_strips; ++i) {
+                const int s = order[i];
+                if (pl->strips[s].n == 0) { band_of[s] = cur_band; continue; }
+                const double frac = (double)acc / (double)tot;
+                int b = 0;
+                while (b < want - 1 && frac >= cum[b + 1]) ++b;
+                if (b > cur_band && rlo[s] > top) cur_band = std::min(b, cur_band + 1);
+                band_of[s] = cur_band;
+                top = std::max(top, rhi[s]);
+                acc += pl->strips[s].n;
+            }
+            want = cur_band + 1;
+            part.n_bands = want;
+            part.fin_row.assign(want, ny);
+            for (int b = want - 2; b >= 0; --b) {
+                int lo = part.fin_row[b + 1];
+                for (int s = 0; s < n_strips; ++s)
+                    if (band_of[s] == b + 1 && pl->strips[s].n > 0) lo = std::min(lo, rlo[s]);
+                part.fin_row[b] = std::max(0, std::min(lo, ny));
+            }
+            std::vector<Item> bflat;
+            part.phase_off.assign((size_t)want * (phases.size() + 1), 0);
+            for (int b = 0; b < want; ++b)
+                for (size_t ph = 0; ph <= phases.size(); ++ph) {
+                    part.phase_off[(size_t)b * (phases.size() + 1) + ph] = (int)bflat.size();
+                    if (ph == phases.size()) break;
+                    for (const Item& it : phases[ph])
+                        if (band_of[it.strip] == b) bflat.push_back(it);
+                }
+            std::vector<int> bstrips;
+            part.strip_off.assign(want + 1, 0);
+            for (int b = 0; b < want; ++b) {
+                for (int s = 0; s < n_strips; ++s)
+                    if (band_of[s] == b && pl->strips[s].n > 0) bstrips.push_back(s);
+                part.strip_off[b + 1] = (int)bstrips.size();
+            }
+            E2E_CUDA(cudaMalloc(&part.d_strips, sizeof(int) * std::max<size_t>(1, bstrips.size())));
+            if (!bstrips.empty()) E2E_CUDA(cudaMemcpy(part.d_strips, bstrips.data(), sizeof(int) * bstrips.size(), cudaMemcpyHostToDevice));
+            E2E_CUDA(cudaMalloc(&part.d_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
+            if (!bflat.empty()) E2E_CUDA(cudaMemcpy(part.d_items, bflat.data(), sizeof(Item) * bflat.size(), cudaMemcpyHostToDevice));
+            return E2E_OK;
+        };
+        // host path: 8 bands of growing size when a band's launches are few (2 colours x 2 classes); frames with many
+        // colours (10 fibers per order: 10 launches per band) measured better with 6 equal bands
         const bool many_phases = phases.size() > 4;
         int want = many_phases ? 6 : kHostBands;
         if (const char* e = getenv("E2E_HOST_BANDS")) want = std::max(1, std::min(atoi(e), 16));
-        // band b takes the share wgt[b] of the samples: the first bands are small, so that the copy engine starts early,
-        // the later ones up to 3x larger (the copy is the slower side and must only never run dry); E2E_HOST_BAND_RAMP=0:
-        // equal shares
-        std::vector<double> cum(want + 1, 0.0);
-        {
-            const char* ramp = getenv("E2E_HOST_BAND_RAMP");
-            std::vector<double> wgt(want, 1.0);
-            if (ramp ? ramp[0] != '0' : !many_phases)
-                for (int b = 0; b < want; ++b) wgt[b] = 1.0 + 2.0 * (double)b / (double)std::max(1, want - 1);
-            double sum = 0.0;
-            for (double w : wgt) sum += w;
-            for (int b = 0; b < want; ++b) cum[b + 1] = cum[b] + wgt[b] / sum;
-        }
-        std::vector<int> band_of(n_strips, 0);
-        long long acc = 0;
-        const long long tot = std::max<long long>(pl->total_samples, 1);
-        // A band may only start at a GAP -- a strip whose first row lies above every row of the strips before it -- so that
-        // no pixel belongs to two bands: bands can then be rendered concurrently (two streams) and the rows of a band are
-        // final as soon as that band alone is done.  Without enough gaps (orders that overlap everywhere) there are fewer
-        // bands, down to one.
-        std::vector<int> rhi(n_strips, INT_MIN);
-        for (int s = 0; s < n_strips; ++s)
-            for (int B = 0; B < nB; ++B)
-                if (cov_lo[(size_t)s * nB + B] <= cov_hi[(size_t)s * nB + B]) rhi[s] = std::max(rhi[s], cov_hi[(size_t)s * nB + B]);
-        int cur_band = 0, top = INT_MIN;
-        for (int i = 0; i < n_strips; ++i) {
-            const int s = order[i];
-            if (pl->strips[s].n == 0) { band_of[s] = cur_band; continue; }
-            const double frac = (double)acc / (double)tot;
-            int b = 0;
-            while (b < want - 1 && frac >= cum[b + 1]) ++b;
-            if (b > cur_band && rlo[s] > top) cur_band = std::min(b, cur_band + 1);
-            band_of[s] = cur_band;
-            top = std::max(top, rhi[s]);
-            acc += pl->strips[s].n;
-        }
-        want = cur_band + 1;
-        pl->n_bands = want;
-        pl->n_phases_all = (int)phases.size();
-        pl->band_fin_row.assign(want, ny);
-        for (int b = want - 2; b >= 0; --b) {
-            int lo = pl->band_fin_row[b + 1];
-            for (int s = 0; s < n_strips; ++s)
-                if (band_of[s] == b + 1 && pl->strips[s].n > 0) lo = std::min(lo, rlo[s]);
-            pl->band_fin_row[b] = std::max(0, std::min(lo, ny));
-        }
-        std::vector<Item> bflat;
-        pl->band_phase_off.assign((size_t)want * (phases.size() + 1), 0);
-        for (int b = 0; b < want; ++b)
-            for (size_t ph = 0; ph <= phases.size(); ++ph) {
-                pl->band_phase_off[(size_t)b * (phases.size() + 1) + ph] = (int)bflat.size();
-                if (ph == phases.size()) break;
-                for (const Item& it : phases[ph])
-                    if (band_of[it.strip] == b) bflat.push_back(it);
-            }
-        std::vector<int> bstrips;
-        pl->band_strip_off.assign(want + 1, 0);
-        for (int b = 0; b < want; ++b) {
-            for (int s = 0; s < n_strips; ++s)
-                if (band_of[s] == b && pl->strips[s].n > 0) bstrips.push_back(s);
-            pl->band_strip_off[b + 1] = (int)bstrips.size();
-        }
-        E2E_CUDA(cudaMalloc(&pl->d_band_strips, sizeof(int) * std::max<size_t>(1, bstrips.size())));
-        if (!bstrips.empty()) E2E_CUDA(cudaMemcpy(pl->d_band_strips, bstrips.data(), sizeof(int) * bstrips.size(), cudaMemcpyHostToDevice));
-        E2E_CUDA(cudaMalloc(&pl->d_band_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
-        if (!bflat.empty()) E2E_CUDA(cudaMemcpy(pl->d_band_items, bflat.data(), sizeof(Item) * bflat.size(), cudaMemcpyHostToDevice));
+        const char* rampenv = getenv("E2E_HOST_BAND_RAMP");
+        int rc = build_part(want, rampenv ? rampenv[0] != '0' : !many_phases, pl->host);
+        if (rc) return rc;
+        int parts = kDeviceParts;
+        if (const char* e = getenv("E2E_DEVICE_PARTS")) parts = std::max(1, std::min(atoi(e), 4));
+        rc = build_part(parts, false, pl->halves);
+        if (rc) return rc;
     }
     *out = pl.get();
     F->plans.push_back(std::move(pl));
@@ -769,7 +784,7 @@ static int check_spectra(const e2e_format* F, const e2e_spectrum_t* spectra, con
 }
 
 static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spectrum_t* spectra, double* d_x, double* d_y,
-                        double* d_w, cudaStream_t stream, int band = -1)
+                        double* d_w, cudaStream_t stream, const e2e_plan::BandPart* part = nullptr, int band = -1)
 {
     SpectraParam sp;
     memset(&sp, 0, sizeof(sp));
@@ -779,9 +794,9 @@ static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spect
     if (nmax == 0) return E2E_OK;
     const int* ids = nullptr;
     int ny_grid = pl->n_strips;
-    if (band >= 0) {                                            // one row band of the host path
-        ids = pl->d_band_strips + pl->band_strip_off[band];
-        ny_grid = pl->band_strip_off[band + 1] - pl->band_strip_off[band];
+    if (part && band >= 0) {                                    // one row band
+        ids = part->d_strips + part->strip_off[band];
+        ny_grid = part->strip_off[band + 1] - part->strip_off[band];
         if (ny_grid == 0) return E2E_OK;
     }
     dim3 grid((unsigned)((nmax + 255) / 256), (unsigned)ny_grid);
@@ -971,7 +986,29 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     {
         StageTimer tm(kStageRender, stream);
         const long long before = g_launches.load();
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+        const int nparts = pl->halves.n_bands;
+        HostPipe* hp = nparts >= 2 ? host_pipe() : nullptr;
+        if (hp) {
+            // row bands that share no pixel, rendered concurrently: the tail of one band's launch (a few long items on
+            // otherwise idle SMs) overlaps the other bands' work.  Fork to the library's streams and join.
+            std::lock_guard<std::mutex> lk(hp->mu);
+            const int np1 = pl->n_phases_all + 1;
+            cudaStream_t sp[4] = {stream, hp->aux, hp->aux2[0], hp->aux2[1]};
+            cudaEvent_t done[4] = {nullptr, hp->ev_aux_done, hp->ev_aux2_done[0], hp->ev_aux2_done[1]};
+            cudaError_t ce = cudaEventRecord(hp->ev_start, stream);
+            for (int b = 1; b < nparts && ce == cudaSuccess; ++b) ce = cudaStreamWaitEvent(sp[b], hp->ev_start, 0);
+            if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: fork");
+            for (int b = 0; b < nparts && !rc; ++b)
+                rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, sp[b], pl->halves.d_items,
+                                   pl->halves.phase_off.data() + (size_t)b * np1, pl->n_phases_all);
+            for (int b = 1; b < nparts && ce == cudaSuccess; ++b) {
+                ce = cudaEventRecord(done[b], sp[b]);
+                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, done[b], 0);
+            }
+            if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: join");
+        } else {
+            rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+        }
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
     }
     return rc;
@@ -1088,7 +1125,7 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
     rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
     HostPipe* hp = host_pipe();
-    if (pl->n_bands <= 1 || !hp) {
+    if (pl->host.n_bands <= 1 || !hp) {
         // one pass: render, detector, copy
         rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
         if (rc) return rc;
@@ -1116,14 +1153,14 @@ int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e
     E2E_CUDA(cudaEventRecord(hp->ev_start, stream));
     E2E_CUDA(cudaStreamWaitEvent(hp->aux, hp->ev_start, 0));
     int row0 = 0;
-    for (int b = 0; b < pl->n_bands; ++b) {
+    for (int b = 0; b < pl->host.n_bands; ++b) {
         cudaStream_t cs = (b & 1) ? hp->aux : stream;
-        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, b);              // a1-a3 of this band's strips only
+        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &pl->host, b);   // a1-a3 of this band's strips only
         if (rc) return rc;
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, pl->d_band_items,
-                           pl->band_phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, pl->host.d_items,
+                           pl->host.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
         if (rc) return rc;
-        const int row1 = std::max(row0, pl->band_fin_row[b]);
+        const int row1 = std::max(row0, pl->host.fin_row[b]);
         if (row1 > row0) {
             const size_t off = (size_t)row0 * nx;
             const long long npx = (long long)(row1 - row0) * nx;

@@ -176,16 +176,18 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     e2e::Item* d_items = nullptr;
     int n_items = 0;
     int n_colors = 0;
-    // host path (e2e_render_frame_host): the same items regrouped into row bands so that finished rows can travel to
-    // the host while later bands render.  band_phase_off[b * (n_phases_all + 1) + ph] indexes d_band_items; rows below
-    // band_fin_row[b] are final once band b has been rendered (no later band writes them)
-    int n_bands = 0;
-    int n_phases_all = 0;          // phases before empty ones were dropped (colour x parity)
-    std::vector<int> band_phase_off;
-    std::vector<int> band_fin_row;
-    e2e::Item* d_band_items = nullptr;
-    std::vector<int> band_strip_off;   // [n_bands + 1] into d_band_strips: the strips of each band
-    int* d_band_strips = nullptr;
+    // The same items regrouped into row bands that share no pixel (build_plan).  `host`: up to 8 bands of growing size for
+    // e2e_render_frame_host (finished rows travel to the host while later bands render); `halves`: 2 equal bands that
+    // e2e_render_frame renders concurrently on two streams (the tail of one band's launch overlaps the other band's work).
+    // phase_off[b * (n_phases_all + 1) + ph] indexes d_items; rows below fin_row[b] belong to bands <= b only.
+    struct BandPart {
+        int n_bands = 0;
+        std::vector<int> phase_off, fin_row, strip_off;
+        e2e::Item* d_items = nullptr;
+        int* d_strips = nullptr;
+    };
+    BandPart host, halves;
+    int n_phases_all = 0;          // phases before empty ones were dropped (colour x class)
     ~e2e_plan();
 };
 

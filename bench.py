@@ -35,8 +35,8 @@ C_ERFC, C_PSI = 60.0, 90.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture of this command (profiles/, file named beside each value); None = not captured for that kernel
 NCU_TRAFFIC_BYTES = {
-    # profiles/r1_v7_espresso.md, launch ids 1-4 (dram__bytes_read.sum + dram__bytes_write.sum, mean)
-    "render_moment_kernel<2>": 550.9e6,
+    # profiles/r1_v8_espresso.md, launch ids 1-8 (dram__bytes_read.sum + dram__bytes_write.sum, mean over the 8 launches of a step)
+    "render_moment_kernel<2>": 258.7e6,
 }
 
 

@@ -167,12 +167,19 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         const double dy = __dsub_rn(__dsub_rn(yk, (double)jlo), Q.c0y);
         __syncwarp();                                          // previous batch's readers are done
         {
-            double vx = wk;
+            // w dx^p by repeated squaring: the same number of multiplications, dependency depth log2(NP) instead of NP
+            double v[NP];
+            v[0] = wk;
+            double sq = dx;
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                S.vx[p * kMomLdk + lane] = vx;
-                vx *= dx;
+            for (int h = 1; h < NP; h *= 2) {
+#pragma unroll
+                for (int p = 0; p < h; ++p)
+                    if (h + p < NP) v[h + p] = v[p] * sq;
+                sq *= sq;
             }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) S.vx[p * kMomLdk + lane] = v[p];
         }
         __syncwarp();
         int pos = 0;
@@ -202,12 +209,15 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
             // powers of delta for this run (delta is relative to the cell's window, so they are staged per run)
             __syncwarp();                                      // the previous run's step-1 reads of vy are done
             {
-                double vy = 1.0;
-#pragma unroll
-                for (int p = 0; p < 8; ++p) {
-                    S.vy[p * kMomLdk + lane] = vy;
-                    vy *= dl;
-                }
+                const double d2 = dl * dl, d3 = d2 * dl, d4 = d2 * d2;
+                S.vy[0 * kMomLdk + lane] = 1.0;
+                S.vy[1 * kMomLdk + lane] = dl;
+                S.vy[2 * kMomLdk + lane] = d2;
+                S.vy[3 * kMomLdk + lane] = d3;
+                S.vy[4 * kMomLdk + lane] = d4;
+                S.vy[5 * kMomLdk + lane] = d4 * dl;
+                S.vy[6 * kMomLdk + lane] = d4 * d2;
+                S.vy[7 * kMomLdk + lane] = d4 * d3;
             }
             __syncwarp();
             // ---- step 1: MT += VX VY^T over the samples [pos, pend)

@@ -98,7 +98,7 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
                     for (int b = 0; b < 3; ++b) { out[a][b][0] = 0.0; out[a][b][1] = 0.0; }
-#pragma unroll 1
+#pragma unroll 2                                        // two terms in flight: step 2 of one overlaps step 3 of the other
                 for (int t = 0; t < Q.T; ++t) {
                     const double2* fy = Q.fy + ((size_t)(cYb * Q.T + t) * Q.njt + jp) * 32 + lane;
                     const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;

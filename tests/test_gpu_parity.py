@@ -434,6 +434,42 @@ def test_render_frame_host_banded_pipeline(B):
         r.close()
 
 
+def test_concurrent_renders_on_two_streams_from_two_threads(B):
+    """include/e2e.h: handles are read-only during render, so concurrent renders on different streams into different
+    frames are legal.  Two host threads render two different scenes repeatedly on their own streams (the library's fork /
+    join stream and events are shared between the calls); every frame must equal the serial result bit for bit"""
+    import threading
+    import torch
+    sa = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 3, 40, 41, 42, 84])
+    sb = small_tiny(spp=40.0, lam=(5005.0, 5045.0))
+    ra, rb = B.Renderer(sa), B.Renderer(sb)
+    try:
+        ref_a, ref_b = ra.render().clone(), rb.render().clone()
+        torch.cuda.synchronize()
+        errors = []
+
+        def work(r, ref, n):
+            try:
+                st = torch.cuda.Stream()
+                fr = torch.empty_like(ref)
+                for _ in range(n):
+                    with torch.cuda.stream(st):
+                        B.e2e_render_frame(r.fmt, r.psf, r.spectra, fr, False, r.workspace, st)
+                    st.synchronize()
+                    if not torch.equal(fr, ref):
+                        errors.append("frame differs from the serial render")
+                        return
+            except Exception as e:                                  # noqa: BLE001
+                errors.append(repr(e))
+
+        ta = threading.Thread(target=work, args=(ra, ref_a, 6))
+        tb = threading.Thread(target=work, args=(rb, ref_b, 40))
+        ta.start(); tb.start(); ta.join(); tb.join()
+        assert not errors, errors
+    finally:
+        ra.close(); rb.close()
+
+
 # ------------------------------------------------------------------------------------------ a6 detector
 def test_detector_bit_exact(B):
     import torch

@@ -275,6 +275,22 @@ def test_render_espresso_full_frame_windows(B, espresso_gpu):
     assert worst <= 1.0
 
 
+def test_render_espresso_whole_order_both_fibers(B, espresso_gpu):
+    """one whole order (index 40, both fibers, all 9216 columns, every row either fiber touches) of the full-size frame
+    against the oracle, element by element: ~577 k samples, several thousand footprint cells, both strip ends"""
+    s, G = espresso_gpu
+    o = 40
+    n = oracle.order_nsamples(s, o)
+    ys = np.concatenate([oracle.samples(s, f, o, k, k + 1)[2] for f in (0, 1) for k in range(0, n, n // 64)] +
+                        [oracle.samples(s, f, o, n - 1, n)[2] for f in (0, 1)])
+    j0, j1 = int(np.floor(ys.min())) - 16, int(np.ceil(ys.max())) + 16
+    O = oracle.render(s, window=(0, j0, s.nx, j1 - j0))
+    assert oracle.render.last_touched == 2 * n                      # every sample of both fibers is inside the window
+    assert np.all(O[0] == 0.0) and np.all(O[-1] == 0.0)             # and nothing else reaches it (orders are 92 px apart)
+    e = assert_frame_parity(G[j0:j1], O, "order 40, both fibers, full x range")
+    assert e["max_rel_core"] < 1e-11
+
+
 def test_render_espresso_flux_conservation_and_gaps(B, espresso_gpu):
     s, G = espresso_gpu
     tot = oracle.total_weight(s)
@@ -308,7 +324,6 @@ def test_render_hires_full_frame_windows(B):
 def small_field_scene(gx=3, gy=2, npix=7, os=4, seed=77, nx=300, ny=120):
     s = small_tiny(spp=3.0, lam=(5010.0, 5013.0))
     s.nx, s.ny = nx, ny
-    s.coef_x = np.array([150.0, 2400.0, 1.0, 0.0])        # u in [-0.6, -0.48] -> x spans the whole 300-px detector... see below
     s.coef_x = np.array([1590.0, 2400.0, 1.0, 0.0])       # x = 1590 + 2400 u: u = -0.6 -> 150.4 ; u = -0.48 -> 438
     s.lam_max = np.array([5012.5])                        # u = -0.5 -> 390 - ... keeps part of the trace off the detector (G11)
     s.coef_y = np.array([60.0, 40.0, 0.0, 0.0])
@@ -419,10 +434,21 @@ def test_render_frame_host_banded_pipeline(B):
         mx = dev.max()
         assert np.abs(H - dev).max() <= 1e-13 * mx
         assert np.array_equal(H == 0.0, dev == 0.0)
+        # the host path against the ORACLE (not only against the device path): windows at strip ends, fiber overlaps, band seams
+        for o, frac in ((0, 0.001), (1, 0.5), (3, 0.25), (4, 0.999), (6, 0.6)):
+            n = oracle.order_nsamples(s, o)
+            k = int(frac * (n - 1))
+            lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
+            i0, j0 = max(0, int(x[0]) - 24), max(0, int(y[0]) - 20)
+            O = oracle.render(s, window=(i0, j0, 48, 40))
+            assert O.max() > 0
+            assert_frame_parity(H[j0:j0 + 40, i0:i0 + 48], O, f"host path window {i0},{j0}")
         out.fill_(float("nan"))
         B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws, det=det)
         Hn = out.numpy()
         assert np.isfinite(Hn).all()
+        # a6 of the host path is bit-exact against the oracle's detector stage applied to the host path's own noise-free frame
+        assert np.array_equal(Hn, oracle.detector(H, det))
         # identical draws; a last-bit difference of mu can move a Poisson count only at a rounding boundary
         assert (Hn == dev_noisy).mean() > 0.9999
         assert np.abs(Hn - dev_noisy).max() <= 2.0
@@ -534,8 +560,8 @@ def test_detector_ex_bit_exact(B):
 
 def test_render_frames_batch_equals_single_renders(B):
     """batch render on fixed geometry.  The five Doppler-shifted frames of the RV sweep in one call are,
-    frame by frame, the bits of five single renders (and frame 0 passes the oracle parity of the other tests);
-    the sparse-sampling scene takes the frame-after-frame route of the non-production kernels"""
+    frame by frame, the bits of five single renders, and every one of them matches the oracle's render of that velocity
+    per pixel; the sparse-sampling scene takes the frame-after-frame route of the non-production kernels"""
     import torch
     for make in (lambda v: W.rv_sweep(v), lambda v: _sparse_rv(v)):
         scenes = [make(v) for v in (0.0, 0.01, 0.1, 1.0, 10.0)]
@@ -559,6 +585,10 @@ def test_render_frames_batch_equals_single_renders(B):
             torch.cuda.synchronize()
             for a, b in zip(frames, singles):
                 assert torch.equal(a, b)
+            for a, sc in zip(frames, scenes):                        # every frame of the batch against the oracle, per pixel
+                O = oracle.render(sc)
+                assert O.max() > 0
+                assert_frame_parity(a.cpu().numpy(), O, f"batch frame {sc.name} v={sc.notes.get('v_mps')}")
             assert not torch.equal(frames[0], frames[4])            # the shift is there
             # accumulate = 1 adds on top
             B.e2e_render_frames(r.fmt, r.psf, descs, frames, True, ws)
@@ -580,9 +610,11 @@ def _sparse_rv(v):
 
 
 def test_rv_sweep_photocenter_linear_in_velocity(B):
-    """BASELINE.json configs[4]: 5 Doppler-shifted frames; global photocenter shift vs the analytic slope and
-    per-line centroid residual against a straight line in v < 1e-6 px; GPU == oracle on the v = 10 m/s frame;
-    detector stage bit-exact on the rendered frame"""
+    """BASELINE.json configs[4]: 5 Doppler-shifted frames.  DESIGN.md G14 (the CPU-only pin of the same three checks is
+    tests/test_oracle_render.py::test_g14_rv_sweep_photocenter_linear_in_velocity): (i) global photocenter == flux-weighted
+    mean of the oracle's mapped samples at every velocity; (ii) residual against a least-squares line in v < 1e-6 px,
+    globally and per line; (iii) shift == closed-form slope of the line list INCLUDING the blaze-slope term to 1e-7 px.
+    GPU == oracle per pixel on the v = 10 m/s frame; detector stage bit-exact on the rendered frame"""
     import torch
     frames, xc = [], []
     for v in W.RV_SWEEP_V:
@@ -606,6 +638,19 @@ def test_rv_sweep_photocenter_linear_in_velocity(B):
     coef, *_ = np.linalg.lstsq(A, np.array(xc), rcond=None)
     assert np.max(np.abs(np.array(xc) - A @ coef)) < 1e-6
     assert 1e-3 < xc[-1] - xc[0] < 1e-2
+    # (iii) closed-form slope (G14): d xbar / d beta = [sum W lam X' + sum E' lam (X - xbar)] / sum W over the 200 lines
+    cen = W.rv_sweep(0.0).notes["line_centers"]
+    Xf = lambda l: 1024 + 1000 * ((l - 5025) / 25) + ((l - 5025) / 25) ** 2
+    Xp = lambda l: (1000 + 2 * ((l - 5025) / 25)) / 25
+
+    def E(l):
+        a = np.pi * 100 * (5025.0 / l - 1)
+        return np.where(np.abs(a) < 1e-12, 1.0, (np.sin(a) / np.where(a == 0, 1.0, a)) ** 2)
+    Wl, h = E(cen), 1e-4
+    Ep = (E(cen + h) - E(cen - h)) / (2 * h)
+    xbar = (Wl * Xf(cen)).sum() / Wl.sum()
+    slope = ((Wl * cen * Xp(cen)).sum() + (Ep * cen * (Xf(cen) - xbar)).sum()) / Wl.sum()
+    assert np.max(np.abs((np.array(xc) - xc[0]) - slope * v / W.C_LIGHT)) < 1e-7
     # per-line windows (Voronoi cells of integer columns between line positions)
     cen = W.rv_sweep(0.0).notes["line_centers"]
     xl = 1024 + 1000 * (cen - 5025) / 25 + ((cen - 5025) / 25) ** 2

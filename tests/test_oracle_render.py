@@ -243,3 +243,64 @@ def test_p9_integer_translation():
     b = oracle.render(t, window=(387, 97, 180, 80))
     assert np.allclose(a, b, rtol=1e-10, atol=1e-14 * a.max())
     assert a.max() > 0
+
+
+# ---------------------------------------------------------------- G14: RV sweep ("cm/s")
+def _rv_crop(v):
+    s = W.rv_sweep(v)
+    s.lam_min = np.array([5010.0]); s.lam_max = np.array([5014.0])       # 16 of the 200 lines, 256 samples/px
+    return s
+
+
+def test_g14_rv_sweep_photocenter_linear_in_velocity():
+    """BASELINE.json configs[4] on a crop of the RV-sweep scene, oracle only.  DESIGN.md G14 (re-read in round 2):
+    (i) P5 at every velocity: the frame's global photocenter is the flux-weighted mean of the mapped samples (1e-9 px);
+    (ii) it moves linearly with v: residual against a least-squares line through the 5 velocities < 1e-6 px, globally and per
+    line (Voronoi windows of integer columns between line positions);
+    (iii) the slope is the closed form of the line list: with W_l = E(lam_l), X_l = X(lam_l), xbar = sum W X / sum W,
+          d xbar / d beta = [ sum_l W_l lam_l X'(lam_l)  +  sum_l E'(lam_l) lam_l (X_l - xbar) ] / sum_l W_l ,   beta = v / c.
+    The second sum is the blaze-slope term: a Doppler shift moves every line along the blaze function, so the lines'
+    relative weights change and the *global* centroid moves even where no line moved.  SURVEY 8(c) G14 wrote the slope
+    without it (sum w X' lam / c); on this crop that formula is off by 5.9e-5 px at 10 m/s, the full one by < 2e-8 px."""
+    v = np.array(W.RV_SWEEP_V)
+    beta = v / W.C_LIGHT
+    xc, xs, frames = [], [], []
+    for vv in W.RV_SWEEP_V:
+        s = _rv_crop(vv)
+        lam, x, y, w = oracle.samples(s, 0, 0)
+        i0 = int(x.min()) - 12
+        wn = int(x.max()) + 12 - i0
+        fr = oracle.render(s, window=(i0, 100, wn, 80))
+        cols = i0 + np.arange(wn)
+        xc.append(float((fr.sum(axis=0) * cols).sum() / fr.sum()))
+        xs.append(float((w * x).sum() / w.sum()))
+        frames.append(fr)
+    xc, xs = np.array(xc), np.array(xs)
+    assert np.max(np.abs(xc - xs)) < 1e-9                                       # (i)
+    A = np.vstack([v, np.ones_like(v)]).T
+    coef, *_ = np.linalg.lstsq(A, xc, rcond=None)
+    assert np.max(np.abs(xc - A @ coef)) < 1e-6                                 # (ii) global
+    cen = W.rv_sweep(0.0).notes["line_centers"]
+    cen = cen[(cen > 5010.0) & (cen < 5014.0)]
+    assert len(cen) == 16
+    X = lambda l: 1024 + 1000 * ((l - 5025) / 25) + ((l - 5025) / 25) ** 2      # Tiny recipe (SURVEY 8(d))
+    Xp = lambda l: (1000 + 2 * ((l - 5025) / 25)) / 25
+
+    def E(l):                                                                  # G7 blaze, m = 100, lam_c = 5025
+        a = np.pi * 100 * (5025.0 / l - 1)
+        return (np.sin(a) / a) ** 2
+    edges = np.round(0.5 * (X(cen)[1:] + X(cen)[:-1])).astype(int) - i0
+    for ell in (1, 7, 14):                                                      # (ii) per line
+        c0, c1 = edges[ell - 1], edges[ell]
+        pcs = np.array([float((f[:, c0:c1].sum(axis=0) * np.arange(c0, c1)).sum() / f[:, c0:c1].sum()) for f in frames])
+        coef, *_ = np.linalg.lstsq(A, pcs, rcond=None)
+        assert np.max(np.abs(pcs - A @ coef)) < 1e-6
+        assert 5e-3 < pcs[-1] - pcs[0] < 8e-3                                   # ~ lam X' beta = 6.7e-3 px at 10 m/s
+    h = 1e-4
+    Ep = (E(cen + h) - E(cen - h)) / (2 * h)
+    Wl = E(cen)
+    xbar = (Wl * X(cen)).sum() / Wl.sum()
+    slope = ((Wl * cen * Xp(cen)).sum() + (Ep * cen * (X(cen) - xbar)).sum()) / Wl.sum()
+    assert np.max(np.abs((xc - xc[0]) - slope * beta)) < 1e-7                   # (iii) full closed form
+    naive = (Wl * cen * Xp(cen)).sum() / Wl.sum()
+    assert abs((xc[-1] - xc[0]) - naive * beta[-1]) > 1e-5                      # the survey's formula misses the blaze term

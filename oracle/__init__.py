@@ -93,8 +93,14 @@ def lib():
             L.orc_exp.argtypes = [C.c_double]
             L.orc_detector_draws.restype = None
             L.orc_detector_draws.argtypes = [C.c_void_p, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p]
-            L.orc_detector_ex.restype = None
+            L.orc_detector_ex.restype = C.c_int
             L.orc_detector_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
+            L.orc_log_series.restype = C.c_double
+            L.orc_log_series.argtypes = [C.c_double]
+            L.orc_sin2pi.restype = C.c_double
+            L.orc_sin2pi.argtypes = [C.c_double]
+            L.orc_gaussian_pair.restype = None
+            L.orc_gaussian_pair.argtypes = [C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -236,23 +242,57 @@ def detector(frame: np.ndarray, det, pixel_offset: int = 0) -> np.ndarray:
 
 class _DetectorEx(C.Structure):
     _fields_ = [("base", _Detector), ("prnu", C.c_void_p), ("dark", C.c_void_p),
-                ("full_well", C.c_double), ("e_per_adu", C.c_double), ("adu_max", C.c_double)]
+                ("full_well", C.c_double), ("e_per_adu", C.c_double), ("adu_max", C.c_double),
+                ("nx", C.c_int32), ("n_ports", C.c_int32), ("xtalk", C.c_void_p)]
 
 
 def detector_ex(frame: np.ndarray, det, prnu=None, dark=None, full_well: float = 0.0, e_per_adu: float = 0.0,
-                adu_max: float = 65535.0, pixel_offset: int = 0) -> np.ndarray:
-    """Full detector stage (detector_oracle.c orc_detector_ex): PRNU / dark maps, full-well saturation, ADC."""
+                adu_max: float = 65535.0, pixel_offset: int = 0, xtalk=None) -> np.ndarray:
+    """Full detector stage (detector_oracle.c orc_detector_ex): PRNU / dark maps, full-well saturation, ADC, and -- with
+    xtalk = [n_ports][n_ports] coupling matrix on a 2-D frame -- cross-talk between the read-out ports (G20)."""
     a = _f64(frame).reshape(-1)
     pr = _f64(prnu).reshape(-1) if prnu is not None else None
     dk = _f64(dark).reshape(-1) if dark is not None else None
     assert pr is None or pr.shape == a.shape
     assert dk is None or dk.shape == a.shape
+    xt, nx, n_ports = None, 0, 0
+    if xtalk is not None:
+        xt = _f64(xtalk)
+        assert xt.ndim == 2 and xt.shape[0] == xt.shape[1] and np.asarray(frame).ndim == 2
+        nx, n_ports = int(np.asarray(frame).shape[1]), int(xt.shape[0])
     d = _DetectorEx(_Detector(det.gain, det.dark_e, det.ron_e, det.bias, det.seed),
                     pr.ctypes.data if pr is not None else None, dk.ctypes.data if dk is not None else None,
-                    float(full_well), float(e_per_adu), float(adu_max))
+                    float(full_well), float(e_per_adu), float(adu_max), nx, n_ports,
+                    xt.ctypes.data if xt is not None else None)
     out = np.zeros_like(a)
-    lib().orc_detector_ex(a.ctypes.data, out.ctypes.data, a.shape[0], pixel_offset, C.addressof(d))
+    rc = lib().orc_detector_ex(a.ctypes.data, out.ctypes.data, a.shape[0], pixel_offset, C.addressof(d))
+    if rc != 0:
+        raise ValueError("oracle detector_ex: cross-talk needs whole rows and nx divisible by n_ports")
     return out.reshape(np.asarray(frame).shape)
+
+
+def detector_adu16(frame: np.ndarray, det, **kw) -> np.ndarray:
+    """ADC counts as uint16: detector_ex with e_per_adu > 0 and adu_max <= 65535, cast (the values are whole numbers)"""
+    assert kw.get("e_per_adu", 0.0) > 0.0 and kw.get("adu_max", 65535.0) <= 65535.0
+    return detector_ex(frame, det, **kw).astype(np.uint16)
+
+
+def olog_series(x: float) -> float:
+    return float(lib().orc_log_series(x))
+
+
+def osin2pi(y: float) -> float:
+    return float(lib().orc_sin2pi(y))
+
+
+def gaussian_pairs(seed: int, n: int, pixel0: int = 0):
+    z1, z2 = np.zeros(n), np.zeros(n)
+    a, b = C.c_double(), C.c_double()
+    L = lib()
+    for p in range(n):
+        L.orc_gaussian_pair(seed, pixel0 + p, C.byref(a), C.byref(b))
+        z1[p], z2[p] = a.value, b.value
+    return z1, z2
 
 
 def olog(x: float) -> float:

@@ -186,9 +186,14 @@ E2E_API int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf,
 
 /* ------------------------------------------------------------------------------------------------
  * Detector stage (a6; "photon noise and all other specific detector noises ... are added on the
- * final synthetic echellogram").  out[p] = (Poisson(max(0, gain*in[p] + dark_e)) + bias) + ron_e * N(0,1),
- * drawn from a Philox4x32-10 stream keyed by (seed, pixel index p = j*nx + i): the result does not depend
- * on launch geometry and is reproducible bit for bit (algorithm: DESIGN.md G12).
+ * final synthetic echellogram").  out[p] = (n + bias) + ron_e * z1 with mu = max(0, gain*in[p] + dark_e),
+ * n ~ Poisson(mu), z1 ~ N(0,1), drawn from a Philox4x32-10 stream keyed by (seed, pixel index p = j*nx + i): the
+ * result does not depend on launch geometry and is reproducible bit for bit.  Algorithm (G12, round 2):
+ * block 0 of the pixel's stream gives a Box-Muller pair (z1, z2); mu < 64: n by inversion (sequential search) with one
+ * uniform of block 1 -- an exact Poisson draw up to the 53-bit uniform, capped at n = 255 (probability < 1e-70);
+ * mu >= 64: n = max(0, floor(mu + sqrt(mu) z2 + (z2^2 - 1)/6 + 1/2)), the normal approximation with the first
+ * Cornish-Fisher term -- NOT an exact Poisson draw: mean mu, skewness 1/sqrt(mu) as Poisson, variance mu + 5/36
+ * (0.2 % high at mu = 64, 3e-6 at 4e4 e-), and the law changes at mu = 64.
  * ------------------------------------------------------------------------------------------------ */
 typedef struct e2e_detector {
     double gain, dark_e, ron_e, bias;
@@ -199,16 +204,24 @@ typedef struct e2e_detector {
 E2E_API int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny,
                        const e2e_detector_t* det, void* cuda_stream);
 
-/* Full detector stage ("... all other specific detector noises (e.g. dark current, RON ...)";
- * reading G19 of DESIGN.md).  Per pixel p:
+/* Full detector stage ("... all other specific detector noises (e.g. dark current, RON, pixels
+ * non-uniform response and cross-talk)"; readings G19 and G20 of DESIGN.md).  Per pixel p:
  *   mu = max(0, gain * prnu[p] * in[p] + dark[p]);  (z1, n) = the draws of the basic stage;
  *   e  = min(n, full_well_e) when full_well_e > 0 (the well saturates before read-out);
- *   e_per_adu <= 0:  out[p] = (e + bias) + ron_e * z1                                  (electrons)
- *   e_per_adu  > 0:  out[p] = clamp(floor(((e + ron_e * z1) / e_per_adu + bias) + 1/2), 0, adu_max)   (ADC counts)
+ *   v  = e + ron_e * z1                                                               (video signal)
+ *   no cross-talk:
+ *     e_per_adu <= 0:  out[p] = (e + bias) + ron_e * z1                               (electrons)
+ *     e_per_adu  > 0:  out[p] = clamp(floor((v / e_per_adu + bias) + 1/2), 0, adu_max)   (ADC counts)
+ *   cross-talk (xtalk != NULL and n_ports > 1; G20): the detector is read through n_ports ports, port a = columns
+ *   [a W, (a+1) W), W = nx / n_ports, all clocked together; a fraction X[a][b] of the video signal of port b appears in
+ *   port a at the same in-port column c:  s = v_a; for b = 0 .. n_ports-1, b != a: s = s + X[a][b] * v_b;
+ *     e_per_adu <= 0:  out = s + bias;      e_per_adu > 0:  out = clamp(floor((s / e_per_adu + bias) + 1/2), 0, adu_max)
  * d_prnu (pixel response non-uniformity) and d_dark (dark electrons per pixel) are DEVICE [ny*nx] maps owned by the
- * caller, or NULL (= 1 and base.dark_e).  With both NULL, full_well_e = 0 and e_per_adu = 0 the result equals
- * e2e_apply_detector bit for bit.  Errors: NULL frame / det, non-finite or negative full_well_e, e_per_adu, adu_max
- * -> E2E_ERR_INVALID_ARG.  Asynchronous on cuda_stream; in may equal out; the maps must not alias out. */
+ * caller, or NULL (= 1 and base.dark_e).  xtalk is a HOST [n_ports][n_ports] matrix (copied by the call; the diagonal is
+ * ignored), n_ports <= 16, nx divisible by n_ports.  With both maps NULL, full_well_e = 0, e_per_adu = 0 and no
+ * cross-talk the result equals e2e_apply_detector bit for bit.  Errors: NULL frame / det, non-finite or negative
+ * full_well_e, e_per_adu, adu_max, a non-finite coupling -> E2E_ERR_INVALID_ARG; n_ports > 16 or nx % n_ports != 0 ->
+ * E2E_ERR_UNSUPPORTED.  Asynchronous on cuda_stream; in may equal out; the maps must not alias out. */
 typedef struct e2e_detector_ex {
     e2e_detector_t base;
     const double* d_prnu;
@@ -216,9 +229,17 @@ typedef struct e2e_detector_ex {
     double full_well_e;
     double e_per_adu;
     double adu_max;
+    int32_t n_ports;                /* read-out ports for the cross-talk; 0 or 1 = none */
+    const double* xtalk;            /* HOST [n_ports][n_ports] coupling X[a][b], or NULL */
 } e2e_detector_ex_t;
 E2E_API int e2e_apply_detector_ex(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny,
                           const e2e_detector_ex_t* det, void* cuda_stream);
+
+/* The same stage with the ADC counts stored as uint16 (raw frames of ~40 000 ADU px^-1): needs
+ * e_per_adu > 0 and adu_max <= 65535 (else E2E_ERR_INVALID_ARG); d_frame_out: DEVICE uint16 [ny*nx], a quarter of the
+ * fp64 frame's bytes on the way to the host.  Element for element the value of e2e_apply_detector_ex, cast. */
+E2E_API int e2e_apply_detector_adu16(const double* d_frame_in, uint16_t* d_frame_out, int32_t nx, int32_t ny,
+                             const e2e_detector_ex_t* det, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Measurement helpers (used by bench.py; not part of the rendering path)

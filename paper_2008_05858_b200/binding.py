@@ -23,7 +23,7 @@ ERROR_NAMES = {-1: "E2E_ERR_INVALID_ARG", -2: "E2E_ERR_NOT_MONOTONIC", -3: "E2E_
 SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_destroy", "e2e_format_num_samples",
            "e2e_psf_create", "e2e_psf_destroy", "e2e_psf_info", "e2e_render_workspace_bytes", "e2e_setup_samples", "e2e_render_frame",
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_apply_detector_ex",
-           "e2e_measure_fp64_peak",
+           "e2e_apply_detector_adu16", "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
            "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames"]
 
@@ -68,7 +68,7 @@ class DetectorDesc(C.Structure):
 
 class DetectorExDesc(C.Structure):
     _fields_ = [("base", DetectorDesc), ("d_prnu", C.c_void_p), ("d_dark", C.c_void_p), ("full_well_e", C.c_double),
-                ("e_per_adu", C.c_double), ("adu_max", C.c_double)]
+                ("e_per_adu", C.c_double), ("adu_max", C.c_double), ("n_ports", C.c_int32), ("xtalk", C.c_void_p)]
 
 
 _lib = None
@@ -114,6 +114,8 @@ def load():
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
     L.e2e_apply_detector_ex.restype = C.c_int
     L.e2e_apply_detector_ex.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorExDesc), vp]
+    L.e2e_apply_detector_adu16.restype = C.c_int
+    L.e2e_apply_detector_adu16.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorExDesc), vp]
     L.e2e_measure_fp64_peak.restype = C.c_int
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_render_kernel_info.restype = C.c_int
@@ -328,15 +330,32 @@ def e2e_apply_detector(d_in, d_out, nx: int, ny: int, det, stream=None):
                                      _stream_ptr(stream)))
 
 
-def e2e_apply_detector_ex(d_in, d_out, nx: int, ny: int, det, d_prnu=None, d_dark=None, full_well_e: float = 0.0,
-                          e_per_adu: float = 0.0, adu_max: float = 65535.0, stream=None):
-    """full detector stage (e2e.h): d_prnu / d_dark are device tensors [ny*nx] or None"""
+def detector_ex_desc(det, d_prnu=None, d_dark=None, full_well_e: float = 0.0, e_per_adu: float = 0.0,
+                     adu_max: float = 65535.0, xtalk=None):
+    """``e2e_detector_ex_t`` (+ the host array the xtalk pointer refers to, which the caller must keep alive)"""
+    xt = _host(xtalk) if xtalk is not None else None
     d = DetectorExDesc(DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed)),
                        int(d_prnu.data_ptr()) if d_prnu is not None else None,
                        int(d_dark.data_ptr()) if d_dark is not None else None,
-                       float(full_well_e), float(e_per_adu), float(adu_max))
+                       float(full_well_e), float(e_per_adu), float(adu_max),
+                       int(xt.shape[0]) if xt is not None else 0, xt.ctypes.data if xt is not None else None)
+    return d, xt
+
+
+def e2e_apply_detector_ex(d_in, d_out, nx: int, ny: int, det, d_prnu=None, d_dark=None, full_well_e: float = 0.0,
+                          e_per_adu: float = 0.0, adu_max: float = 65535.0, xtalk=None, stream=None):
+    """full detector stage (e2e.h): d_prnu / d_dark are device tensors [ny*nx] or None, xtalk a host [n_ports][n_ports] array"""
+    d, keep = detector_ex_desc(det, d_prnu, d_dark, full_well_e, e_per_adu, adu_max, xtalk)
     _check(load().e2e_apply_detector_ex(int(d_in.data_ptr()), int(d_out.data_ptr()), int(nx), int(ny), C.byref(d),
                                         _stream_ptr(stream)))
+
+
+def e2e_apply_detector_adu16(d_in, d_out_u16, nx: int, ny: int, det, d_prnu=None, d_dark=None, full_well_e: float = 0.0,
+                             e_per_adu: float = 1.0, adu_max: float = 65535.0, xtalk=None, stream=None):
+    """the same stage with uint16 ADC counts (d_out_u16: uint16 device tensor [ny*nx])"""
+    d, keep = detector_ex_desc(det, d_prnu, d_dark, full_well_e, e_per_adu, adu_max, xtalk)
+    _check(load().e2e_apply_detector_adu16(int(d_in.data_ptr()), int(d_out_u16.data_ptr()), int(nx), int(ny), C.byref(d),
+                                           _stream_ptr(stream)))
 
 
 def e2e_measure_fp64_peak(repeats: int = 60):

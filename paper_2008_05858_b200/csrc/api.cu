@@ -30,7 +30,8 @@ int fail_cuda(cudaError_t e, const char* what)
 }
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream, long long p0 = 0);
-int launch_detector_ex(const double* d_in, double* d_out, long long n, const e2e_detector_ex_t& det, cudaStream_t stream);
+int launch_detector_ex(const double* d_in, void* d_out, bool out16, long long n, int nx, const e2e_detector_ex_t& det,
+                       cudaStream_t stream, long long p0 = 0);
 int measure_fp64_peak(int repeats, double* burst, double* sustained);
 
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
@@ -1195,23 +1196,53 @@ int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx
     return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
 }
 
+static int check_detector_ex(const e2e_detector_ex_t* det, int32_t nx, const void* d_out, bool out16, const char* who)
+{
+    const std::string w(who);
+    const e2e_detector_t& b = det->base;
+    if (!is_fin(b.gain) || !is_fin(b.dark_e) || !is_fin(b.ron_e) || !is_fin(b.bias))
+        return fail(E2E_ERR_INVALID_ARG, w + ": non-finite parameter");
+    if (!is_fin(det->full_well_e) || det->full_well_e < 0.0 || !is_fin(det->e_per_adu) || det->e_per_adu < 0.0)
+        return fail(E2E_ERR_INVALID_ARG, w + ": full_well_e / e_per_adu must be finite and >= 0");
+    if (det->e_per_adu > 0.0 && (!is_fin(det->adu_max) || det->adu_max < 0.0))
+        return fail(E2E_ERR_INVALID_ARG, w + ": adu_max must be finite and >= 0");
+    if (out16 && !(det->e_per_adu > 0.0 && det->adu_max <= 65535.0))
+        return fail(E2E_ERR_INVALID_ARG, w + ": the uint16 output needs e_per_adu > 0 and adu_max <= 65535");
+    if ((const void*)det->d_prnu == d_out || (const void*)det->d_dark == d_out)
+        return fail(E2E_ERR_INVALID_ARG, w + ": a map aliases the output frame");
+    if (det->n_ports < 0) return fail(E2E_ERR_INVALID_ARG, w + ": n_ports < 0");
+    if (det->xtalk && det->n_ports > 1) {
+        if (det->n_ports > 16) return fail(E2E_ERR_UNSUPPORTED, w + ": more than 16 read-out ports");
+        if (nx % det->n_ports != 0) return fail(E2E_ERR_UNSUPPORTED, w + ": nx is not divisible by n_ports");
+        for (int i = 0; i < det->n_ports * det->n_ports; ++i)
+            if (!is_fin(det->xtalk[i])) return fail(E2E_ERR_INVALID_ARG, w + ": non-finite cross-talk coupling");
+    }
+    return E2E_OK;
+}
+
 int e2e_apply_detector_ex(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_ex_t* det,
                           void* cuda_stream)
 {
     if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: NULL argument");
     if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: bad frame size");
-    const e2e_detector_t& b = det->base;
-    if (!is_fin(b.gain) || !is_fin(b.dark_e) || !is_fin(b.ron_e) || !is_fin(b.bias))
-        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: non-finite parameter");
-    if (!is_fin(det->full_well_e) || det->full_well_e < 0.0 || !is_fin(det->e_per_adu) || det->e_per_adu < 0.0)
-        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: full_well_e / e_per_adu must be finite and >= 0");
-    if (det->e_per_adu > 0.0 && (!is_fin(det->adu_max) || det->adu_max < 0.0))
-        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: adu_max must be finite and >= 0");
-    if (det->d_prnu == d_frame_out || det->d_dark == d_frame_out)
-        return fail(E2E_ERR_INVALID_ARG, "apply_detector_ex: a map aliases the output frame");
+    int rc = check_detector_ex(det, nx, d_frame_out, false, "apply_detector_ex");
+    if (rc) return rc;
     StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
     if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
-    return launch_detector_ex(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
+    return launch_detector_ex(d_frame_in, d_frame_out, false, (long long)nx * ny, nx, *det, (cudaStream_t)cuda_stream);
+}
+
+int e2e_apply_detector_adu16(const double* d_frame_in, uint16_t* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_ex_t* det,
+                             void* cuda_stream)
+{
+    if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector_adu16: NULL argument");
+    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector_adu16: bad frame size");
+    if ((const void*)d_frame_in == (const void*)d_frame_out) return fail(E2E_ERR_INVALID_ARG, "apply_detector_adu16: in aliases out");
+    int rc = check_detector_ex(det, nx, d_frame_out, true, "apply_detector_adu16");
+    if (rc) return rc;
+    StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
+    if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
+    return launch_detector_ex(d_frame_in, d_frame_out, true, (long long)nx * ny, nx, *det, (cudaStream_t)cuda_stream);
 }
 
 int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name, double* fma_cell, double* fma_sample)

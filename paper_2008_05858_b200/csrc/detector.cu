@@ -1,179 +1,329 @@
-// detector.cu -- step a6: Poisson photon noise + gaussian read noise on the rendered frame.
+// detector.cu -- step a6: the detector stage on the rendered frame.
 //
-// P:79 "photon noise and all other specific detector noises (e.g. dark current, RON ...) are added on the
-// final synthetic echellogram".  The paper names the noises only; the algorithm is reading G12 of DESIGN.md.
-// It is made of IEEE-exact operations only (+ - * / sqrt fma and integer ops; the log and exp are spelled
-// out below), and this file is compiled with --fmad=false, so the result is reproducible bit for bit and
-// independent of the launch geometry: pixel p owns the Philox4x32-10 stream (key = seed, counter = (p, block)).
+// P:79 "photon noise and all other specific detector noises (e.g. dark current, RON, pixels non-uniform response and
+// cross-talk) are added on the final synthetic echellogram".  The paper names the noises only; the algorithm is reading
+// G12 of DESIGN.md as re-specified in round 2 (a FIXED number of Philox blocks per pixel: one for the Box-Muller pair,
+// at most one more for the Poisson count; no rejection loop), G19 (PRNU / dark maps, full well, ADC) and G20 (cross-talk
+// between read-out ports).  Everything is made of IEEE-exact operations (+ - * / sqrt fma, integer ops; log, exp and
+// sin 2 pi y are spelled out below) and this file is compiled with --fmad=false, so the result is reproducible bit for bit
+// and independent of the launch geometry: pixel p owns the Philox4x32-10 stream (key = seed, counter = (p, block)).
 #include "common.cuh"
+
+#include <algorithm>
+#include <cstring>
 
 namespace e2e {
 
-// Philox4x32-10 stream of one pixel, consumed a whole counter block (4 words = 2 uniforms) at a time so that the
-// words stay in registers; the word order is the stream's: block 0 words 0..3, block 1 words 0..3, ...
-struct Philox {
-    uint32_t k0, k1;      // key
-    uint32_t c0, c1;      // pixel index (low, high)
-    uint32_t block;       // next counter block
-
-    __device__ __forceinline__ void init(uint64_t seed, uint64_t pixel)
-    {
-        k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32);
-        c0 = (uint32_t)pixel; c1 = (uint32_t)(pixel >> 32);
-        block = 0;
-    }
-    __device__ __forceinline__ void next_block(uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3)
-    {
-        uint32_t x0 = c0, x1 = c1, x2 = block, x3 = 0, ka = k0, kb = k1;
+// ------------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11): block `block` of pixel `pixel`
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t p_lo, uint32_t p_hi, uint32_t block,
+                                             uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3)
+{
+    uint32_t x0 = p_lo, x1 = p_hi, x2 = block, x3 = 0u;
 #pragma unroll
-        for (int r = 0; r < 10; ++r) {
-            uint32_t h0 = __umulhi(0xD2511F53u, x0), l0 = 0xD2511F53u * x0;
-            uint32_t h1 = __umulhi(0xCD9E8D57u, x2), l1 = 0xCD9E8D57u * x2;
-            uint32_t y0 = h1 ^ x1 ^ ka, y2 = h0 ^ x3 ^ kb;
-            x0 = y0; x1 = l1; x2 = y2; x3 = l0;
-            ka += 0x9E3779B9u; kb += 0xBB67AE85u;
-        }
-        w0 = x0; w1 = x1; w2 = x2; w3 = x3;
-        block += 1;
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t ka = k0 + (uint32_t)r * 0x9E3779B9u, kb = k1 + (uint32_t)r * 0xBB67AE85u;
+        const uint32_t h0 = __umulhi(0xD2511F53u, x0), l0 = 0xD2511F53u * x0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, x2), l1 = 0xCD9E8D57u * x2;
+        x0 = h1 ^ x1 ^ ka; x1 = l1; x2 = h0 ^ x3 ^ kb; x3 = l0;
     }
-    // u = ((hi >> 5) * 2^26 + (lo >> 6) + 1/2) * 2^-53  in (0, 1)
-    static __device__ __forceinline__ double uniform(uint32_t hi, uint32_t lo)
-    {
-        double a = (double)(hi >> 5), b = (double)(lo >> 6);
-        return (a * 67108864.0 + b + 0.5) * (1.0 / 9007199254740992.0);
-    }
-};
+    w0 = x0; w1 = x1; w2 = x2; w3 = x3;
+}
 
-// natural log of a normal x > 0: x = m 2^e, m in [sqrt(1/2), sqrt(2)); r = (m-1)/(m+1);
+// U(hi, lo) = ((hi >> 5) 2^26 + (lo >> 6) + 1/2) 2^-53  in (0, 1)
+__device__ __forceinline__ double uniform53(uint32_t hi, uint32_t lo)
+{
+    const double a = (double)(hi >> 5), b = (double)(lo >> 6);
+    return (a * 67108864.0 + b + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+// ------------------------------------------------------------------------------------------------
+// tables of the stage, rebuilt by every CTA in shared memory (4 KB; ~100 fp64 operations per thread, once)
+//   invc[i] = 1 / c_i, logc[i] = -series_log(invc[i]) for the 128 intervals of the mantissa range [0.7071, 1.4142)
+//   rcp[n]  = 1 / n (IEEE division), n = 1 .. 255, for the Poisson inversion's p <- (p mu) (1/n)
+// ------------------------------------------------------------------------------------------------
+struct DetTables {
+    double invc[128], logc[128], rcp[256];
+};
+constexpr unsigned long long kLogOff = 0x3fe6a09e00000000ULL;       // just below sqrt(1/2)
+
+// series log of a normal x > 0 (the generator of the table): x = m 2^e, m in [sqrt(1/2), sqrt(2)); r = (m-1)/(m+1);
 // log x = e ln2 + 2 r (1 + r^2/3 + ... + r^22/23), fma-Horner
-__device__ __forceinline__ double spec_log(double x)
+__device__ double series_log(double x)
 {
     unsigned long long b = (unsigned long long)__double_as_longlong(x);
     int e = (int)((b >> 52) & 0x7ff) - 1022;
     b = (b & 0x000fffffffffffffULL) | 0x3fe0000000000000ULL;
     double m = __longlong_as_double((long long)b);
     if (m < 0.70710678118654752440) { m = m * 2.0; e -= 1; }
-    double r = (m - 1.0) / (m + 1.0);
-    double r2 = r * r;
+    const double r = (m - 1.0) / (m + 1.0);
+    const double r2 = r * r;
     double P = 1.0 / 23.0;
 #pragma unroll
     for (int i = 10; i >= 0; --i) P = fma(P, r2, 1.0 / (double)(2 * i + 1));
     return fma((double)e, 0.693147180559945309417232, (2.0 * r) * P);
 }
 
+__device__ __forceinline__ void build_tables(DetTables& T)
+{
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) {
+        if (i < 128) {
+            const unsigned long long lo = kLogOff + ((unsigned long long)i << 45), hi = lo + (1ULL << 45);
+            const double c = 0.5 * __longlong_as_double((long long)lo) + 0.5 * __longlong_as_double((long long)hi);   // exact
+            const double ic = 1.0 / c;
+            T.invc[i] = ic;
+            T.logc[i] = -series_log(ic);
+        }
+        T.rcp[i] = i > 0 ? 1.0 / (double)i : 0.0;
+    }
+    __syncthreads();
+}
+
+// table log: t = bits(x) - OFF; k = t >> 52 (arithmetic); i = (t >> 45) & 127; z = bits^-1(bits(x) - (k << 52));
+// r = fma(z, invc[i], -1), log1p(r) = r + r^2 (-1/2 + r/3 - r^2/4 + r^3/5 - r^4/6 + r^5/7); log x = fma(k, ln2, logc[i] + log1p(r))
+__device__ __forceinline__ double table_log(const DetTables& T, double x)
+{
+    const unsigned long long ix = (unsigned long long)__double_as_longlong(x);
+    const unsigned long long t = ix - kLogOff;
+    const long long k = (long long)t >> 52;
+    const int i = (int)((t >> 45) & 127);
+    const double z = __longlong_as_double((long long)(ix - ((unsigned long long)k << 52)));
+    const double r = fma(z, T.invc[i], -1.0);
+    double P = 1.0 / 7.0;
+    P = fma(P, r, -1.0 / 6.0);
+    P = fma(P, r, 1.0 / 5.0);
+    P = fma(P, r, -1.0 / 4.0);
+    P = fma(P, r, 1.0 / 3.0);
+    P = fma(P, r, -0.5);
+    const double y = fma(r * r, P, r);
+    return fma((double)k, 0.693147180559945309417232, T.logc[i] + y);
+}
+
 // exp(y), |y| < 700: k = rint(y / ln2), r = y - k ln2 (two constants), Taylor to degree 13, times 2^k
 __device__ __forceinline__ double spec_exp(double y)
 {
-    double k = rint(y * 1.44269504088896340736);
+    const double k = rint(y * 1.44269504088896340736);
     double r = fma(-k, 6.93147180369123816490e-01, y);
     r = fma(-k, 1.90821492927058770002e-10, r);
     double c[14];
     c[0] = 1.0;
 #pragma unroll
-    for (int i = 1; i <= 13; ++i) c[i] = c[i - 1] / (double)i;
+    for (int i = 1; i <= 13; ++i) c[i] = c[i - 1] / (double)i;          // folded at compile time (IEEE division)
     double P = c[13];
 #pragma unroll
     for (int i = 12; i >= 0; --i) P = fma(P, r, c[i]);
-    unsigned long long b = (unsigned long long)((long long)k + 1023) << 52;
+    const unsigned long long b = (unsigned long long)((long long)k + 1023) << 52;
     return P * __longlong_as_double((long long)b);
 }
 
-// the draws of one pixel (G12): z1 for the read noise, cnt = Poisson(mu)
-__device__ __forceinline__ void detector_draws(uint64_t seed, long long p, double mu, double& z1_out, double& cnt_out)
+// sin(2 pi y), y in [0, 1.25]: y -= rint(y); fold to |y| <= 1/4; Taylor series to y^23, fma-Horner in y^2
+__device__ __forceinline__ double sin2pi(double y)
 {
-    Philox g;
-    g.init(seed, (uint64_t)p);
-    // Marsaglia polar pair: the rejection loop only draws (v1, v2, q); the log / sqrt run once after it, converged
-    double v1, v2, q;
+    y = y - rint(y);
+    if (y > 0.25) y = 0.5 - y;
+    if (y < -0.25) y = -0.5 - y;
+    const double g = y * y;
+    double P = -0.00008823533599243005134484484;
+    P = fma(P, g, 0.001130923748251796187770218);
+    P = fma(P, g, -0.01203158594212062723320257);
+    P = fma(P, g, 0.1042291622081398411727104);
+    P = fma(P, g, -0.7181223017785005122317403);
+    P = fma(P, g, 3.819952584848282127733792);
+    P = fma(P, g, -15.09464257682299039182662);
+    P = fma(P, g, 42.05869394489765314498681);
+    P = fma(P, g, -76.70585975306138584163064);
+    P = fma(P, g, 81.60524927607505420339768);
+    P = fma(P, g, -41.34170224039976023396842);
+    P = fma(P, g, 6.283185307179586476925287);
+    return y * P;
+}
+
+// the draws of one pixel (G12 round 2): z1 for the read noise, cnt = Poisson(mu)
+__device__ __forceinline__ void detector_draws(const DetTables& T, uint64_t seed, unsigned long long p, double mu, double& z1_out,
+                                               double& cnt_out)
+{
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), p_lo = (uint32_t)p, p_hi = (uint32_t)(p >> 32);
     uint32_t w0, w1, w2, w3;
-    do {
-        g.next_block(w0, w1, w2, w3);
-        v1 = 2.0 * Philox::uniform(w0, w1) - 1.0;
-        v2 = 2.0 * Philox::uniform(w2, w3) - 1.0;
-        q = fma(v1, v1, v2 * v2);
-    } while (!(q < 1.0 && q > 0.0));
-    const double fz = sqrt(-2.0 * spec_log(q) / q);
-    const double z1 = v1 * fz, z2 = v2 * fz;
+    philox_block(k0, k1, p_lo, p_hi, 0u, w0, w1, w2, w3);
+    const double u1 = uniform53(w0, w1), u2 = uniform53(w2, w3);
+    const double rho = sqrt(-2.0 * table_log(T, u1));
+    z1_out = rho * sin2pi(u2 + 0.25);                     // cos(2 pi u2)
     double cnt;
     if (!(mu > 0.0)) {
         cnt = 0.0;
-    } else if (mu < 64.0) {                        // Knuth multiplication method
-        bool second = false;                       // the uniforms after the gaussian pair start on a block boundary
-        auto next_u = [&]() {
-            second = !second;
-            if (second) { g.next_block(w0, w1, w2, w3); return Philox::uniform(w0, w1); }
-            return Philox::uniform(w2, w3);
-        };
-        double L = spec_exp(-mu), prod = next_u();
-        cnt = 0.0;
-        while (prod > L) { cnt += 1.0; prod = prod * next_u(); }
-    } else {                                       // normal + first Cornish-Fisher term
-        double a = sqrt(mu) * z2;
-        double b = (z2 * z2 - 1.0) / 6.0;
+    } else if (mu < 64.0) {                               // inversion by sequential search, one uniform of block 1
+        philox_block(k0, k1, p_lo, p_hi, 1u, w0, w1, w2, w3);
+        const double v = uniform53(w0, w1);
+        double pr = spec_exp(-mu), F = pr;
+        int n = 0;
+        while (v > F && n < 255) {
+            n += 1;
+            pr = (pr * mu) * T.rcp[n];
+            F = F + pr;
+        }
+        cnt = (double)n;
+    } else {                                              // normal + first Cornish-Fisher term
+        const double z2 = rho * sin2pi(u2);
+        const double a = sqrt(mu) * z2;
+        const double b = (z2 * z2 - 1.0) * (1.0 / 6.0);
         cnt = floor(((mu + a) + b) + 0.5);
         if (cnt < 0.0) cnt = 0.0;
     }
-    z1_out = z1; cnt_out = cnt;
+    cnt_out = cnt;
 }
+
+// parameters of one launch (by value)
+struct DetParams {
+    e2e_detector_t base;
+    const double* prnu;            // whole-frame maps (indexed by the pixel's index in the frame) or nullptr
+    const double* dark;
+    double full_well, e_per_adu, adu_max;
+    int n_ports, port_w;           // cross-talk: ports and columns per port (0 = none)
+    int nx;
+    double xtalk[16 * 16];         // X[a][b]
+};
+
+// video signal of one pixel before cross-talk / bias / ADC: e (electrons after the well) and z1
+__device__ __forceinline__ double pixel_signal(const DetTables& T, const DetParams& D, double f, unsigned long long gp, double& z1)
+{
+    double g = D.base.gain;
+    if (D.prnu) g = g * __ldg(D.prnu + gp);
+    double mu = g * f + (D.dark ? __ldg(D.dark + gp) : D.base.dark_e);
+    if (!(mu > 0.0)) mu = 0.0;
+    double e;
+    detector_draws(T, D.base.seed, gp, mu, z1, e);
+    if (D.full_well > 0.0 && e > D.full_well) e = D.full_well;
+    return e;
+}
+
+__device__ __forceinline__ double adc(const DetParams& D, double v)
+{
+    double a = floor((v / D.e_per_adu + D.base.bias) + 0.5);
+    if (a < 0.0) a = 0.0;
+    if (a > D.adu_max) a = D.adu_max;
+    return a;
+}
+
+template <typename OutT>
+__device__ __forceinline__ void store_out(OutT* out, long long p, double v);
+template <>
+__device__ __forceinline__ void store_out<double>(double* out, long long p, double v) { out[p] = v; }
+template <>
+__device__ __forceinline__ void store_out<uint16_t>(uint16_t* out, long long p, double v) { out[p] = (uint16_t)(unsigned)v; }   // whole number in [0, 65535]
 
 // in / out point at pixel p0 of the frame (the host path applies the stage band by band); the stream is keyed by the
-// pixel's index in the whole frame, so the result does not depend on how the frame is split into launches
-__global__ void __launch_bounds__(256, 6) detector_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, long long p0, e2e_detector_t det)
+// pixel's index in the whole frame, so the result does not depend on how the frame is split into launches.  in may
+// alias out (each pixel is read before it is written, by the same thread): no __restrict__ on the two.
+template <typename OutT>
+__global__ void __launch_bounds__(256) detector_kernel(const double* in, OutT* out, long long n, long long p0, DetParams D)
 {
-    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    double mu = det.gain * in[p] + det.dark_e;
-    if (!(mu > 0.0)) mu = 0.0;
-    double z1, cnt;
-    detector_draws(det.seed, p0 + p, mu, z1, cnt);
-    out[p] = (cnt + det.bias) + det.ron_e * z1;
+    __shared__ DetTables T;
+    build_tables(T);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const bool use_adc = D.e_per_adu > 0.0;
+    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        double z1;
+        const double e = pixel_signal(T, D, in[p], (unsigned long long)(p0 + p), z1);
+        double r;
+        if (!use_adc) r = (e + D.base.bias) + D.base.ron_e * z1;
+        else r = adc(D, e + D.base.ron_e * z1);
+        store_out<OutT>(out, p, r);
+    }
 }
 
-// full detector stage (e2e.h e2e_apply_detector_ex; G19): PRNU / dark maps, full well, ADC
-__global__ void detector_ex_kernel(const double* __restrict__ in, double* __restrict__ out, long long n, e2e_detector_ex_t det)
+// cross-talk (G20): thread <-> (row, in-port column c); it draws the video signal v_b = e + ron z1 of that column in every
+// port b, then writes s_a = v_a + sum_{b != a, ascending} X[a][b] v_b (+ bias, or through the ADC) for every port a.
+// Reads of one thread precede its writes and no other thread touches those pixels: in may alias out.
+template <typename OutT>
+__global__ void __launch_bounds__(128) detector_xtalk_kernel(const double* in, OutT* out, long long n_rows, long long p0, DetParams D)
 {
-    long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    double g = det.base.gain;
-    if (det.d_prnu) g = g * __ldg(det.d_prnu + p);
-    double mu = g * in[p] + (det.d_dark ? __ldg(det.d_dark + p) : det.base.dark_e);
-    if (!(mu > 0.0)) mu = 0.0;
-    double z1, e;
-    detector_draws(det.base.seed, p, mu, z1, e);
-    if (det.full_well_e > 0.0 && e > det.full_well_e) e = det.full_well_e;
-    if (!(det.e_per_adu > 0.0)) {
-        out[p] = (e + det.base.bias) + det.base.ron_e * z1;
-    } else {
-        const double v = e + det.base.ron_e * z1;
-        double a = floor((v / det.e_per_adu + det.base.bias) + 0.5);
-        if (a < 0.0) a = 0.0;
-        if (a > det.adu_max) a = det.adu_max;
-        out[p] = a;
+    __shared__ DetTables T;
+    __shared__ double V[16][128];
+    build_tables(T);
+    const int W = D.port_w, np = D.n_ports;
+    const long long per_row = (W + 127) / 128;                  // CTAs per row
+    const bool use_adc = D.e_per_adu > 0.0;
+    for (long long blk = blockIdx.x; blk < n_rows * per_row; blk += gridDim.x) {
+        const long long row = blk / per_row;
+        const int c = (int)(blk - row * per_row) * 128 + threadIdx.x;
+        if (c < W) {
+            for (int b = 0; b < np; ++b) {
+                const long long p = row * D.nx + (long long)b * W + c;
+                double z1;
+                const double e = pixel_signal(T, D, in[p], (unsigned long long)(p0 + p), z1);
+                V[b][threadIdx.x] = e + D.base.ron_e * z1;
+            }
+            for (int a = 0; a < np; ++a) {
+                double s = V[a][threadIdx.x];
+                for (int b = 0; b < np; ++b)
+                    if (b != a) s = s + D.xtalk[a * np + b] * V[b][threadIdx.x];
+                const double r = use_adc ? adc(D, s) : s + D.base.bias;
+                store_out<OutT>(out, row * D.nx + (long long)a * W + c, r);
+            }
+        }
     }
+}
+
+static int resident_ctas(int threads)
+{
+    static int sms[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148 * 8;
+    if (!sms[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        sms[dev] = n;
+    }
+    return sms[dev] * (2048 / threads);
+}
+
+template <typename OutT>
+static int launch_detector_any(const double* d_in, OutT* d_out, long long n, int nx, const DetParams& D, cudaStream_t stream, long long p0)
+{
+    if (n <= 0) return E2E_OK;
+    if (D.n_ports > 1) {
+        const long long rows = n / nx, per_row = (D.port_w + 127) / 128;
+        const long long blocks = std::min<long long>(rows * per_row, resident_ctas(128));
+        detector_xtalk_kernel<OutT><<<(unsigned)blocks, 128, 0, stream>>>(d_in, d_out, rows, p0, D);
+    } else {
+        const long long blocks = std::min<long long>((n + 255) / 256, resident_ctas(256));
+        detector_kernel<OutT><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+    }
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "detector kernel launch");
+    return E2E_OK;
+}
+
+static DetParams basic_params(const e2e_detector_t& det)
+{
+    DetParams D;
+    memset(&D, 0, sizeof(D));
+    D.base = det;
+    return D;
 }
 
 int launch_detector(const double* d_in, double* d_out, long long n, const e2e_detector_t& det, cudaStream_t stream, long long p0)
 {
-    if (n <= 0) return E2E_OK;
-    const int threads = 256;
-    long long blocks = (n + threads - 1) / threads;
-    detector_kernel<<<(unsigned)blocks, threads, 0, stream>>>(d_in, d_out, n, p0, det);
-    count_launch();
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail_cuda(e, "detector_kernel launch");
-    return E2E_OK;
+    return launch_detector_any<double>(d_in, d_out, n, 1, basic_params(det), stream, p0);
 }
 
-int launch_detector_ex(const double* d_in, double* d_out, long long n, const e2e_detector_ex_t& det, cudaStream_t stream)
+// full stage.  d_in / d_out point at pixel p0 (a whole number of rows from the frame start when cross-talk is on);
+// the maps are whole-frame pointers.  out16 selects the uint16 ADC output.
+int launch_detector_ex(const double* d_in, void* d_out, bool out16, long long n, int nx, const e2e_detector_ex_t& det,
+                       cudaStream_t stream, long long p0)
 {
-    if (n <= 0) return E2E_OK;
-    const int threads = 256;
-    long long blocks = (n + threads - 1) / threads;
-    detector_ex_kernel<<<(unsigned)blocks, threads, 0, stream>>>(d_in, d_out, n, det);
-    count_launch();
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail_cuda(e, "detector_ex_kernel launch");
-    return E2E_OK;
+    DetParams D = basic_params(det.base);
+    D.prnu = det.d_prnu; D.dark = det.d_dark;
+    D.full_well = det.full_well_e; D.e_per_adu = det.e_per_adu; D.adu_max = det.adu_max;
+    D.nx = nx;
+    if (det.xtalk && det.n_ports > 1) {
+        D.n_ports = det.n_ports; D.port_w = nx / det.n_ports;
+        for (int i = 0; i < det.n_ports * det.n_ports; ++i) D.xtalk[i] = det.xtalk[i];
+    }
+    if (out16) return launch_detector_any<uint16_t>(d_in, (uint16_t*)d_out, n, nx, D, stream, p0);
+    return launch_detector_any<double>(d_in, (double*)d_out, n, nx, D, stream, p0);
 }
 
 }  // namespace e2e

@@ -558,6 +558,58 @@ def test_detector_ex_bit_exact(B):
         B.e2e_apply_detector_ex(d_out, d_out, nx, ny, det, d_prnu=d_out)
 
 
+def test_detector_crosstalk_and_adu16_bit_exact(B):
+    """G20 cross-talk between read-out ports and the uint16 ADC output: every variant bit-exact vs the oracle,
+    in place too; shapes that do not fit are refused"""
+    import torch
+    rng = np.random.default_rng(8)
+    nx, ny = 16 * 37, 23                                      # 37 columns per port with 16 ports, 148 with 4
+    fr = rng.uniform(0.0, 200.0, (ny, nx))
+    fr[3, :40] = 0.0
+    fr[4, :40] = rng.uniform(0.0, 3.0, 40)
+    fr[:, 5] = 5.0e4                                          # a bright column: its ghost shows up in the other ports
+    prnu = rng.normal(1.0, 0.02, (ny, nx))
+    dark = rng.uniform(0.0, 3.0, (ny, nx))
+    det = W.Detector(gain=0.9, dark_e=0.2, ron_e=2.5, bias=300.0, seed=0x5EED_0000_0000_0007)
+    d_in, d_pr, d_dk = (torch.from_numpy(a).cuda() for a in (fr, prnu, dark))
+    d_out = torch.empty_like(d_in)
+    d_u16 = torch.empty((ny, nx), dtype=torch.uint16, device="cuda")
+    for n_ports in (2, 4, 16):
+        X = rng.uniform(-2e-4, 8e-4, (n_ports, n_ports))
+        for kw in (dict(), dict(e_per_adu=1.1, adu_max=65535.0), dict(full_well_e=4.0e4, e_per_adu=0.8, adu_max=40000.0)):
+            okw = {("full_well" if k == "full_well_e" else k): x for k, x in kw.items()}
+            B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det, d_prnu=d_pr, d_dark=d_dk, xtalk=X, **kw)
+            O = oracle.detector_ex(fr, det, prnu=prnu, dark=dark, xtalk=X, **okw)
+            assert np.array_equal(d_out.cpu().numpy(), O), (n_ports, kw)
+            if kw:
+                B.e2e_apply_detector_adu16(d_in, d_u16, nx, ny, det, d_prnu=d_pr, d_dark=d_dk, xtalk=X, **kw)
+                G16 = d_u16.cpu().numpy()
+                assert G16.dtype == np.uint16
+                assert np.array_equal(G16, oracle.detector_adu16(fr, det, prnu=prnu, dark=dark, xtalk=X, **okw))
+        # in place
+        tmp = d_in.clone()
+        B.e2e_apply_detector_ex(tmp, tmp, nx, ny, det, xtalk=X)
+        assert np.array_equal(tmp.cpu().numpy(), oracle.detector_ex(fr, det, xtalk=X))
+    # the ghost of the bright column is there: same in-port column of port 1, scaled by X[1][0]
+    X = np.zeros((4, 4)); X[1, 0] = 1e-3
+    B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det, xtalk=X)
+    plain = torch.empty_like(d_in)
+    B.e2e_apply_detector_ex(d_in, plain, nx, ny, det)
+    diff = (d_out - plain).cpu().numpy()
+    assert np.all(np.abs(diff[:, 148 + 5] - 1e-3 * 0.9 * 5.0e4) < 3.0) and np.all(diff[:, :148] == 0.0)
+    # uint16 without cross-talk, and without maps
+    B.e2e_apply_detector_adu16(d_in, d_u16, nx, ny, det, e_per_adu=1.3)
+    assert np.array_equal(d_u16.cpu().numpy(), oracle.detector_adu16(fr, det, e_per_adu=1.3))
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det, xtalk=np.zeros((5, 5)))         # 592 % 5 != 0
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_ex(d_in, d_out, nx, ny, det, xtalk=np.zeros((32, 32)))
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_adu16(d_in, d_u16, nx, ny, det, e_per_adu=0.0)
+    with pytest.raises(B.E2EError):
+        B.e2e_apply_detector_adu16(d_in, d_u16, nx, ny, det, e_per_adu=1.0, adu_max=1.0e5)
+
+
 def test_render_frames_batch_equals_single_renders(B):
     """batch render on fixed geometry.  The five Doppler-shifted frames of the RV sweep in one call are,
     frame by frame, the bits of five single renders, and every one of them matches the oracle's render of that velocity

@@ -17,16 +17,19 @@ namespace e2e {
 // ------------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11): block `block` of pixel `pixel`
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void philox_block(uint32_t k0, uint32_t k1, uint32_t p_lo, uint32_t p_hi, uint32_t block,
+// rk = the 10 round keys (k0 + r 0x9E3779B9, k1 + r 0xBB67AE85), computed once on the host (integer arithmetic: exact)
+struct PhiloxKeys { uint32_t a[10], b[10]; };
+
+__device__ __forceinline__ void philox_block(const PhiloxKeys& rk, uint32_t p_lo, uint32_t p_hi, uint32_t block,
                                              uint32_t& w0, uint32_t& w1, uint32_t& w2, uint32_t& w3)
 {
     uint32_t x0 = p_lo, x1 = p_hi, x2 = block, x3 = 0u;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint32_t ka = k0 + (uint32_t)r * 0x9E3779B9u, kb = k1 + (uint32_t)r * 0xBB67AE85u;
-        const uint32_t h0 = __umulhi(0xD2511F53u, x0), l0 = 0xD2511F53u * x0;
-        const uint32_t h1 = __umulhi(0xCD9E8D57u, x2), l1 = 0xCD9E8D57u * x2;
-        x0 = h1 ^ x1 ^ ka; x1 = l1; x2 = h0 ^ x3 ^ kb; x3 = l0;
+        const unsigned long long m0 = (unsigned long long)0xD2511F53u * x0;      // one IMAD.WIDE each: high and low word
+        const unsigned long long m1 = (unsigned long long)0xCD9E8D57u * x2;
+        x0 = (uint32_t)(m1 >> 32) ^ x1 ^ rk.a[r]; x1 = (uint32_t)m1;
+        x2 = (uint32_t)(m0 >> 32) ^ x3 ^ rk.b[r]; x3 = (uint32_t)m0;
     }
     w0 = x0; w1 = x1; w2 = x2; w3 = x3;
 }
@@ -43,6 +46,22 @@ __device__ __forceinline__ double uniform53(uint32_t hi, uint32_t lo)
 //   invc[i] = 1 / c_i, logc[i] = -series_log(invc[i]) for the 128 intervals of the mantissa range [0.7071, 1.4142)
 //   rcp[n]  = 1 / n (IEEE division), n = 1 .. 255, for the Poisson inversion's p <- (p mu) (1/n)
 // ------------------------------------------------------------------------------------------------
+// polynomial coefficients in the constant bank: fp64 instructions take them as c[][] operands (an immediate would cost two
+// moves per coefficient).  kLog1p: -1/2 .. 1/7;  kSin: Taylor series of sin(2 pi y) in y^2, y^1 .. y^23
+__constant__ double kLog1p[6] = {-0.5, 1.0 / 3.0, -1.0 / 4.0, 1.0 / 5.0, -1.0 / 6.0, 1.0 / 7.0};
+__constant__ double kSin[12] = {6.283185307179586476925287, -41.34170224039976023396842, 81.60524927607505420339768,
+                                -76.70585975306138584163064, 42.05869394489765314498681, -15.09464257682299039182662,
+                                3.819952584848282127733792, -0.7181223017785005122317403, 0.1042291622081398411727104,
+                                -0.01203158594212062723320257, 0.001130923748251796187770218, -0.00008823533599243005134484484};
+__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2.0, (1.0 / 2.0) / 3.0, ((1.0 / 2.0) / 3.0) / 4.0, (((1.0 / 2.0) / 3.0) / 4.0) / 5.0,
+                                 ((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0, (((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0,
+                                 ((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0,
+                                 (((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0) / 9.0,
+                                 ((((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0) / 9.0) / 10.0,
+                                 (((((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0) / 9.0) / 10.0) / 11.0,
+                                 ((((((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0) / 9.0) / 10.0) / 11.0) / 12.0,
+                                 (((((((((((1.0 / 2.0) / 3.0) / 4.0) / 5.0) / 6.0) / 7.0) / 8.0) / 9.0) / 10.0) / 11.0) / 12.0) / 13.0};   // c[i] = c[i-1] / i (IEEE)
+
 struct DetTables {
     double invc[128], logc[128], rcp[256];
 };
@@ -90,12 +109,9 @@ __device__ __forceinline__ double table_log(const DetTables& T, double x)
     const int i = (int)((t >> 45) & 127);
     const double z = __longlong_as_double((long long)(ix - ((unsigned long long)k << 52)));
     const double r = fma(z, T.invc[i], -1.0);
-    double P = 1.0 / 7.0;
-    P = fma(P, r, -1.0 / 6.0);
-    P = fma(P, r, 1.0 / 5.0);
-    P = fma(P, r, -1.0 / 4.0);
-    P = fma(P, r, 1.0 / 3.0);
-    P = fma(P, r, -0.5);
+    double P = kLog1p[5];
+#pragma unroll
+    for (int i = 4; i >= 0; --i) P = fma(P, r, kLog1p[i]);
     const double y = fma(r * r, P, r);
     return fma((double)k, 0.693147180559945309417232, T.logc[i] + y);
 }
@@ -106,13 +122,9 @@ __device__ __forceinline__ double spec_exp(double y)
     const double k = rint(y * 1.44269504088896340736);
     double r = fma(-k, 6.93147180369123816490e-01, y);
     r = fma(-k, 1.90821492927058770002e-10, r);
-    double c[14];
-    c[0] = 1.0;
+    double P = kExpC[13];
 #pragma unroll
-    for (int i = 1; i <= 13; ++i) c[i] = c[i - 1] / (double)i;          // folded at compile time (IEEE division)
-    double P = c[13];
-#pragma unroll
-    for (int i = 12; i >= 0; --i) P = fma(P, r, c[i]);
+    for (int i = 12; i >= 0; --i) P = fma(P, r, kExpC[i]);
     const unsigned long long b = (unsigned long long)((long long)k + 1023) << 52;
     return P * __longlong_as_double((long long)b);
 }
@@ -124,58 +136,66 @@ __device__ __forceinline__ double sin2pi(double y)
     if (y > 0.25) y = 0.5 - y;
     if (y < -0.25) y = -0.5 - y;
     const double g = y * y;
-    double P = -0.00008823533599243005134484484;
-    P = fma(P, g, 0.001130923748251796187770218);
-    P = fma(P, g, -0.01203158594212062723320257);
-    P = fma(P, g, 0.1042291622081398411727104);
-    P = fma(P, g, -0.7181223017785005122317403);
-    P = fma(P, g, 3.819952584848282127733792);
-    P = fma(P, g, -15.09464257682299039182662);
-    P = fma(P, g, 42.05869394489765314498681);
-    P = fma(P, g, -76.70585975306138584163064);
-    P = fma(P, g, 81.60524927607505420339768);
-    P = fma(P, g, -41.34170224039976023396842);
-    P = fma(P, g, 6.283185307179586476925287);
+    double P = kSin[11];
+#pragma unroll
+    for (int i = 10; i >= 0; --i) P = fma(P, g, kSin[i]);
     return y * P;
 }
 
-// the draws of one pixel (G12 round 2): z1 for the read noise, cnt = Poisson(mu)
-__device__ __forceinline__ void detector_draws(const DetTables& T, uint64_t seed, unsigned long long p, double mu, double& z1_out,
-                                               double& cnt_out)
+// the draws of NP pixels (G12 round 2): z1 for the read noise, cnt = Poisson(mu).  The straight-line part (Philox block 0,
+// Box-Muller) runs for the NP pixels side by side so that their dependent fp64 chains overlap; the Poisson part branches.
+template <int NP>
+__device__ __forceinline__ void detector_draws(const DetTables& T, const PhiloxKeys& rk, const unsigned long long (&p)[NP],
+                                               const double (&mu)[NP], double (&z1_out)[NP], double (&cnt_out)[NP])
 {
-    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32), p_lo = (uint32_t)p, p_hi = (uint32_t)(p >> 32);
-    uint32_t w0, w1, w2, w3;
-    philox_block(k0, k1, p_lo, p_hi, 0u, w0, w1, w2, w3);
-    const double u1 = uniform53(w0, w1), u2 = uniform53(w2, w3);
-    const double rho = sqrt(-2.0 * table_log(T, u1));
-    z1_out = rho * sin2pi(u2 + 0.25);                     // cos(2 pi u2)
-    double cnt;
-    if (!(mu > 0.0)) {
-        cnt = 0.0;
-    } else if (mu < 64.0) {                               // inversion by sequential search, one uniform of block 1
-        philox_block(k0, k1, p_lo, p_hi, 1u, w0, w1, w2, w3);
-        const double v = uniform53(w0, w1);
-        double pr = spec_exp(-mu), F = pr;
-        int n = 0;
-        while (v > F && n < 255) {
-            n += 1;
-            pr = (pr * mu) * T.rcp[n];
-            F = F + pr;
-        }
-        cnt = (double)n;
-    } else {                                              // normal + first Cornish-Fisher term
-        const double z2 = rho * sin2pi(u2);
-        const double a = sqrt(mu) * z2;
-        const double b = (z2 * z2 - 1.0) * (1.0 / 6.0);
-        cnt = floor(((mu + a) + b) + 0.5);
-        if (cnt < 0.0) cnt = 0.0;
+    double u2[NP], rho[NP];
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
+        uint32_t w0, w1, w2, w3;
+        philox_block(rk, (uint32_t)p[i], (uint32_t)(p[i] >> 32), 0u, w0, w1, w2, w3);
+        const double u1 = uniform53(w0, w1);
+        u2[i] = uniform53(w2, w3);
+        rho[i] = sqrt(-2.0 * table_log(T, u1));
     }
-    cnt_out = cnt;
+#pragma unroll
+    for (int i = 0; i < NP; ++i) z1_out[i] = rho[i] * sin2pi(u2[i] + 0.25);      // cos(2 pi u2)
+#pragma unroll
+    for (int i = 0; i < NP; ++i) {
+        double cnt;
+        if (!(mu[i] > 0.0)) {
+            cnt = 0.0;
+        } else if (mu[i] < 64.0) {                        // inversion by sequential search, one uniform of block 1
+            uint32_t w0, w1, w2, w3;
+            philox_block(rk, (uint32_t)p[i], (uint32_t)(p[i] >> 32), 1u, w0, w1, w2, w3);
+            const double v = uniform53(w0, w1);
+            int n = 0;
+            // Exact shortcut for the PSF wings (mu << 1, about half of an echellogram's illuminated pixels): the search
+            // returns n = 0 iff v <= F0 = spec_exp(-mu), and F0 >= (1 - mu)(1 - 6e-16) (e^-mu >= 1 - mu; spec_exp is within
+            // 5e-16 relative of e^y, pinned by the oracle's tests), so v < (1 - mu) - 1e-15 implies v <= F0: same n, no exp.
+            if (!(mu[i] < 0.5 && v < (1.0 - mu[i]) - 1.0e-15)) {
+                double pr = spec_exp(-mu[i]), F = pr;
+                while (v > F && n < 255) {
+                    n += 1;
+                    pr = (pr * mu[i]) * T.rcp[n];
+                    F = F + pr;
+                }
+            }
+            cnt = (double)n;
+        } else {                                          // normal + first Cornish-Fisher term
+            const double z2 = rho[i] * sin2pi(u2[i]);
+            const double a = sqrt(mu[i]) * z2;
+            const double b = (z2 * z2 - 1.0) * (1.0 / 6.0);
+            cnt = floor(((mu[i] + a) + b) + 0.5);
+            if (cnt < 0.0) cnt = 0.0;
+        }
+        cnt_out[i] = cnt;
+    }
 }
 
 // parameters of one launch (by value)
 struct DetParams {
     e2e_detector_t base;
+    PhiloxKeys rk;
     const double* prnu;            // whole-frame maps (indexed by the pixel's index in the frame) or nullptr
     const double* dark;
     double full_well, e_per_adu, adu_max;
@@ -183,19 +203,6 @@ struct DetParams {
     int nx;
     double xtalk[16 * 16];         // X[a][b]
 };
-
-// video signal of one pixel before cross-talk / bias / ADC: e (electrons after the well) and z1
-__device__ __forceinline__ double pixel_signal(const DetTables& T, const DetParams& D, double f, unsigned long long gp, double& z1)
-{
-    double g = D.base.gain;
-    if (D.prnu) g = g * __ldg(D.prnu + gp);
-    double mu = g * f + (D.dark ? __ldg(D.dark + gp) : D.base.dark_e);
-    if (!(mu > 0.0)) mu = 0.0;
-    double e;
-    detector_draws(T, D.base.seed, gp, mu, z1, e);
-    if (D.full_well > 0.0 && e > D.full_well) e = D.full_well;
-    return e;
-}
 
 __device__ __forceinline__ double adc(const DetParams& D, double v)
 {
@@ -215,20 +222,45 @@ __device__ __forceinline__ void store_out<uint16_t>(uint16_t* out, long long p, 
 // in / out point at pixel p0 of the frame (the host path applies the stage band by band); the stream is keyed by the
 // pixel's index in the whole frame, so the result does not depend on how the frame is split into launches.  in may
 // alias out (each pixel is read before it is written, by the same thread): no __restrict__ on the two.
-template <typename OutT>
+// GENERAL = false: the basic stage (no maps, no well, no ADC) without the tests for them; kDetPix pixels per thread and
+// iteration, 256 pixels apart (coalesced).
+constexpr int kDetPix = 2;
+template <typename OutT, bool GENERAL>
 __global__ void __launch_bounds__(256) detector_kernel(const double* in, OutT* out, long long n, long long p0, DetParams D)
 {
     __shared__ DetTables T;
     build_tables(T);
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    const bool use_adc = D.e_per_adu > 0.0;
-    for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
-        double z1;
-        const double e = pixel_signal(T, D, in[p], (unsigned long long)(p0 + p), z1);
-        double r;
-        if (!use_adc) r = (e + D.base.bias) + D.base.ron_e * z1;
-        else r = adc(D, e + D.base.ron_e * z1);
-        store_out<OutT>(out, p, r);
+    const long long stride = (long long)gridDim.x * (256 * kDetPix);
+    const bool use_adc = GENERAL && D.e_per_adu > 0.0;
+    for (long long base = (long long)blockIdx.x * (256 * kDetPix) + threadIdx.x; base < n; base += stride) {
+        unsigned long long gp[kDetPix];
+        double mu[kDetPix], z1[kDetPix], e[kDetPix];
+#pragma unroll
+        for (int i = 0; i < kDetPix; ++i) {
+            const long long p = base + 256 * i;
+            const bool ok = p < n;
+            gp[i] = (unsigned long long)(p0 + p);
+            double g = D.base.gain, dk = D.base.dark_e;
+            if (GENERAL) {
+                if (D.prnu && ok) g = g * __ldg(D.prnu + gp[i]);
+                if (D.dark && ok) dk = __ldg(D.dark + gp[i]);
+            }
+            double m = g * (ok ? in[p] : 0.0) + dk;
+            if (!(m > 0.0)) m = 0.0;
+            mu[i] = m;
+        }
+        detector_draws<kDetPix>(T, D.rk, gp, mu, z1, e);
+#pragma unroll
+        for (int i = 0; i < kDetPix; ++i) {
+            const long long p = base + 256 * i;
+            if (p < n) {
+                double r;
+                if (GENERAL && D.full_well > 0.0 && e[i] > D.full_well) e[i] = D.full_well;
+                if (!use_adc) r = (e[i] + D.base.bias) + D.base.ron_e * z1[i];
+                else r = adc(D, e[i] + D.base.ron_e * z1[i]);
+                store_out<OutT>(out, p, r);
+            }
+        }
     }
 }
 
@@ -250,9 +282,15 @@ __global__ void __launch_bounds__(128) detector_xtalk_kernel(const double* in, O
         if (c < W) {
             for (int b = 0; b < np; ++b) {
                 const long long p = row * D.nx + (long long)b * W + c;
-                double z1;
-                const double e = pixel_signal(T, D, in[p], (unsigned long long)(p0 + p), z1);
-                V[b][threadIdx.x] = e + D.base.ron_e * z1;
+                const unsigned long long gp[1] = {(unsigned long long)(p0 + p)};
+                double g = D.base.gain;
+                if (D.prnu) g = g * __ldg(D.prnu + gp[0]);
+                double mu[1] = {g * in[p] + (D.dark ? __ldg(D.dark + gp[0]) : D.base.dark_e)};
+                if (!(mu[0] > 0.0)) mu[0] = 0.0;
+                double z1[1], e[1];
+                detector_draws<1>(T, D.rk, gp, mu, z1, e);
+                if (D.full_well > 0.0 && e[0] > D.full_well) e[0] = D.full_well;
+                V[b][threadIdx.x] = e[0] + D.base.ron_e * z1[0];
             }
             for (int a = 0; a < np; ++a) {
                 double s = V[a][threadIdx.x];
@@ -287,8 +325,11 @@ static int launch_detector_any(const double* d_in, OutT* d_out, long long n, int
         const long long blocks = std::min<long long>(rows * per_row, resident_ctas(128));
         detector_xtalk_kernel<OutT><<<(unsigned)blocks, 128, 0, stream>>>(d_in, d_out, rows, p0, D);
     } else {
-        const long long blocks = std::min<long long>((n + 255) / 256, resident_ctas(256));
-        detector_kernel<OutT><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        const long long per = 256 * kDetPix;
+        const long long blocks = std::min<long long>((n + per - 1) / per, resident_ctas(256));
+        const bool general = D.prnu || D.dark || D.full_well > 0.0 || D.e_per_adu > 0.0;
+        if (general) detector_kernel<OutT, true><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        else detector_kernel<OutT, false><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
     }
     count_launch();
     cudaError_t e = cudaGetLastError();
@@ -301,6 +342,10 @@ static DetParams basic_params(const e2e_detector_t& det)
     DetParams D;
     memset(&D, 0, sizeof(D));
     D.base = det;
+    for (int r = 0; r < 10; ++r) {
+        D.rk.a[r] = (uint32_t)det.seed + (uint32_t)r * 0x9E3779B9u;
+        D.rk.b[r] = (uint32_t)(det.seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
     return D;
 }
 

@@ -596,7 +596,8 @@ def test_detector_crosstalk_and_adu16_bit_exact(B):
     plain = torch.empty_like(d_in)
     B.e2e_apply_detector_ex(d_in, plain, nx, ny, det)
     diff = (d_out - plain).cpu().numpy()
-    assert np.all(np.abs(diff[:, 148 + 5] - 1e-3 * 0.9 * 5.0e4) < 3.0) and np.all(diff[:, :148] == 0.0)
+    assert np.all(np.abs(diff[:, 148 + 5] - 1e-3 * 0.9 * 5.0e4) < 3.0)
+    assert np.abs(diff[:, :148]).max() < 1e-9            # port 0 receives nothing ((e + ron z1) + bias vs (e + bias) + ron z1: rounding only)
     # uint16 without cross-talk, and without maps
     B.e2e_apply_detector_adu16(d_in, d_u16, nx, ny, det, e_per_adu=1.3)
     assert np.array_equal(d_u16.cpu().numpy(), oracle.detector_adu16(fr, det, e_per_adu=1.3))

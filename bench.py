@@ -32,12 +32,45 @@ UNIT = "contributions/s"
 # "survey_formula" figure; the headline roofline counts the irreducible FMAs only)
 C_ERFC, C_PSI = 60.0, 90.0
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-# capture of this command (profiles/, file named beside each value); None = not captured for that kernel
-NCU_TRAFFIC_BYTES = {
-    # profiles/r1_v8_espresso.md, launch ids 1-8 (dram__bytes_read.sum + dram__bytes_write.sum, mean over the 8 launches of a step)
-    "render_moment_kernel<2>": 258.7e6,
-}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures: profiles/traffic.json
+# holds, per (workload, kernel), the bytes, the profile file they come from and the sha256 of the kernel's source file at
+# capture time.  A value is reported only while that hash still matches the source in the tree (else null + a note).
+KERNEL_SOURCES = {"render_moment_kernel": "render_moment.cuh", "render_tabcell_kernel": "render_tabcell.cuh",
+                  "render_poly_kernel": "render_poly.cuh", "render_analytic_kernel": "render_analytic.cuh",
+                  "render_tabulated_kernel": "render_tabulated.cuh", "detector_kernel": "detector.cu",
+                  "setup_samples_kernel": "setup.cuh"}
+
+
+def source_hash(kernel: str):
+    import hashlib
+    base = kernel.split("<")[0]
+    f = ROOT / "paper_2008_05858_b200" / "csrc" / KERNEL_SOURCES.get(base, "")
+    if not f.is_file():
+        return None
+    return hashlib.sha256(f.read_bytes()).hexdigest()
+
+
+def ncu_traffic(workload: str, kernel: str):
+    """(bytes per launch or None, note)"""
+    try:
+        table = json.loads((ROOT / "profiles" / "traffic.json").read_text())
+    except Exception:
+        return None, "profiles/traffic.json missing"
+    e = table.get(f"{workload}:{kernel}")
+    if not e:
+        return None, "no ncu capture committed for this (workload, kernel)"
+    if e.get("source_sha256") != source_hash(kernel):
+        return None, f"stale: {KERNEL_SOURCES.get(kernel.split('<')[0])} changed since {e.get('profile')}"
+    return float(e["bytes_per_launch"]), f"{e.get('profile')} ({e.get('launches_per_step')} launches per step)"
+
+
+def measured_peaks():
+    """driver-written MEASURED_PEAKS.json (HBM GB/s, bf16 TF/s); fallback = B200_PROFILING.md's figure, flagged"""
+    try:
+        d = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())
+        return float(d["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback): MEASURED_PEAKS.json absent"
 
 
 def make_scene(name: str):
@@ -233,31 +266,23 @@ def aggregate_value(world: int, units_per_rank: float, seconds_per_step: float) 
     return world * units_per_rank / seconds_per_step
 
 
-def run_ours(args, rank: int, world: int, local_rank: int):
-    import torch
-    from paper_2008_05858_b200 import build as _build
-    if rank == 0:
-        _build.build()
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
-        dist.barrier()
-    from paper_2008_05858_b200 import binding as B, workloads as W
-    B.load()                                             # raises if libe2e.so is missing: no CPU fallback
-    dev = torch.device(f"cuda:{local_rank}")
-    torch.cuda.set_device(dev)
-    scene, wname = make_scene(args.workload)
+def measure_device(B, W, torch, name: str, steps: int, warmup: int, rank: int, world: int, dev, batch_frames: int = 1,
+                   sampler=None):
+    """K timed steps of the whole hot path (a1-a6) on one workload with inputs resident in HBM.  Returns the raw numbers
+    (times in ms per step, counts per step) plus the live objects the e2e leg reuses."""
+    scene, wname = make_scene(name)
     det = scene.detector or W.Detector(gain=1.0, dark_e=0.0, ron_e=3.0, bias=0.0, seed=2008_05858 + rank)
     r = B.Renderer(scene, device=str(dev))
     info = r.psf.info()
     hbx, hby = support_half_widths(scene.psf)
     contrib, n_cells = count_contributions(B, r, hbx, hby)
     kinfo = B.e2e_render_kernel_info(r.fmt, r.psf)
+    alg = B.e2e_render_algorithmic_fma(r.fmt, r.psf)
     n_samples = r.n_samples
     frame = torch.empty((scene.ny, scene.nx), dtype=torch.float64, device=dev)
     noisy = torch.empty_like(frame)
     stream = torch.cuda.current_stream()
-    nbatch = max(1, args.batch_frames)
+    nbatch = max(1, batch_frames)
     host_dopplers = [1.0]
     if nbatch > 1:
         # --batch-frames N: N Doppler-shifted copies of the workload's spectra (the RV-sweep velocities, cycled) rendered by
@@ -271,15 +296,15 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             for x in sp:
                 x.doppler = x.doppler * dop
             batch_descs.append(B.spectra_array(sp, [t.data_ptr() for t in r.flux]))
-        batch_frames = [torch.empty_like(frame) for _ in range(nbatch)]
+        batch_frames_t = [torch.empty_like(frame) for _ in range(nbatch)]
         batch_ws = torch.empty(B.e2e_render_frames_workspace_bytes(r.fmt, r.psf, nbatch), dtype=torch.uint8, device=dev)
         contrib, n_cells, n_samples = contrib * nbatch, n_cells * nbatch, n_samples * nbatch
         wname += f", batch of {nbatch} Doppler-shifted frames per step (e2e_render_frames)"
 
     def step():
         if nbatch > 1:
-            B.e2e_render_frames(r.fmt, r.psf, batch_descs, batch_frames, False, batch_ws, stream)
-            for fr in batch_frames:
+            B.e2e_render_frames(r.fmt, r.psf, batch_descs, batch_frames_t, False, batch_ws, stream)
+            for fr in batch_frames_t:
                 B.e2e_apply_detector(fr, noisy, scene.nx, scene.ny, det, stream)
             return
         B.e2e_render_frame(r.fmt, r.psf, r.spectra, frame, False, r.workspace, stream)
@@ -291,14 +316,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         step()
     barrier()
     # ---- device-timed region: K steps, inputs resident in HBM
     B.e2e_profile_enable(True)
     B.e2e_profile_read(reset=True)
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
+    if sampler is not None:
         sampler.start()
         time.sleep(0.25)
     barrier()
@@ -307,7 +331,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     t_wall0 = time.time()
     torch.cuda.profiler.start()                          # ncu --profile-from-start off: launch list of the timed region only
     ev0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     ev1.record(stream)
     barrier()
@@ -317,10 +341,95 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     ms_total = ev0.elapsed_time(ev1)
     prof = B.e2e_profile_read(reset=True)
     B.e2e_profile_enable(False)
-    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    ms_total = max_over_ranks(ms_total, world, dev)
-    ms_step = ms_total / args.steps
-    value = aggregate_value(world, contrib, ms_step * 1e-3)
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler is not None else None
+    ms_step = max_over_ranks(ms_total, world, dev) / steps
+    ncalls = max(prof["n_calls"], 1)
+    return {"scene": scene, "wname": wname, "det": det, "r": r, "info": info, "hbx": hbx, "hby": hby, "contrib": contrib,
+            "n_cells": n_cells, "n_samples": n_samples, "kinfo": kinfo, "alg": alg, "ms_step": ms_step, "steps": steps,
+            "stage_ms": {k: prof[k] / ncalls for k in ("ms_zero", "ms_setup", "ms_render", "ms_detector")},
+            "render_launches": prof["n_render"] / ncalls, "launches": int(launches), "clocks": clocks, "nbatch": nbatch,
+            "host_dopplers": host_dopplers, "barrier": barrier, "stream": stream}
+
+
+def stage_rooflines(m, name: str, peak_tf: float, burst_tf: float):
+    """SURVEY 8(d) 'report the respective bound too': one entry per stage.  setup / zero-fill / detector against the HBM roof
+    (algorithmic bytes: what the stage must move once), render against the FP64 pipe (DESIGN.md 5.3 / 5.5 work counts)."""
+    scene, kinfo, alg = m["scene"], m["kinfo"], m["alg"]
+    hbm_gbs, hbm_src = measured_peaks()
+    npx = scene.nx * scene.ny * m["nbatch"]
+    n_samples, n_cells = m["n_samples"], m["n_cells"]
+    table_bytes = sum(int(np.asarray(sp.flux).shape[0]) * 8 for sp in {id(sp.flux): sp for sp in scene.spectra}.values())
+    out = {}
+
+    def hbm(stage, ms, nbytes, what, kernel):
+        if ms <= 0:
+            return
+        ach = nbytes / (ms * 1e-3) / 1e9
+        traffic, tnote = ncu_traffic(name, kernel) if kernel else (None, "cudaMemsetAsync (no kernel of the library)")
+        out[stage] = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs, "traffic": traffic,
+                      "traffic_note": tnote, "kernel": kernel, "ms_per_step": ms, "algorithmic_bytes": nbytes, "definition": what,
+                      "peak_source": hbm_src}
+
+    hbm("zero", m["stage_ms"]["ms_zero"], 8.0 * npx, "8 B per pixel written", None)
+    hbm("setup", m["stage_ms"]["ms_setup"], 24.0 * n_samples + table_bytes * m["nbatch"],
+        "24 B per sample written (x, y, w) + the spectrum tables read once", "setup_samples_kernel")
+    hbm("detector", m["stage_ms"]["ms_detector"], 16.0 * npx, "16 B per pixel (fp64 frame read + fp64 frame written)", "detector_kernel<double, false>")
+    ms_render = m["stage_ms"]["ms_render"]
+    if ms_render > 0:
+        sec = ms_render * 1e-3
+        alg_flops = 2.0 * (n_cells * alg["fma_per_cell"] + n_samples * alg["fma_per_sample"])
+        executed = 2.0 * (n_cells * kinfo["executed_fma_per_cell"] + n_samples * kinfo["executed_fma_per_sample"])
+        ncols, nrows = np.floor(2 * m["hbx"]), np.floor(2 * m["hby"])
+        fma_flops, survey_flops = algorithmic_flops_per_sample(scene.psf, m["info"]["n_nodes"], ncols, nrows)
+        definition = ("algorithmic = un-padded fp64 flops of the cell-moment method (DESIGN.md 5.3 'Roofline'): per cell "
+                      "2 T (8 (P+1) w + 8 w h), per sample 2 * 8 (P+1); x measured cell / sample counts of the workload")
+        if kinfo["name"].startswith("render_tabcell"):
+            definition = ("algorithmic = fp64 flops of the cell-deposit method (DESIGN.md 5.5): per cell 2 x nodes x 2 y-offset rows x "
+                          "(os+1) x-offsets x (npix+1)^2 window pixels, per sample 2 x 4 x nodes deposit products; x measured counts")
+        if alg_flops <= 0 and fma_flops is not None:         # kernels that do not work cell by cell: the direct method's accumulate
+            alg_flops = n_samples * fma_flops
+            definition = "algorithmic = bare rank-T accumulate of the per-sample method, 2 T w h flop per sample"
+        traffic, tnote = ncu_traffic(name, kinfo["name"])
+        ach = alg_flops / sec / 1e12
+        rl = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf, "traffic": traffic,
+              "traffic_note": tnote, "kernel": kinfo["name"], "kernel_ms_per_step": ms_render,
+              "kernel_launches_per_step": m["render_launches"],
+              "peak_source": "measured in this run: e2e_measure_fp64_peak, sustained FP64-pipe rate (max of DFMA and DMMA chains) x 2 "
+                             "(MEASURED_PEAKS.json has no fp64 entry)",
+              "peak_burst": burst_tf, "flops_per_sample": alg_flops / max(n_samples, 1), "definition": definition,
+              "footprint_cells": n_cells}
+        if executed > 0:
+            rl.update({"executed_tflops": executed / sec / 1e12, "executed_frac": executed / sec / 1e12 / peak_tf,
+                       "executed_definition": "fp64 FMAs the kernel issues (DMMA = 256, padded tiles) x 2, from e2e_render_kernel_info x cell / sample counts"})
+        if fma_flops is not None:
+            rl.update({"direct_method_flops_per_sample": fma_flops,
+                       "direct_method_tflops_equivalent": n_samples * fma_flops / sec / 1e12,
+                       "direct_method_definition": "bare rank-T accumulate of the per-sample method, 2*T*w*h flop per sample: what this kernel would "
+                                                   "have to sustain if it evaluated every (sample, pixel) product (it does not: context only)",
+                       "survey_flops_per_sample": survey_flops,
+                       "survey_formula_tflops_equivalent": n_samples * survey_flops / sec / 1e12})
+        out["render"] = rl
+    return out
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_2008_05858_b200 import build as _build
+    if rank == 0:
+        _build.build()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    from paper_2008_05858_b200 import binding as B, workloads as W
+    B.load()                                             # raises if libe2e.so is missing: no CPU fallback
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    m = measure_device(B, W, torch, args.workload, args.steps, args.warmup, rank, world, dev, args.batch_frames,
+                       sampler=ClockSampler(local_rank) if rank == 0 else None)
+    scene, r, det, stream, barrier = m["scene"], m["r"], m["det"], m["stream"], m["barrier"]
+    contrib, n_samples, nbatch = m["contrib"], m["n_samples"], m["nbatch"]
+    value = aggregate_value(world, contrib, m["ms_step"] * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D of the spectra, D2H of the frame, every step
     e2e = None
@@ -334,77 +443,82 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         nbytes = B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc)
         ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
         h_frame = torch.empty((scene.ny, scene.nx), dtype=torch.float64).pin_memory()
+        h_adu = torch.empty((scene.ny, scene.nx), dtype=torch.uint16).pin_memory()
         h2d = nbatch * sum(int(np.asarray(sp.flux).shape[0]) * 8 for sp in {id(sp.flux): sp for sp in scene.spectra}.values())
-        d2h = nbatch * scene.nx * scene.ny * 8
-        def host_step():
-            for dop in host_dopplers:                         # one host call per frame of the batch (1 frame by default)
+        # raw-frame variant: the same stage through the ADC (1 e-/ADU, bias 1000 ADU), delivered as uint16
+        adu_desc, _keep = B.detector_ex_desc(W.Detector(gain=det.gain, dark_e=det.dark_e, ron_e=det.ron_e, bias=1000.0, seed=det.seed),
+                                             e_per_adu=1.0, adu_max=65535.0)
+
+        def host_step(adu16: bool):
+            for dop in m["host_dopplers"]:                    # one host call per frame of the batch (1 frame by default)
                 for f in range(len(desc)):
                     desc[f].doppler = float(scene.spectra[f].doppler) * dop
-                B.e2e_render_frame_host(r.fmt, r.psf, desc, h_frame.data_ptr(), ws, det=det, stream=stream)   # synchronises
-        host_step()                                           # warm-up
-        barrier()
-        k_e2e = max(2, min(args.steps, 5))
-        t0 = time.perf_counter()
-        for _ in range(k_e2e):
-            host_step()
-        barrier()
-        dt = (time.perf_counter() - t0) / k_e2e
-        dt = max_over_ranks(dt, world, dev)
-        e2e = {"value": aggregate_value(world, contrib, dt), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "ms_per_step": dt * 1e3, "steps": k_e2e}
-        del ws, h_frame
+                if adu16:
+                    B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, h_adu.data_ptr(), ws, adu_desc, stream=stream, adu16=True)
+                else:
+                    B.e2e_render_frame_host(r.fmt, r.psf, desc, h_frame.data_ptr(), ws, det=det, stream=stream)   # synchronises
 
+        k_e2e = max(2, min(args.steps, 5))
+        res = {}
+        for adu16 in (False, True):
+            host_step(adu16)                                  # warm-up
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(k_e2e):
+                host_step(adu16)
+            barrier()
+            res[adu16] = max_over_ranks((time.perf_counter() - t0) / k_e2e, world, dev)
+        e2e = {"value": aggregate_value(world, contrib, res[False]), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": nbatch * scene.nx * scene.ny * 8, "ms_per_step": res[False] * 1e3, "steps": k_e2e,
+               "call": "e2e_render_frame_host (fp64 electrons out)",
+               "adu16": {"value": aggregate_value(world, contrib, res[True]), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                         "d2h_bytes_per_step": nbatch * scene.nx * scene.ny * 2, "ms_per_step": res[True] * 1e3, "steps": k_e2e,
+                         "call": "e2e_render_frame_host_adu16 (uint16 ADC counts out: the raw frame, P:89 / P:119)"}}
+        del ws, h_frame, h_adu
+
+    # ---- the other BASELINE.json configs, device-resident only (parity-test sizes and the other full-size frames)
+    others = {}
+    if args.others and rank == 0 and world == 1 and nbatch == 1:
+        r.close()
+        del m["r"]
+        torch.cuda.empty_cache()
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel (render): plain FP64 ALU bound
+    # ---- roofline of every stage; the dominant kernel (render) against the FP64 pipe
     burst, sustained = B.e2e_measure_fp64_peak(80)
-    peak_tf = 2.0 * sustained / 1e12
-    ncols, nrows = info["footprint_cols"], info["footprint_rows"]
-    nominal = float(np.floor(2 * hbx) * np.floor(2 * hby))
-    fma_flops, survey_flops = algorithmic_flops_per_sample(scene.psf, info["n_nodes"], np.floor(2 * hbx), np.floor(2 * hby))
-    ms_render = prof["ms_render"] / max(prof["n_calls"], 1)
-    roofline = None
-    if fma_flops is not None and ms_render > 0:
-        alg = B.e2e_render_algorithmic_fma(r.fmt, r.psf)
-        alg_flops = 2.0 * (n_cells * alg["fma_per_cell"] + n_samples * alg["fma_per_sample"])
-        executed = 2.0 * (n_cells * kinfo["executed_fma_per_cell"] + n_samples * kinfo["executed_fma_per_sample"])
-        sec = ms_render * 1e-3
-        if alg_flops <= 0:                                   # kernels that do not work cell by cell: the direct method's accumulate
-            alg_flops = n_samples * fma_flops
-        ach = alg_flops / sec / 1e12
-        roofline = {"bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                    "traffic": NCU_TRAFFIC_BYTES.get(kinfo["name"]),
-                    "kernel": kinfo["name"], "kernel_ms_per_step": ms_render,
-                    "kernel_launches_per_step": prof["n_render"] / max(prof["n_calls"], 1),
-                    "peak_source": "measured in this run: e2e_measure_fp64_peak, sustained FP64-pipe rate (max of DFMA and DMMA chains) x 2 "
-                                   "(MEASURED_PEAKS.json has no fp64 entry)",
-                    "peak_burst": 2.0 * burst / 1e12,
-                    "flops_per_sample": alg_flops / n_samples,
-                    "definition": "algorithmic = un-padded fp64 flops of the cell-moment method (DESIGN.md 5.3 'Roofline'): per cell "
-                                  "2 T (8 (P+1) w + 8 w h), per sample 2 * 8 (P+1); x measured cell / sample counts of the workload",
-                    "footprint_cells": n_cells,
-                    "executed_tflops": executed / sec / 1e12, "executed_frac": executed / sec / 1e12 / peak_tf,
-                    "executed_definition": "fp64 FMAs the kernel issues (DMMA = 256, padded tiles) x 2, from e2e_render_kernel_info x cell / sample counts",
-                    "direct_method_flops_per_sample": fma_flops,
-                    "direct_method_tflops_equivalent": n_samples * fma_flops / sec / 1e12,
-                    "direct_method_definition": "bare rank-T accumulate of the per-sample method, 2*T*w*h flop per sample: what this kernel would "
-                                                "have to sustain if it evaluated every (sample, pixel) product (it does not: context only)",
-                    "survey_flops_per_sample": survey_flops,
-                    "survey_formula_tflops_equivalent": n_samples * survey_flops / sec / 1e12}
+    peak_tf, burst_tf = 2.0 * sustained / 1e12, 2.0 * burst / 1e12
+    stages = stage_rooflines(m, args.workload, peak_tf, burst_tf)
+    if args.others and world == 1 and nbatch == 1:
+        for name in ("tiny", "espresso_like", "hires_like", "field_psf", "rv_sweep"):
+            if name == args.workload:
+                continue
+            o = measure_device(B, W, torch, name, max(3, min(args.steps, 5)), 3, 0, 1, dev)
+            st = stage_rooflines(o, name, peak_tf, burst_tf)
+            others[name] = {"workload": o["wname"], "n_samples": o["n_samples"], "contributions": o["contrib"],
+                            "frame_ms": o["ms_step"], "value": o["contrib"] / (o["ms_step"] * 1e-3), "unit": UNIT,
+                            "stage_ms_per_step": o["stage_ms"], "gpu_launches_per_step": o["launches"] / o["steps"],
+                            "render_kernel": o["kinfo"]["name"],
+                            "stage_roofline_frac": {k: (v["frac"], v["bound"]) for k, v in st.items()},
+                            "render_executed_frac": st.get("render", {}).get("executed_frac")}
+            o["r"].close()
+            del o
+            torch.cuda.empty_cache()
     cpu = None
     if not args.no_cpu:
         c = time_oracle(scene, args.oracle_samples)
         cpu = {k: c[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    info = m["info"]
+    nominal = float(np.floor(2 * m["hbx"]) * np.floor(2 * m["hby"]))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "ms_per_step": m["ms_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": wname, "n_samples": n_samples, "contributions": contrib, "footprint_nominal_px": nominal,
+            "config": {"workload": m["wname"], "n_samples": n_samples, "contributions": contrib, "footprint_nominal_px": nominal,
                        "chord_nodes_Q": info["n_nodes"], "frame": [scene.ny, scene.nx], "stages": "a1-a6 (zero-fill, setup, render, detector)",
                        "l2": "inputs larger than L2: sample arrays %.0f MB + frame %.0f MB vs 126 MB L2" % (n_samples * 24 / 1e6, scene.nx * scene.ny * 8 / 1e6),
-                       "multi_gpu": "replicas only"},
-            "frame_ms": ms_step, "samples_per_s": world * n_samples / (ms_step * 1e-3),
-            "stage_ms_per_step": {k: prof[k] / max(prof["n_calls"], 1) for k in ("ms_zero", "ms_setup", "ms_render", "ms_detector")},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+                       "multi_gpu": "replicas only", "others": others or None},
+            "frame_ms": m["ms_step"], "samples_per_s": world * n_samples / (m["ms_step"] * 1e-3),
+            "stage_ms_per_step": m["stage_ms"], "stage_roofline": {k: v for k, v in stages.items() if k != "render"},
+            "clocks": m["clocks"], "e2e": e2e, "gpu_launches": m["launches"], "roofline": stages.get("render"), "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
 
 
@@ -418,6 +532,8 @@ def main():
     ap.add_argument("--oracle-samples", type=int, default=1_500_000, help="size of the CPU oracle's bounded sample")
     ap.add_argument("--batch-frames", type=int, default=1, help="render N Doppler-shifted frames per step with e2e_render_frames")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-others", dest="others", action="store_false",
+                    help="skip the device-resident numbers of the other BASELINE.json configs (config.others)")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

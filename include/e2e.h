@@ -134,7 +134,8 @@ typedef struct {
 } e2e_spectrum_t;
 
 /* bytes of device scratch e2e_render_frame needs for this (format, psf): the per-sample arrays x, y, w of
- * step a1-a3 (24 B per sample) plus the schedule.  256-byte aligned workspace required. */
+ * step a1-a3 (24 B per sample) plus the control block of the persistent render launch (4 B per work item).
+ * 256-byte aligned workspace required. */
 E2E_API int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, size_t* bytes);
 
 /* a1-a3 only, for one (fiber, order): writes lam, x, y, w of its samples to DEVICE arrays of length
@@ -171,7 +172,7 @@ E2E_API int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int
  * [ny*nx] array (pinned memory gives full PCIe speed).  The call copies the tables to the device, renders,
  * applies the detector stage a6 when det != NULL, copies the frame back and synchronises the stream before
  * returning.  Device scratch is taken from d_workspace, which must hold e2e_render_host_workspace_bytes() bytes.
- * The (fiber, order) strips are rendered in up to 8 row bands (E2E_HOST_BANDS overrides, 1..16) that share no pixel
+ * The (fiber, order) strips are rendered in up to 8 row bands that share no pixel
  * (a band starts only where a strip's first row lies above every row of the strips before it): even bands run on
  * cuda_stream, odd bands on a second stream owned by the library, and as soon as a band is done a6 runs on its rows
  * and they travel to the host on the library's copy stream.  The frame is bit-reproducible call to call; against
@@ -183,6 +184,18 @@ struct e2e_detector;
 E2E_API int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                           const struct e2e_detector* det /* may be NULL */, double* h_frame, void* d_workspace,
                           size_t workspace_bytes, void* cuda_stream);
+
+/* The same with the full detector stage (e2e_detector_ex_t below; det must not be NULL), fp64 electrons or ADC counts out. */
+struct e2e_detector_ex;
+E2E_API int e2e_render_frame_host_ex(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                             const struct e2e_detector_ex* det, double* h_frame, void* d_workspace, size_t workspace_bytes,
+                             void* cuda_stream);
+/* The same with the ADC counts delivered as uint16 (the raw frame an instrument writes, ~40 000 ADU px^-1):
+ * h_frame: HOST uint16 [ny*nx]; needs det->e_per_adu > 0 and det->adu_max <= 65535.  The device-to-host copy, which bounds
+ * the fp64 host path, shrinks 4x.  Element for element the value of e2e_render_frame_host_ex, cast. */
+E2E_API int e2e_render_frame_host_adu16(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                                const struct e2e_detector_ex* det, uint16_t* h_frame, void* d_workspace,
+                                size_t workspace_bytes, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Detector stage (a6; "photon noise and all other specific detector noises ... are added on the
@@ -263,6 +276,26 @@ E2E_API int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf
  * 0 for the kernels that do not work cell by cell.  Output pointers may be NULL. */
 E2E_API int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, double* fma_per_cell,
                                        double* fma_per_sample);
+
+/* Test hook: verifies on the device, pixel by pixel, the invariants of the render schedule that make the frame
+ * bit-reproducible although it is accumulated with L2 reductions: every footprint box (G9) of every work
+ * item is stamped into an int32 owner frame and
+ *   phase_conflicts        pixels claimed by two items of one phase launch (render_poly / _analytic / _tabcell / _tabulated);
+ *   queue_conflicts        persistent launch (render_moment): pixels whose previous writer is not a direct dependency of the
+ *                          item that writes next, run under the render kernel's own queue discipline (whole queue + the
+ *                          host path's band queues); zero in one run proves every pixel's writers form a chain;
+ *   device_band_conflicts  pixels shared between the two row bands the phase-launched kernels render concurrently;
+ *   host_band_conflicts    pixels shared between the host path's row bands;
+ *   host_rows_not_final    pixels a host band writes above the rows already declared final (copied to the host)
+ * must all be 0.  claimed_px = pixels inside at least one footprint box (> 0).  Synchronous on the device; allocates and
+ * frees 4 bytes per pixel. */
+typedef struct {
+    int64_t n_items, n_phases, n_dependencies;
+    int64_t claimed_px;
+    int64_t phase_conflicts, queue_conflicts, device_band_conflicts, host_band_conflicts, host_rows_not_final;
+    int32_t n_host_bands, n_device_bands;
+} e2e_plan_check_t;
+E2E_API int e2e_plan_check(const e2e_format_t* fmt, const e2e_psf_t* psf, e2e_plan_check_t* out);
 
 /* Number of kernel launches the library has issued since load (all entry points), for bench.py's gpu_launches. */
 E2E_API int64_t e2e_launch_count(void);

@@ -25,7 +25,8 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_render_host_workspace_bytes", "e2e_render_frame_host", "e2e_apply_detector", "e2e_apply_detector_ex",
            "e2e_apply_detector_adu16", "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
-           "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames"]
+           "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames",
+           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check"]
 
 
 class E2EError(RuntimeError):
@@ -71,6 +72,13 @@ class DetectorExDesc(C.Structure):
                 ("e_per_adu", C.c_double), ("adu_max", C.c_double), ("n_ports", C.c_int32), ("xtalk", C.c_void_p)]
 
 
+class PlanCheckDesc(C.Structure):
+    _fields_ = [("n_items", C.c_int64), ("n_phases", C.c_int64), ("n_dependencies", C.c_int64), ("claimed_px", C.c_int64),
+                ("phase_conflicts", C.c_int64), ("queue_conflicts", C.c_int64), ("device_band_conflicts", C.c_int64),
+                ("host_band_conflicts", C.c_int64), ("host_rows_not_final", C.c_int64), ("n_host_bands", C.c_int32),
+                ("n_device_bands", C.c_int32)]
+
+
 _lib = None
 
 
@@ -110,6 +118,12 @@ def load():
     L.e2e_render_host_workspace_bytes.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(C.c_size_t)]
     L.e2e_render_frame_host.restype = C.c_int
     L.e2e_render_frame_host.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorDesc), vp, vp, C.c_size_t, vp]
+    L.e2e_render_frame_host_ex.restype = C.c_int
+    L.e2e_render_frame_host_ex.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorExDesc), vp, vp, C.c_size_t, vp]
+    L.e2e_render_frame_host_adu16.restype = C.c_int
+    L.e2e_render_frame_host_adu16.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorExDesc), vp, vp, C.c_size_t, vp]
+    L.e2e_plan_check.restype = C.c_int
+    L.e2e_plan_check.argtypes = [vp, vp, C.POINTER(PlanCheckDesc)]
     L.e2e_apply_detector.restype = C.c_int
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
     L.e2e_apply_detector_ex.restype = C.c_int
@@ -322,6 +336,21 @@ def e2e_render_frame_host(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: int,
         d = C.byref(DetectorDesc(float(det.gain), float(det.dark_e), float(det.ron_e), float(det.bias), int(det.seed)))
     _check(load().e2e_render_frame_host(fmt.handle, psf.handle, spectra_desc, d, int(h_frame_ptr), int(d_workspace.data_ptr()),
                                         int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
+
+
+def e2e_render_frame_host_ex(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: int, d_workspace, det_ex_desc, stream=None,
+                             adu16: bool = False):
+    """host path with the full detector stage; det_ex_desc from detector_ex_desc(); adu16: h_frame_ptr is a uint16 array"""
+    fn = load().e2e_render_frame_host_adu16 if adu16 else load().e2e_render_frame_host_ex
+    _check(fn(fmt.handle, psf.handle, spectra_desc, C.byref(det_ex_desc), int(h_frame_ptr), int(d_workspace.data_ptr()),
+              int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
+
+
+def e2e_plan_check(fmt: Format, psf: Psf) -> dict:
+    """device-side check of the schedule invariants (test hook): every *_conflicts / host_rows_not_final must be 0"""
+    d = PlanCheckDesc()
+    _check(load().e2e_plan_check(fmt.handle, psf.handle, C.byref(d)))
+    return {k: int(getattr(d, k)) for k, _ in PlanCheckDesc._fields_}
 
 
 def e2e_apply_detector(d_in, d_out, nx: int, ny: int, det, stream=None):

@@ -6,6 +6,7 @@
 #include "render_tabcell.cuh"
 #include "render_poly.cuh"
 #include "render_moment.cuh"
+#include "plan_check.cuh"
 #include "poly_tables.h"
 
 #include <algorithm>
@@ -131,9 +132,15 @@ e2e_plan::~e2e_plan()
 {
     if (d_strips) cudaFree(d_strips);
     if (d_items) cudaFree(d_items);
+    if (d_dep_off) cudaFree(d_dep_off);
+    if (d_dep_idx) cudaFree(d_dep_idx);
+    if (d_succ_off) cudaFree(d_succ_off);
+    if (d_succ_idx) cudaFree(d_succ_idx);
+    if (d_ctrl_init) cudaFree(d_ctrl_init);
     for (BandPart* bp : {&host, &halves}) {
         if (bp->d_items) cudaFree(bp->d_items);
         if (bp->d_strips) cudaFree(bp->d_strips);
+        if (bp->d_queue) cudaFree(bp->d_queue);
     }
 }
 
@@ -402,9 +409,8 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
             A.n_terms = nt;
         }
         // production path: pixel-phase polynomial tables (the direct special-function kernel stays as the fallback
-        // for PSFs whose tables do not converge, and under E2E_FORCE_DIRECT=1 for A/B checks)
-        const char* force = getenv("E2E_FORCE_DIRECT");
-        if (!(force && force[0] == '1')) {
+        // for PSFs whose tables do not converge: sigma below ~0.3 px)
+        {
             PsfShape shape;
             shape.sx = d->sigma_x; shape.sy = d->sigma_y; shape.by_gauss = A.by_gauss != 0;
             for (int i = 0; i < A.n_terms; ++i) {
@@ -649,8 +655,7 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         const long long nchunks = (N + 31) / 32;
         items_k2 += (nchunks + run_length(s % no, nchunks) - 1) / run_length(s % no, nchunks);
     }
-    int K = items_k2 < kSmallFrameItems ? 4 : 2;
-    if (const char* e = getenv("E2E_RUN_CLASSES")) K = std::max(2, std::min(atoi(e), 16));
+    const int K = items_k2 < kSmallFrameItems ? 4 : 2;
     std::vector<std::vector<Item>> phases((size_t)n_colors * K);
     for (int s = 0; s < n_strips; ++s) {
         const int o = s % no;
@@ -673,6 +678,82 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
     }
     pl->n_phases = (int)pl->phase_off.size() - 1;
     pl->n_items = (int)flat.size();
+    // ---- dependency lists for the persistent launch (render_moment.cuh).  The queue order is the order of `flat`
+    //      (phase-major); item i depends on every item j < i that may share a pixel with it: same strip or a strip whose
+    //      rows may overlap (adj, from the per-bin row coverage above), and overlapping column ranges.  Column range of an
+    //      item = footprint boxes of its first and last sample (x is monotone along a strip).
+    {
+        const FormatView& v = F->view;
+        auto host_x = [&](int o, long long k) {
+            const double lam = fma((double)k + 0.5, F->dl[o], F->lam_min[o]);
+            const double L = (lam - v.lam0) * v.inv_dlam, M = ((double)F->order_m[o] - v.m0) * v.inv_dm;
+            return poly2(v.coef_x, v.deg_l, v.deg_m, L, M);
+        };
+        const int ni = (int)flat.size();
+        std::vector<int> clo(ni), chi(ni);
+        struct Run { int clo, chi, idx; };
+        std::vector<std::vector<Run>> runs(n_strips);
+        for (int i = 0; i < ni; ++i) {
+            const Item& it = flat[i];
+            const int f = it.strip / no, o = it.strip % no;
+            const long long k0 = (long long)it.chunk0 * 32;
+            const long long k1 = std::min<long long>(F->nsamp[o], ((long long)it.chunk0 + it.nchunks) * 32) - 1;
+            const double xa = host_x(o, k0) + F->fiber_dx[f], xb = host_x(o, k1) + F->fiber_dx[f];
+            // exactly the first column of the leftmost box and the last column of the rightmost one (G9: ceil(x - hbx),
+            // floor(x + hbx); host_x runs the device's operation sequence, so these are the device's integers).  No padding:
+            // a padded range would link runs of one class to each other and serialise the strip (e2e_plan_check verifies
+            // on the device that no edge is missing)
+            const double lo = std::max(std::min(xa, xb) - P->hbx, -1.0e9), hi = std::min(std::max(xa, xb) + P->hbx, 1.0e9);
+            clo[i] = (int)std::ceil(lo); chi[i] = (int)std::floor(hi);
+            runs[it.strip].push_back(Run{clo[i], chi[i], i});
+        }
+        for (auto& r : runs) std::sort(r.begin(), r.end(), [](const Run& a, const Run& b) { return a.clo < b.clo || (a.clo == b.clo && a.idx < b.idx); });
+        for (auto& a : adj) { std::sort(a.begin(), a.end()); a.erase(std::unique(a.begin(), a.end()), a.end()); }
+        pl->dep_off.assign(ni + 1, 0);
+        pl->dep_idx.clear();
+        std::vector<int> mine;
+        for (int i = 0; i < ni; ++i) {
+            const int s = flat[i].strip;
+            mine.clear();
+            auto scan = [&](int t) {
+                const std::vector<Run>& r = runs[t];
+                // runs are consecutive along x: clo and chi both ascend; first run with chi >= clo[i]
+                size_t lo = 0, hi = r.size();
+                while (lo < hi) { const size_t mid = (lo + hi) / 2; if (r[mid].chi < clo[i]) lo = mid + 1; else hi = mid; }
+                // chi is not strictly sorted when a strip ends with a short run: step back over equal / larger values
+                while (lo > 0 && r[lo - 1].chi >= clo[i]) --lo;
+                for (size_t j = lo; j < r.size() && r[j].clo <= chi[i]; ++j)
+                    if (r[j].chi >= clo[i] && r[j].idx < i) mine.push_back(r[j].idx);
+            };
+            scan(s);
+            for (int t : adj[s]) scan(t);
+            std::sort(mine.begin(), mine.end());
+            pl->dep_idx.insert(pl->dep_idx.end(), mine.begin(), mine.end());
+            pl->dep_off[i + 1] = (int)pl->dep_idx.size();
+        }
+        // transposed lists (successors) and the initial control block
+        {
+            std::vector<int> soff(ni + 1, 0), sidx(pl->dep_idx.size());
+            for (int j : pl->dep_idx) soff[j + 1] += 1;
+            for (int i = 0; i < ni; ++i) soff[i + 1] += soff[i];
+            std::vector<int> fill(soff.begin(), soff.end() - 1);
+            for (int i = 0; i < ni; ++i)
+                for (int d = pl->dep_off[i]; d < pl->dep_off[i + 1]; ++d) sidx[fill[pl->dep_idx[d]]++] = i;
+            std::vector<unsigned> init((size_t)kCtrlHeads + std::max(ni, 1), 0u);
+            for (int i = 0; i < ni; ++i) init[kCtrlHeads + i] = (unsigned)(pl->dep_off[i + 1] - pl->dep_off[i]);
+            E2E_CUDA(cudaMalloc(&pl->d_succ_off, sizeof(int) * (ni + 1)));
+            E2E_CUDA(cudaMemcpy(pl->d_succ_off, soff.data(), sizeof(int) * (ni + 1), cudaMemcpyHostToDevice));
+            E2E_CUDA(cudaMalloc(&pl->d_succ_idx, sizeof(int) * std::max<size_t>(1, sidx.size())));
+            if (!sidx.empty()) E2E_CUDA(cudaMemcpy(pl->d_succ_idx, sidx.data(), sizeof(int) * sidx.size(), cudaMemcpyHostToDevice));
+            E2E_CUDA(cudaMalloc(&pl->d_ctrl_init, sizeof(unsigned) * init.size()));
+            E2E_CUDA(cudaMemcpy(pl->d_ctrl_init, init.data(), sizeof(unsigned) * init.size(), cudaMemcpyHostToDevice));
+        }
+        E2E_CUDA(cudaMalloc(&pl->d_dep_off, sizeof(int) * (ni + 1)));
+        E2E_CUDA(cudaMemcpy(pl->d_dep_off, pl->dep_off.data(), sizeof(int) * (ni + 1), cudaMemcpyHostToDevice));
+        E2E_CUDA(cudaMalloc(&pl->d_dep_idx, sizeof(int) * std::max<size_t>(1, pl->dep_idx.size())));
+        if (!pl->dep_idx.empty())
+            E2E_CUDA(cudaMemcpy(pl->d_dep_idx, pl->dep_idx.data(), sizeof(int) * pl->dep_idx.size(), cudaMemcpyHostToDevice));
+    }
     E2E_CUDA(cudaMalloc(&pl->d_strips, sizeof(Strip) * std::max(1, n_strips)));
     E2E_CUDA(cudaMemcpy(pl->d_strips, pl->strips.data(), sizeof(Strip) * n_strips, cudaMemcpyHostToDevice));
     E2E_CUDA(cudaMalloc(&pl->d_items, sizeof(Item) * std::max<size_t>(1, flat.size())));
@@ -751,19 +832,25 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
             if (!bstrips.empty()) E2E_CUDA(cudaMemcpy(part.d_strips, bstrips.data(), sizeof(int) * bstrips.size(), cudaMemcpyHostToDevice));
             E2E_CUDA(cudaMalloc(&part.d_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
             if (!bflat.empty()) E2E_CUDA(cudaMemcpy(part.d_items, bflat.data(), sizeof(Item) * bflat.size(), cudaMemcpyHostToDevice));
+            // the band's items (ids = positions in `flat`) in queue order, for the persistent launch
+            std::vector<int> bq;
+            part.queue_off.assign(want + 1, 0);
+            for (int b = 0; b < want; ++b) {
+                for (int i = 0; i < (int)flat.size(); ++i)
+                    if (band_of[flat[i].strip] == b) bq.push_back(i);
+                part.queue_off[b + 1] = (int)bq.size();
+            }
+            E2E_CUDA(cudaMalloc(&part.d_queue, sizeof(int) * std::max<size_t>(1, bq.size())));
+            if (!bq.empty()) E2E_CUDA(cudaMemcpy(part.d_queue, bq.data(), sizeof(int) * bq.size(), cudaMemcpyHostToDevice));
             return E2E_OK;
         };
         // host path: 8 bands of growing size when a band's launches are few (2 colours x 2 classes); frames with many
         // colours (10 fibers per order: 10 launches per band) measured better with 6 equal bands
         const bool many_phases = phases.size() > 4;
-        int want = many_phases ? 6 : kHostBands;
-        if (const char* e = getenv("E2E_HOST_BANDS")) want = std::max(1, std::min(atoi(e), 16));
-        const char* rampenv = getenv("E2E_HOST_BAND_RAMP");
-        int rc = build_part(want, rampenv ? rampenv[0] != '0' : !many_phases, pl->host);
+        const int want = many_phases ? 6 : kHostBands;
+        int rc = build_part(want, !many_phases, pl->host);
         if (rc) return rc;
-        int parts = kDeviceParts;
-        if (const char* e = getenv("E2E_DEVICE_PARTS")) parts = std::max(1, std::min(atoi(e), 4));
-        rc = build_part(parts, false, pl->halves);
+        rc = build_part(kDeviceParts, false, pl->halves);
         if (rc) return rc;
     }
     *out = pl.get();
@@ -808,73 +895,100 @@ static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spect
     return E2E_OK;
 }
 
-// dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials.
-// E2E_RENDER=poly|moment overrides the rule (A/B measurements)
+// dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials
 static bool choose_moment(const e2e_format* F, const e2e_psf* P)
 {
-    const char* mode = getenv("E2E_RENDER");
-    bool use = P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
-    if (mode && !strcmp(mode, "poly")) use = false;
-    if (mode && !strcmp(mode, "moment") && P->kind == 0 && P->moment_npt > 0) use = true;
-    return use;
+    return P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
 }
 
-// tabulated PSF: cell-deposit kernel unless the oversampling is too fine for its weight array;
-// E2E_TAB=lattice forces the per-sample lattice kernel (A/B measurements)
-static bool choose_tabcell(const e2e_psf* P)
+// tabulated PSF: cell-deposit kernel unless the oversampling is too fine for its weight array
+static bool choose_tabcell(const e2e_psf* P) { return P->kind == 1 && P->tab.pi != nullptr; }
+
+// control block of the persistent render launch: kCtrlHeads head counters + one flag per item (zeroed before the launch)
+static size_t ctrl_bytes(const e2e_plan* pl) { return align_up(sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)), 256); }
+
+// (re)initialise a control block in the caller's workspace for one launch: head counters 0, dependency counters from the plan
+static cudaError_t ctrl_reset(const e2e_plan* pl, unsigned* ctrl, cudaStream_t stream)
 {
-    const char* mode = getenv("E2E_TAB");
-    return P->kind == 1 && P->tab.pi != nullptr && !(mode && !strcmp(mode, "lattice"));
+    return cudaMemcpyAsync(ctrl, pl->d_ctrl_init, sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)),
+                           cudaMemcpyDeviceToDevice, stream);
+}
+
+// one queue of a persistent launch: the whole plan (queue = nullptr) or one row band of the host path
+struct QueueSel {
+    unsigned* ctrl = nullptr;      // zeroed control block in the caller's workspace
+    const int* queue = nullptr;
+    int n = 0;
+    int head = 0;
+};
+
+// dynamic shared memory attribute of the moment kernel: per device, set once
+template <int NPT>
+static int moment_kernel_attr(size_t smem)
+{
+    static bool set[64] = {};
+    int dev = 0;
+    E2E_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(E2E_ERR_UNSUPPORTED, "render: device index above 63");
+    if (!set[dev]) {
+        E2E_CUDA(cudaFuncSetAttribute(render_moment_kernel<NPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        set[dev] = true;
+    }
+    return E2E_OK;
 }
 
 static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const double* d_x, const double* d_y,
-                         const double* d_w, double* d_frame, cudaStream_t stream, const Item* d_item_list = nullptr,
+                         const double* d_w, double* d_frame, cudaStream_t stream, const QueueSel& qs, const Item* d_item_list = nullptr,
                          const int* phase_off = nullptr, int n_phases = -1, int n_frames = 1, long long w_stride = 0,
                          double* const* d_frames = nullptr, double* const* h_frames = nullptr)
 {
-    // batch (e2e_render_frames): the production kernel takes the frame index from blockIdx.y; the other kernels
-    // render frame after frame
-    if (n_frames > 1 && !choose_moment(F, P)) {
+    const bool use_moment = choose_moment(F, P);
+    if (use_moment) {
+        // production kernel: ONE launch for the whole queue, one warp per item (all frames of a batch: blockIdx.y = frame)
+        if (!qs.ctrl) return fail(E2E_ERR_WORKSPACE, "render: no control block");
+        if (qs.n <= 0) return E2E_OK;
+        QueueParam W;
+        W.queue = qs.queue; W.n = qs.n; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
+        W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx;
+        W.ctrl = qs.ctrl; W.head = qs.head; W.ctrl_stride = (long long)(ctrl_bytes(pl) / sizeof(unsigned));
+#define E2E_MOM_CASE(NPT)                                                                                               \
+    case NPT: {                                                                                                         \
+        const size_t sm = sizeof(MomentWarpSmem<NPT>) * kMomWarps;                                                      \
+        int rc = moment_kernel_attr<NPT>(sm);                                                                           \
+        if (rc) return rc;                                                                                              \
+        const unsigned pb = (unsigned)((qs.n + kMomWarps - 1) / kMomWarps);                                             \
+        render_moment_kernel<NPT><<<dim3(pb, n_frames), kMomWarps * 32, sm, stream>>>(                                  \
+            d_x, d_y, d_w, pl->d_strips, pl->d_items, W, P->mom, d_frame, F->view.nx, F->view.ny, w_stride,             \
+            n_frames > 1 ? d_frames : nullptr);                                                                          \
+    } break;
+        switch (P->moment_npt) {
+            E2E_MOM_CASE(2) E2E_MOM_CASE(3) E2E_MOM_CASE(4)
+            default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+        }
+#undef E2E_MOM_CASE
+        count_launch();
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(e, "render_moment_kernel launch");
+        return E2E_OK;
+    }
+    // the other kernels: one launch per phase (items of one phase share no pixel); a batch renders frame after frame
+    if (n_frames > 1) {
         for (int b = 0; b < n_frames; ++b) {
-            int rc = launch_render(F, P, pl, d_x, d_y, d_w + (size_t)b * w_stride, h_frames[b], stream, d_item_list, phase_off, n_phases);
+            int rc = launch_render(F, P, pl, d_x, d_y, d_w + (size_t)b * w_stride, h_frames[b], stream, qs, d_item_list, phase_off, n_phases);
             if (rc) return rc;
         }
         return E2E_OK;
     }
     if (!d_item_list) { d_item_list = pl->d_items; phase_off = pl->phase_off.data(); n_phases = pl->n_phases; }
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
     const size_t smem_an = (size_t)kWarpsPerCta * (kWinCols + kWinRows) * kLdk * sizeof(double);
     const int lat_ld = kTabWin + 2;
     const size_t smem_tab = (size_t)kWarpsPerCta * lat_ld * lat_ld * sizeof(double);
-    std::call_once(once, [&] {
-        attr_err = cudaFuncSetAttribute(render_analytic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_an);
-    });
-    if (attr_err != cudaSuccess) return fail_cuda(attr_err, "cudaFuncSetAttribute(render_analytic_kernel)");
-    const bool use_moment = choose_moment(F, P);
     const bool use_tabcell = choose_tabcell(P);
     for (int ph = 0; ph < n_phases; ++ph) {
         const int i0 = phase_off[ph], n = phase_off[ph + 1] - i0;
         if (n <= 0) continue;
         const unsigned blocks = (unsigned)((n + kWarpsPerCta - 1) / kWarpsPerCta);
-        if (use_moment) {
-            const unsigned pb = (unsigned)((n + kMomWarps - 1) / kMomWarps);
-#define E2E_MOM_CASE(NPT)                                                                                               \
-    case NPT: {                                                                                                         \
-        const size_t sm = sizeof(MomentWarpSmem<NPT>) * kMomWarps;                                                      \
-        static cudaError_t attr = cudaFuncSetAttribute(render_moment_kernel<NPT>,                                       \
-                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);           \
-        if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_moment_kernel)");                  \
-        render_moment_kernel<NPT><<<dim3(pb, n_frames), kMomWarps * 32, sm, stream>>>(                                  \
-            d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n, P->mom, d_frame, F->view.nx, F->view.ny, w_stride,        \
-            n_frames > 1 ? d_frames : nullptr);                                                                          \
-    } break;
-            switch (P->moment_npt) {
-                E2E_MOM_CASE(2) E2E_MOM_CASE(3) E2E_MOM_CASE(4)
-                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
-            }
-#undef E2E_MOM_CASE
-        } else if (P->kind == 0 && P->poly_degree > 0) {
+        if (P->kind == 0 && P->poly_degree > 0) {
             const unsigned pb = (unsigned)((n + kPolyWarps - 1) / kPolyWarps);
             const size_t sm = sizeof(PolyWarpSmem) * kPolyWarps;
 #define E2E_POLY_CASE(DEG)                                                                                              \
@@ -887,10 +1001,13 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
                 default: return fail(E2E_ERR_UNSUPPORTED, "render: no kernel for this polynomial degree");
             }
 #undef E2E_POLY_CASE
-        } else if (P->kind == 0)
+        } else if (P->kind == 0) {
+            // the attribute is per device: set it before every launch (cheap) rather than once per process
+            cudaError_t attr = cudaFuncSetAttribute(render_analytic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_an);
+            if (attr != cudaSuccess) return fail_cuda(attr, "cudaFuncSetAttribute(render_analytic_kernel)");
             render_analytic_kernel<<<blocks, kWarpsPerCta * 32, smem_an, stream>>>(d_x, d_y, d_w, pl->d_strips, d_item_list + i0, n,
                                                                                    P->an, d_frame, F->view.nx, F->view.ny);
-        else if (use_tabcell) {
+        } else if (use_tabcell) {
             const unsigned pb = (unsigned)((n + kTcWarps - 1) / kTcWarps);
             const size_t sm = 8 * tabcell_warp_smem_doubles(P->tab.os) * kTcWarps;
             cudaError_t attr = cudaFuncSetAttribute(render_tabcell_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
@@ -919,7 +1036,7 @@ int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, si
     e2e_plan* pl = nullptr;
     int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
-    *bytes = 3 * sample_array_bytes(pl->total_samples);
+    *bytes = 3 * sample_array_bytes(pl->total_samples) + ctrl_bytes(pl);
     return E2E_OK;
 }
 
@@ -968,11 +1085,15 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     if (rc) return rc;
     const size_t per = sample_array_bytes(pl->total_samples);
     if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace NULL or not 256-byte aligned");
-    if (workspace_bytes < 3 * per) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
+    if (workspace_bytes < 3 * per + ctrl_bytes(pl)) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     double* d_x = (double*)d_workspace;
     double* d_y = (double*)((char*)d_workspace + per);
     double* d_w = (double*)((char*)d_workspace + 2 * per);
+    QueueSel qs;
+    qs.ctrl = (unsigned*)((char*)d_workspace + 3 * per);
+    qs.n = pl->n_items;
+    const bool persistent = choose_moment(fmt, psf);
     if (!accumulate) {
         StageTimer tm(kStageZero, stream);
         E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
@@ -980,6 +1101,7 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     {
         StageTimer tm(kStageSetup, stream);
         const long long before = g_launches.load();
+        if (persistent) E2E_CUDA(ctrl_reset(pl, qs.ctrl, stream));
         rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
         if (rc) return rc;
@@ -987,28 +1109,26 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     {
         StageTimer tm(kStageRender, stream);
         const long long before = g_launches.load();
-        const int nparts = pl->halves.n_bands;
+        const int nparts = persistent ? 1 : pl->halves.n_bands;
         HostPipe* hp = nparts >= 2 ? host_pipe() : nullptr;
         if (hp) {
-            // row bands that share no pixel, rendered concurrently: the tail of one band's launch (a few long items on
-            // otherwise idle SMs) overlaps the other bands' work.  Fork to the library's streams and join.
+            // phase-launched kernels: two row bands that share no pixel, rendered concurrently: the tail of one band's launch
+            // (a few long items on otherwise idle SMs) overlaps the other band's work.  Fork to the library's stream and join.
             std::lock_guard<std::mutex> lk(hp->mu);
             const int np1 = pl->n_phases_all + 1;
-            cudaStream_t sp[4] = {stream, hp->aux, hp->aux2[0], hp->aux2[1]};
-            cudaEvent_t done[4] = {nullptr, hp->ev_aux_done, hp->ev_aux2_done[0], hp->ev_aux2_done[1]};
+            cudaStream_t sp[2] = {stream, hp->aux};
             cudaError_t ce = cudaEventRecord(hp->ev_start, stream);
-            for (int b = 1; b < nparts && ce == cudaSuccess; ++b) ce = cudaStreamWaitEvent(sp[b], hp->ev_start, 0);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(hp->aux, hp->ev_start, 0);
             if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: fork");
-            for (int b = 0; b < nparts && !rc; ++b)
-                rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, sp[b], pl->halves.d_items,
+            for (int b = 0; b < 2 && !rc; ++b)
+                rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, sp[b], qs, pl->halves.d_items,
                                    pl->halves.phase_off.data() + (size_t)b * np1, pl->n_phases_all);
-            for (int b = 1; b < nparts && ce == cudaSuccess; ++b) {
-                ce = cudaEventRecord(done[b], sp[b]);
-                if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, done[b], 0);
-            }
+            // join even when a launch failed: the caller's stream must not run ahead of work already forked
+            ce = cudaEventRecord(hp->ev_aux_done, hp->aux);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, hp->ev_aux_done, 0);
             if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: join");
         } else {
-            rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream);
+            rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, qs);
         }
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
     }
@@ -1021,7 +1141,11 @@ int e2e_render_frames_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* 
     size_t one = 0;
     int rc = e2e_render_workspace_bytes(fmt, psf, &one);
     if (rc) return rc;
-    *bytes = one / 3 * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256);
+    e2e_plan* pl = nullptr;
+    rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    *bytes = sample_array_bytes(pl->total_samples) * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256) +
+             ctrl_bytes(pl) * (size_t)n_frames;
     return E2E_OK;
 }
 
@@ -1044,7 +1168,8 @@ int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_f
     int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
     const size_t per = sample_array_bytes(pl->total_samples);
-    const size_t need = per * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256);
+    const size_t ptr_bytes = align_up(sizeof(double*) * (size_t)n_frames, 256);
+    const size_t need = per * (2 + (size_t)n_frames) + ptr_bytes + ctrl_bytes(pl) * (size_t)n_frames;
     if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace NULL or not 256-byte aligned");
     if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace too small");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
@@ -1052,6 +1177,12 @@ int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_f
     double* d_y = (double*)((char*)d_workspace + per);
     double* d_w = (double*)((char*)d_workspace + 2 * per);
     double** d_ptrs = (double**)((char*)d_workspace + per * (2 + (size_t)n_frames));
+    QueueSel qs;
+    qs.ctrl = (unsigned*)((char*)d_ptrs + ptr_bytes);
+    qs.n = pl->n_items;
+    if (choose_moment(fmt, psf))
+        for (int b = 0; b < n_frames; ++b)
+            E2E_CUDA(ctrl_reset(pl, (unsigned*)((char*)qs.ctrl + ctrl_bytes(pl) * (size_t)b), stream));
     // pageable source: the copy is staged before the call returns, so the caller's array need not outlive it
     E2E_CUDA(cudaMemcpyAsync(d_ptrs, d_frames, sizeof(double*) * (size_t)n_frames, cudaMemcpyHostToDevice, stream));
     if (!accumulate) {
@@ -1071,7 +1202,7 @@ int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_f
     {
         StageTimer tm(kStageRender, stream);
         const long long before = g_launches.load();
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frames[0], stream, nullptr, nullptr, -1, n_frames, (long long)(per / 8),
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frames[0], stream, qs, nullptr, nullptr, -1, n_frames, (long long)(per / 8),
                            d_ptrs, d_frames);
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
     }
@@ -1084,7 +1215,8 @@ int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* ps
     size_t inner = 0;
     int rc = e2e_render_workspace_bytes(fmt, psf, &inner);
     if (rc) return rc;
-    size_t total = align_up((size_t)fmt->view.nx * fmt->view.ny * 8, 256);
+    const size_t npx = (size_t)fmt->view.nx * fmt->view.ny;
+    size_t total = align_up(npx * 8, 256) + align_up(npx * 2, 256);       // fp64 frame + uint16 ADC frame
     for (int f = 0; f < fmt->view.n_fibers; ++f) {
         if (spectra[f].n < 2) return fail(E2E_ERR_INVALID_ARG, "render_host_workspace_bytes: bad spectrum descriptor");
         total += align_up((size_t)spectra[f].n * 8, 256);
@@ -1093,108 +1225,7 @@ int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* ps
     return E2E_OK;
 }
 
-int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
-                          const e2e_detector_t* det, double* h_frame, void* d_workspace, size_t workspace_bytes,
-                          void* cuda_stream)
-{
-    if (!fmt || !psf || !h_frame) return fail(E2E_ERR_INVALID_ARG, "render_frame_host: NULL argument");
-    int rc = check_spectra(fmt, spectra, "render_frame_host");
-    if (rc) return rc;
-    size_t need = 0;
-    rc = e2e_render_host_workspace_bytes(fmt, psf, spectra, &need);
-    if (rc) return rc;
-    if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace NULL or not 256-byte aligned");
-    if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace too small");
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    char* p = (char*)d_workspace;
-    double* d_frame = (double*)p;
-    const size_t frame_bytes = (size_t)fmt->view.nx * fmt->view.ny * 8;
-    p += align_up(frame_bytes, 256);
-    std::vector<e2e_spectrum_t> dev(spectra, spectra + fmt->view.n_fibers);
-    for (int f = 0; f < fmt->view.n_fibers; ++f) {
-        // fibers that share one host table share one device copy
-        int same = -1;
-        for (int g = 0; g < f; ++g)
-            if (spectra[g].d_flux == spectra[f].d_flux && spectra[g].n == spectra[f].n) { same = g; break; }
-        if (same >= 0) { dev[f].d_flux = dev[same].d_flux; continue; }
-        E2E_CUDA(cudaMemcpyAsync(p, spectra[f].d_flux, (size_t)spectra[f].n * 8, cudaMemcpyHostToDevice, stream));
-        dev[f].d_flux = (const double*)p;
-        p += align_up((size_t)spectra[f].n * 8, 256);
-    }
-    const size_t used = (size_t)(p - (char*)d_workspace);
-    e2e_plan* pl = nullptr;
-    rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
-    if (rc) return rc;
-    HostPipe* hp = host_pipe();
-    if (pl->host.n_bands <= 1 || !hp) {
-        // one pass: render, detector, copy
-        rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
-        if (rc) return rc;
-        if (det) {
-            rc = e2e_apply_detector(d_frame, d_frame, fmt->view.nx, fmt->view.ny, det, stream);
-            if (rc) return rc;
-        }
-        E2E_CUDA(cudaMemcpyAsync(h_frame, d_frame, frame_bytes, cudaMemcpyDeviceToHost, stream));
-        E2E_CUDA(cudaStreamSynchronize(stream));
-        return E2E_OK;
-    }
-    // banded pipeline: a1-a3 for the whole frame, then per row band a4 + a5 (+ a6 on the rows that became final) on the
-    // caller's stream while the previous band's rows travel to the host on the library's copy stream
-    const size_t per = sample_array_bytes(pl->total_samples);
-    if (workspace_bytes - used < 3 * per) return fail(E2E_ERR_WORKSPACE, "render_frame_host: workspace too small");
-    double* d_x = (double*)p;
-    double* d_y = (double*)(p + per);
-    double* d_w = (double*)(p + 2 * per);
-    const int nx = fmt->view.nx, ny = fmt->view.ny;
-    if (det && (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias)))
-        return fail(E2E_ERR_INVALID_ARG, "render_frame_host: non-finite detector parameter");
-    std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
-    E2E_CUDA(cudaMemsetAsync(d_frame, 0, frame_bytes, stream));
-    // bands share no pixel (build_plan): even bands on the caller's stream, odd bands on the library's second stream
-    E2E_CUDA(cudaEventRecord(hp->ev_start, stream));
-    E2E_CUDA(cudaStreamWaitEvent(hp->aux, hp->ev_start, 0));
-    int row0 = 0;
-    for (int b = 0; b < pl->host.n_bands; ++b) {
-        cudaStream_t cs = (b & 1) ? hp->aux : stream;
-        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &pl->host, b);   // a1-a3 of this band's strips only
-        if (rc) return rc;
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, pl->host.d_items,
-                           pl->host.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
-        if (rc) return rc;
-        const int row1 = std::max(row0, pl->host.fin_row[b]);
-        if (row1 > row0) {
-            const size_t off = (size_t)row0 * nx;
-            const long long npx = (long long)(row1 - row0) * nx;
-            if (det) {
-                rc = launch_detector(d_frame + off, d_frame + off, npx, *det, cs, (long long)off);
-                if (rc) return rc;
-            }
-            cudaEvent_t ev = hp->ev[b % HostPipe::kEvents];
-            E2E_CUDA(cudaEventRecord(ev, cs));
-            E2E_CUDA(cudaStreamWaitEvent(hp->copy, ev, 0));
-            E2E_CUDA(cudaMemcpyAsync(h_frame + off, d_frame + off, (size_t)npx * 8, cudaMemcpyDeviceToHost, hp->copy));
-            row0 = row1;
-        }
-    }
-    E2E_CUDA(cudaEventRecord(hp->ev_aux_done, hp->aux));
-    E2E_CUDA(cudaStreamWaitEvent(stream, hp->ev_aux_done, 0));
-    E2E_CUDA(cudaStreamSynchronize(stream));
-    E2E_CUDA(cudaStreamSynchronize(hp->copy));
-    (void)ny;
-    return E2E_OK;
-}
-
-int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_t* det,
-                       void* cuda_stream)
-{
-    if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector: NULL argument");
-    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector: bad frame size");
-    if (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias))
-        return fail(E2E_ERR_INVALID_ARG, "apply_detector: non-finite parameter");
-    StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
-    if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
-    return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
-}
+}  // extern "C"
 
 static int check_detector_ex(const e2e_detector_ex_t* det, int32_t nx, const void* d_out, bool out16, const char* who)
 {
@@ -1220,6 +1251,165 @@ static int check_detector_ex(const e2e_detector_ex_t* det, int32_t nx, const voi
     return E2E_OK;
 }
 
+// HOST-buffer render: det (basic stage, fp64 electrons out), or det_ex (full stage; out16: uint16 ADC counts), or neither
+static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                                  const e2e_detector_t* det, const e2e_detector_ex_t* det_ex, bool out16, void* h_frame,
+                                  void* d_workspace, size_t workspace_bytes, void* cuda_stream, const char* who)
+{
+    const std::string w(who);
+    if (!fmt || !psf || !h_frame) return fail(E2E_ERR_INVALID_ARG, w + ": NULL argument");
+    int rc = check_spectra(fmt, spectra, who);
+    if (rc) return rc;
+    size_t need = 0;
+    rc = e2e_render_host_workspace_bytes(fmt, psf, spectra, &need);
+    if (rc) return rc;
+    if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, w + ": workspace NULL or not 256-byte aligned");
+    if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
+    const int nx = fmt->view.nx, ny = fmt->view.ny;
+    if (det && (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias)))
+        return fail(E2E_ERR_INVALID_ARG, w + ": non-finite detector parameter");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    char* p = (char*)d_workspace;
+    double* d_frame = (double*)p;
+    const size_t npix = (size_t)nx * ny;
+    p += align_up(npix * 8, 256);
+    uint16_t* d_adu = (uint16_t*)p;
+    p += align_up(npix * 2, 256);
+    if (det_ex) {
+        rc = check_detector_ex(det_ex, nx, out16 ? (void*)d_adu : (void*)d_frame, out16, who);
+        if (rc) return rc;
+    }
+    const size_t out_elem = out16 ? 2 : 8;
+    const char* d_out = out16 ? (const char*)d_adu : (const char*)d_frame;
+    std::vector<e2e_spectrum_t> dev(spectra, spectra + fmt->view.n_fibers);
+    for (int f = 0; f < fmt->view.n_fibers; ++f) {
+        // fibers that share one host table share one device copy
+        int same = -1;
+        for (int g = 0; g < f; ++g)
+            if (spectra[g].d_flux == spectra[f].d_flux && spectra[g].n == spectra[f].n) { same = g; break; }
+        if (same >= 0) { dev[f].d_flux = dev[same].d_flux; continue; }
+        E2E_CUDA(cudaMemcpyAsync(p, spectra[f].d_flux, (size_t)spectra[f].n * 8, cudaMemcpyHostToDevice, stream));
+        dev[f].d_flux = (const double*)p;
+        p += align_up((size_t)spectra[f].n * 8, 256);
+    }
+    const size_t used = (size_t)(p - (char*)d_workspace);
+    e2e_plan* pl = nullptr;
+    rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    // a6 on the rows [row0, row1) of the device frame (in place for fp64 output, into the uint16 frame otherwise)
+    auto detector_rows = [&](int row0, int row1, cudaStream_t cs) -> int {
+        const size_t off = (size_t)row0 * nx;
+        const long long n = (long long)(row1 - row0) * nx;
+        if (det_ex)
+            return launch_detector_ex(d_frame + off, out16 ? (void*)(d_adu + off) : (void*)(d_frame + off), out16, n, nx, *det_ex, cs,
+                                      (long long)off);
+        if (det) return launch_detector(d_frame + off, d_frame + off, n, *det, cs, (long long)off);
+        return E2E_OK;
+    };
+    HostPipe* hp = host_pipe();
+    if (pl->host.n_bands <= 1 || !hp) {
+        // one pass: render, detector, copy
+        rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
+        if (rc) return rc;
+        rc = detector_rows(0, ny, stream);
+        if (rc) return rc;
+        E2E_CUDA(cudaMemcpyAsync(h_frame, d_out, npix * out_elem, cudaMemcpyDeviceToHost, stream));
+        E2E_CUDA(cudaStreamSynchronize(stream));
+        return E2E_OK;
+    }
+    // banded pipeline: per row band a1-a3 of its strips, a4 + a5, a6 on the rows that became final, then those rows travel
+    // to the host on the library's copy stream while the next bands render
+    const size_t per = sample_array_bytes(pl->total_samples);
+    if (workspace_bytes - used < 3 * per + ctrl_bytes(pl)) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
+    double* d_x = (double*)p;
+    double* d_y = (double*)(p + per);
+    double* d_w = (double*)(p + 2 * per);
+    unsigned* d_ctrl = (unsigned*)(p + 3 * per);
+    if (pl->host.n_bands > kCtrlHeads) return fail(E2E_ERR_UNSUPPORTED, w + ": too many row bands");
+    std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
+    E2E_CUDA(cudaMemsetAsync(d_frame, 0, npix * 8, stream));
+    E2E_CUDA(ctrl_reset(pl, d_ctrl, stream));
+    // bands share no pixel (build_plan): even bands on the caller's stream, odd bands on the library's second stream
+    E2E_CUDA(cudaEventRecord(hp->ev_start, stream));
+    E2E_CUDA(cudaStreamWaitEvent(hp->aux, hp->ev_start, 0));
+    // from here on work is forked: every exit goes through the join below (errors are remembered, not returned at once)
+    cudaError_t ce = cudaSuccess;
+    int row0 = 0;
+    for (int b = 0; b < pl->host.n_bands && !rc && ce == cudaSuccess; ++b) {
+        cudaStream_t cs = (b & 1) ? hp->aux : stream;
+        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &pl->host, b);   // a1-a3 of this band's strips only
+        if (rc) break;
+        QueueSel qs;
+        qs.ctrl = d_ctrl; qs.head = b;
+        qs.queue = pl->host.d_queue + pl->host.queue_off[b];
+        qs.n = pl->host.queue_off[b + 1] - pl->host.queue_off[b];
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, qs, pl->host.d_items,
+                           pl->host.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        if (rc) break;
+        const int row1 = std::max(row0, pl->host.fin_row[b]);
+        if (row1 > row0) {
+            rc = detector_rows(row0, row1, cs);
+            if (rc) break;
+            const size_t off = (size_t)row0 * nx;
+            cudaEvent_t ev = hp->ev[b % HostPipe::kEvents];
+            ce = cudaEventRecord(ev, cs);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(hp->copy, ev, 0);
+            if (ce == cudaSuccess)
+                ce = cudaMemcpyAsync((char*)h_frame + off * out_elem, d_out + off * out_elem, (size_t)(row1 - row0) * nx * out_elem,
+                                     cudaMemcpyDeviceToHost, hp->copy);
+            row0 = row1;
+        }
+    }
+    // join: the caller's stream waits for the second stream, and the call for both and for the copies
+    cudaError_t cj = cudaEventRecord(hp->ev_aux_done, hp->aux);
+    if (cj == cudaSuccess) cj = cudaStreamWaitEvent(stream, hp->ev_aux_done, 0);
+    cudaError_t c1 = cudaStreamSynchronize(hp->aux), c2 = cudaStreamSynchronize(stream), c3 = cudaStreamSynchronize(hp->copy);
+    if (rc) return rc;
+    for (cudaError_t e : {ce, cj, c1, c2, c3})
+        if (e != cudaSuccess) return fail_cuda(e, who);
+    return E2E_OK;
+}
+
+extern "C" {
+
+int e2e_render_frame_host(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                          const e2e_detector_t* det, double* h_frame, void* d_workspace, size_t workspace_bytes,
+                          void* cuda_stream)
+{
+    return render_frame_host_impl(fmt, psf, spectra, det, nullptr, false, h_frame, d_workspace, workspace_bytes, cuda_stream,
+                                  "render_frame_host");
+}
+
+int e2e_render_frame_host_ex(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                             const e2e_detector_ex_t* det, double* h_frame, void* d_workspace, size_t workspace_bytes,
+                             void* cuda_stream)
+{
+    if (!det) return fail(E2E_ERR_INVALID_ARG, "render_frame_host_ex: det is NULL");
+    return render_frame_host_impl(fmt, psf, spectra, nullptr, det, false, h_frame, d_workspace, workspace_bytes, cuda_stream,
+                                  "render_frame_host_ex");
+}
+
+int e2e_render_frame_host_adu16(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                                const e2e_detector_ex_t* det, uint16_t* h_frame, void* d_workspace, size_t workspace_bytes,
+                                void* cuda_stream)
+{
+    if (!det) return fail(E2E_ERR_INVALID_ARG, "render_frame_host_adu16: det is NULL");
+    return render_frame_host_impl(fmt, psf, spectra, nullptr, det, true, h_frame, d_workspace, workspace_bytes, cuda_stream,
+                                  "render_frame_host_adu16");
+}
+
+int e2e_apply_detector(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_t* det,
+                       void* cuda_stream)
+{
+    if (!d_frame_in || !d_frame_out || !det) return fail(E2E_ERR_INVALID_ARG, "apply_detector: NULL argument");
+    if (nx <= 0 || ny <= 0) return fail(E2E_ERR_INVALID_ARG, "apply_detector: bad frame size");
+    if (!is_fin(det->gain) || !is_fin(det->dark_e) || !is_fin(det->ron_e) || !is_fin(det->bias))
+        return fail(E2E_ERR_INVALID_ARG, "apply_detector: non-finite parameter");
+    StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
+    if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
+    return launch_detector(d_frame_in, d_frame_out, (long long)nx * ny, *det, (cudaStream_t)cuda_stream);
+}
+
 int e2e_apply_detector_ex(const double* d_frame_in, double* d_frame_out, int32_t nx, int32_t ny, const e2e_detector_ex_t* det,
                           void* cuda_stream)
 {
@@ -1243,6 +1433,97 @@ int e2e_apply_detector_adu16(const double* d_frame_in, uint16_t* d_frame_out, in
     StageTimer tm(kStageDetector, (cudaStream_t)cuda_stream);
     if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_detector += 1; }
     return launch_detector_ex(d_frame_in, d_frame_out, true, (long long)nx * ny, nx, *det, (cudaStream_t)cuda_stream);
+}
+
+// Test hook: verifies on the device, pixel by pixel, the schedule invariants the frame's bit-reproducibility rests on
+// (plan_check.cuh).  Synchronous; allocates an int32 owner frame and frees it before returning.
+int e2e_plan_check(const e2e_format_t* fmt, const e2e_psf_t* psf, e2e_plan_check_t* out)
+{
+    if (!fmt || !psf || !out) return fail(E2E_ERR_INVALID_ARG, "plan_check: NULL argument");
+    if (psf->nx != fmt->view.nx || psf->ny != fmt->view.ny) return fail(E2E_ERR_INVALID_ARG, "plan_check: psf was created for another detector size");
+    memset(out, 0, sizeof(*out));
+    e2e_plan* pl = nullptr;
+    int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
+    if (rc) return rc;
+    const size_t npix = (size_t)fmt->view.nx * fmt->view.ny;
+    int* owner = nullptr;
+    PlanCheckCounters* d_cnt = nullptr;
+    unsigned* d_ctrl = nullptr;
+    E2E_CUDA(cudaMalloc(&owner, npix * sizeof(int)));
+    cudaError_t ce = cudaMalloc(&d_cnt, sizeof(PlanCheckCounters));
+    if (ce == cudaSuccess) ce = cudaMalloc(&d_ctrl, ctrl_bytes(pl));
+    auto done = [&](int code) { cudaFree(owner); if (d_cnt) cudaFree(d_cnt); if (d_ctrl) cudaFree(d_ctrl); return code; };
+    if (ce != cudaSuccess) return done(fail_cuda(ce, "plan_check: cudaMalloc"));
+    PlanCheckCounters h;
+    auto reset = [&](bool frame) {
+        cudaError_t e = cudaMemset(d_cnt, 0, sizeof(PlanCheckCounters));
+        if (e == cudaSuccess && frame) e = cudaMemset(owner, 0, npix * sizeof(int));
+        return e;
+    };
+    auto fetch = [&]() {
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e == cudaSuccess) e = cudaMemcpy(&h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost);
+        return e;
+    };
+    QueueParam nq;
+    memset(&nq, 0, sizeof(nq));
+    auto stamp = [&](const Item* list, int n, int mode, int band, int min_row, const QueueParam& W) {
+        if (n <= 0) return;
+        const int grid = mode == 2 ? std::min(n, 148 * 32) : std::min(n, 1 << 16);
+        plan_check_kernel<<<grid, 32>>>(fmt->view, pl->d_strips, list, n, mode, band, min_row, W, psf->hbx, psf->hby, owner, d_cnt);
+        count_launch();
+    };
+#define E2E_PC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return done(fail_cuda(e__, "plan_check")); } while (0)
+    out->n_items = pl->n_items; out->n_phases = pl->n_phases; out->n_dependencies = (int64_t)pl->dep_idx.size();
+    out->n_host_bands = pl->host.n_bands; out->n_device_bands = pl->halves.n_bands;
+    // (1) every phase launch of the plan: items of one phase share no pixel
+    for (int ph = 0; ph < pl->n_phases; ++ph) {
+        E2E_PC(reset(true));
+        stamp(pl->d_items + pl->phase_off[ph], pl->phase_off[ph + 1] - pl->phase_off[ph], 0, 0, 0, nq);
+        E2E_PC(fetch());
+        out->phase_conflicts += (int64_t)h.conflicts;
+        out->claimed_px = std::max<int64_t>(out->claimed_px, (int64_t)h.claimed);
+    }
+    // (2) the persistent launch: whole queue, then the host path's band queues
+    {
+        QueueParam W;
+        memset(&W, 0, sizeof(W));
+        W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx; W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.ctrl = d_ctrl;
+        E2E_PC(reset(true));
+        E2E_PC(ctrl_reset(pl, d_ctrl, nullptr));
+        W.queue = nullptr; W.n = pl->n_items; W.head = 0;
+        stamp(pl->d_items, pl->n_items, 2, 0, 0, W);
+        E2E_PC(fetch());
+        out->queue_conflicts += (int64_t)h.conflicts;
+        out->claimed_px = (int64_t)h.claimed;
+        E2E_PC(reset(true));
+        E2E_PC(ctrl_reset(pl, d_ctrl, nullptr));
+        for (int b = 0; b < pl->host.n_bands && b < kCtrlHeads; ++b) {
+            W.queue = pl->host.d_queue + pl->host.queue_off[b];
+            W.n = pl->host.queue_off[b + 1] - pl->host.queue_off[b];
+            W.head = b;
+            stamp(pl->d_items, W.n, 2, 0, 0, W);
+        }
+        E2E_PC(fetch());
+        out->queue_conflicts += (int64_t)h.conflicts;
+        if ((int64_t)h.claimed != out->claimed_px) out->queue_conflicts += 1;      // the band queues must cover the same pixels
+    }
+    // (3) row bands: no pixel in two bands; no row written after it was declared final
+    for (int which = 0; which < 2; ++which) {
+        const e2e_plan::BandPart& part = which == 0 ? pl->halves : pl->host;
+        const int np1 = pl->n_phases_all + 1;
+        E2E_PC(reset(true));
+        for (int b = 0; b < part.n_bands; ++b) {
+            const int i0 = part.phase_off[(size_t)b * np1], i1 = part.phase_off[(size_t)b * np1 + pl->n_phases_all];
+            stamp(part.d_items + i0, i1 - i0, 1, b, b > 0 ? part.fin_row[b - 1] : 0, nq);
+        }
+        E2E_PC(fetch());
+        if (which == 0) out->device_band_conflicts = (int64_t)h.conflicts;
+        else { out->host_band_conflicts = (int64_t)h.conflicts; out->host_rows_not_final = (int64_t)h.early_rows; }
+        if ((int64_t)h.claimed != out->claimed_px) out->host_band_conflicts += which == 1, out->device_band_conflicts += which == 0;
+    }
+#undef E2E_PC
+    return done(E2E_OK);
 }
 
 int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name, double* fma_cell, double* fma_sample)

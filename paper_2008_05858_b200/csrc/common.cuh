@@ -176,6 +176,14 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     e2e::Item* d_items = nullptr;
     int n_items = 0;
     int n_colors = 0;
+    // dependency lists of the persistent render launch (render_moment.cuh): item i waits for dep_idx[dep_off[i] .. dep_off[i+1])
+    // -- every item earlier in the queue (= lower index) whose pixels may overlap its own
+    int* d_dep_off = nullptr;
+    int* d_dep_idx = nullptr;
+    std::vector<int> dep_off, dep_idx;
+    int* d_succ_off = nullptr;         // the transposed lists: the items that wait for item i
+    int* d_succ_idx = nullptr;
+    unsigned* d_ctrl_init = nullptr;   // initial control block: head counters 0, then the number of dependencies per item
     // The same items regrouped into row bands that share no pixel (build_plan).  `host`: up to 8 bands of growing size for
     // e2e_render_frame_host (finished rows travel to the host while later bands render); `halves`: 2 equal bands that
     // e2e_render_frame renders concurrently on two streams (the tail of one band's launch overlaps the other band's work).
@@ -185,6 +193,8 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
         std::vector<int> phase_off, fin_row, strip_off;
         e2e::Item* d_items = nullptr;
         int* d_strips = nullptr;
+        std::vector<int> queue_off;    // [n_bands + 1] into d_queue: the band's item ids in queue order (persistent launch)
+        int* d_queue = nullptr;
     };
     BandPart host, halves;
     int n_phases_all = 0;          // phases before empty ones were dropped (colour x class)

@@ -32,9 +32,14 @@
 // ESPRESSO-like PSF (24 x 24 window, T = 6, NPT = 2): 30 DMMAs per term, 180 per cell (the first version of this kernel,
 // with both phases on the full range and the contraction over q last, needed 360).
 //
-// One warp per work item (run of consecutive 32-sample chunks of one strip; schedule of api.cu: items of one launch
-// never touch the same pixel), no block-level cooperation; the finished window is added to the frame by L2 reductions
-// (red.global.add.f64) that the flush's __syncwarp() keeps in cell order -> bit-reproducible.
+// One warp per work item (run of consecutive 32-sample chunks of one strip) and per CTA, no block-level cooperation.  ONE
+// launch renders a whole frame (or one row band of the host path): every warp takes the next item of the queue
+// (atomic ticket), waits until the items it shares pixels with and that come earlier in the queue are done (its counter
+// of unfinished dependencies reaches 0; the lists are built on the host, api.cu build_plan), renders, and decrements the
+// counters of its successors.  A pixel's
+// additions therefore happen in queue order whatever the timing -> bit-reproducible; inside a warp the finished windows
+// are added to the frame by L2 reductions (red.global.add.f64) that the flush's __syncwarp() keeps in cell order.
+// Deadlock-free: an item only waits for items taken before it, and a taken item is held by a running warp.
 #pragma once
 #include "common.cuh"
 #include "render_poly.cuh"
@@ -55,25 +60,82 @@ struct MomentWarpSmem {
     double vy[8 * kMomLdk];            // delta_k^p, p = 0..7 (rewritten for every cell: delta is relative to the cell's window)
 };
 
+// work queue of one render launch
+struct QueueParam {
+    const int* queue;              // item ids in queue order, or nullptr (= 0 .. n - 1)
+    int n;                         // items in the queue
+    const int* succ_off;           // [n_items + 1] CSR: the items that wait for item i (its successors; ids > i)
+    const int* succ_idx;
+    const int* dep_off;            // [n_items + 1] CSR of the transposed lists (the items i waits for); e2e_plan_check only
+    const int* dep_idx;
+    unsigned* ctrl;                // control block, initialised before the launch: head counters, then per item the number
+                                   // of its dependencies that are not finished yet
+    int head;                      // which head counter this launch uses
+    long long ctrl_stride;         // batch render: control block of frame b at ctrl + b * ctrl_stride (in unsigned)
+};
+constexpr int kCtrlHeads = 64;     // unsigned words before the counters
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_dec_u32(unsigned* p)
+{
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(0xffffffffu) : "memory");
+}
+
+// Take the next item of the queue and wait until its dependencies are finished.  The warp takes a TICKET rather than its
+// block index: tickets are handed out in the order in which warps really start, so every item before this one in the queue
+// is held by a warp that is already running (deadlock freedom).  The wait is a warp-uniform spin on ONE word (a per-lane
+// loop over dependency flags made ptxas spill 500 bytes of the render loop's state at 96 registers).  Returns -1 when the
+// queue is exhausted.
+__device__ __forceinline__ int queue_take(const QueueParam& W, unsigned* ctrl, int lane)
+{
+    unsigned qpos = 0;
+    if (lane == 0) qpos = atomicAdd(ctrl + W.head, 1u);
+    qpos = __shfl_sync(0xffffffffu, qpos, 0);
+    if (qpos >= (unsigned)W.n) return -1;
+    const int item_id = W.queue ? W.queue[qpos] : (int)qpos;
+    const unsigned* f = ctrl + kCtrlHeads + item_id;
+    while (ld_acquire_u32(f) != 0u) __nanosleep(100);
+    __syncwarp();
+    return item_id;
+}
+
+// Publish item_id as finished: every lane's frame reductions are performed (fence) before any successor's counter moves
+// (warp barrier, then release reductions on the counters)
+__device__ __forceinline__ void queue_done(const QueueParam& W, unsigned* ctrl, int item_id, int lane)
+{
+    __threadfence();
+    __syncwarp();
+    unsigned* const pend = ctrl + kCtrlHeads;
+    const int s1 = W.succ_off[item_id + 1];
+    for (int d = W.succ_off[item_id] + lane; d < s1; d += 32) red_release_dec_u32(pend + W.succ_idx[d]);
+}
+
 template <int NPT>
 __global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB : 1)
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
-                     const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q,
+                     const Strip* __restrict__ strips, const Item* __restrict__ items, QueueParam W, MomentParam Q,
                      double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int item_id = blockIdx.x * kMomWarps + warp;
-    if (item_id >= n_items) return;
     if (frames) {                                             // batch render (e2e_render_frames): blockIdx.y = frame,
-        frame = frames[blockIdx.y];                           // same geometry, its own weights and target
+        frame = frames[blockIdx.y];                           // same geometry, its own weights, target and control block
         ws += (long long)blockIdx.y * w_stride;
     }
     MomentWarpSmem<NPT>& S = reinterpret_cast<MomentWarpSmem<NPT>*>(smem_raw)[warp];
-    const Item it = items[item_id];
-    const Strip st = strips[it.strip];
     const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
     constexpr int NP = 8 * NPT;
+    const double ywin = 1.0 / (double)Q.nyb;
+
+    const int item_id = queue_take(W, W.ctrl + (frames ? (long long)blockIdx.y * W.ctrl_stride : 0), lane);
+    if (item_id < 0) return;
+    const Item it = items[item_id];
+    const Strip st = strips[it.strip];
 
     long long k = (long long)it.chunk0 * 32;
     long long kend = k + (long long)it.nchunks * 32;
@@ -83,7 +145,6 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
     bool have = false;
     int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
     double cYc = 0.0;                                          // its centre
-    const double ywin = 1.0 / (double)Q.nyb;
 
     // steps 2 + 3 + a5 for the open cell
     auto flush = [&]() {
@@ -237,6 +298,7 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         k += nb;
     }
     if (have) flush();
+    queue_done(W, W.ctrl + (frames ? (long long)blockIdx.y * W.ctrl_stride : 0), item_id, lane);
 }
 
 }  // namespace e2e

@@ -722,3 +722,60 @@ def test_rv_sweep_photocenter_linear_in_velocity(B):
     B.e2e_apply_detector(d_in, d_out, s10.nx, s10.ny, det)
     assert np.array_equal(d_out.cpu().numpy(), oracle.detector(frames[-1], det))
     assert 3e4 < frames[-1].max() < 6e4
+
+
+# ------------------------------------------------------------------------------------------ schedule invariants
+def _assert_plan_ok(B, scene, label):
+    r = B.Renderer(scene)
+    try:
+        c = B.e2e_plan_check(r.fmt, r.psf)
+    finally:
+        r.close()
+    assert c["claimed_px"] > 0 and c["n_items"] > 0, (label, c)
+    for k in ("phase_conflicts", "queue_conflicts", "device_band_conflicts", "host_band_conflicts", "host_rows_not_final"):
+        assert c[k] == 0, (label, k, c)
+    return c
+
+
+def test_schedule_invariants_small_scenes(B):
+    """the frame is accumulated with L2 reductions, so its bits rest on the host schedule: no two items of a
+    phase launch share a pixel, every pair of items that shares a pixel is ordered by a dependency edge of the persistent
+    launch, row bands share no pixel.  e2e_plan_check stamps every footprint box into an owner frame on the device and
+    counts violations: steep multi-fiber traces, overlapping orders, a reversed trace, sparse sampling, a tabulated PSF"""
+    s = small_tiny(spp=8.0, lam=(5005.0, 5045.0))
+    s.coef_y = np.array([128.0, 600.0, 0.0, 0.0])                    # steep: dy/dx = 0.6
+    s.fiber_dx = np.array([0.0, 0.3, -0.2, 0.1]); s.fiber_dy = np.array([-7.0, -2.0, 3.0, 9.0])
+    s.spectra = [s.spectra[0]] * 4
+    c = _assert_plan_ok(B, s, "steep 4-fiber")
+    assert c["n_dependencies"] > 0
+    s = small_tiny(spp=40.0, lam=(5000.0, 5050.0))
+    s.coef_x = np.array([1024.0, -1000.0, 1.0, 0.0])                 # x decreasing with lambda
+    _assert_plan_ok(B, s, "reversed")
+    _assert_plan_ok(B, small_tiny(spp=0.4, lam=(5005.0, 5045.0)), "sparse")
+    _assert_plan_ok(B, W.tiny(), "tiny")
+    _assert_plan_ok(B, small_field_scene(gx=3, gy=2), "tabulated")
+    s = W.espresso_like(n_obj_lines=100, table_dlam=0.02).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    c = _assert_plan_ok(B, s, "espresso 7 orders")
+    assert c["n_host_bands"] >= 2
+
+
+@pytest.mark.parametrize("which", ["espresso_like", "hires_like", "field_psf"])
+def test_schedule_invariants_full_size(B, which):
+    """the same at BASELINE.json's full sizes (the plans bench.py's launches use), plus three renders that must agree bit for
+    bit (the espresso_gpu fixture does that for espresso_like)"""
+    if which == "espresso_like":
+        s = W.espresso_like(n_obj_lines=100, table_dlam=0.02)
+    elif which == "hires_like":
+        s = W.hires_like(n_lines=200, table_dlam=0.02)
+    else:
+        s = W.field_psf(base=W.espresso_like(n_obj_lines=100, table_dlam=0.02))
+    c = _assert_plan_ok(B, s, which)
+    assert c["n_dependencies"] > c["n_items"] // 2
+    if which != "espresso_like":
+        r = B.Renderer(s)
+        try:
+            a = r.render().clone()
+            for _ in range(2):
+                assert r.torch.equal(r.render(), a)
+        finally:
+            r.close()

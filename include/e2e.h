@@ -273,6 +273,8 @@ E2E_API int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf
 /* Algorithmic work of the a4+a5 method e2e_render_frame uses for this pair (DESIGN.md 5.3 "Roofline"), without the
  * padding of the DMMA tiles: fp64 fused multiply-adds per footprint cell, T (8 (P+1) w + 8 w h) with w x h the nominal
  * footprint (2 H + 1 pixels per axis, G9), P the x-phase degree, T the chord terms, and per sample, 8 (P+1) (moment update).
+ * Tabulated PSF (cell-deposit kernel): per cell nodes x 2 y-offset rows x (os+1) x-offsets x (npix+1)^2 window
+ * pixels, per sample 4 x nodes deposit products (nodes = field nodes blended per sample: 1, 2 or 4).
  * 0 for the kernels that do not work cell by cell.  Output pointers may be NULL. */
 E2E_API int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, double* fma_per_cell,
                                        double* fma_per_sample);

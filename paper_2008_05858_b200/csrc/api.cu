@@ -39,7 +39,14 @@ int measure_fp64_peak(int repeats, double* burst, double* sustained);
 constexpr double kMomentMinSpp = 8.0;
 constexpr long long kSmallFrameItems = 4736;   // 2 x (148 SMs x 16 resident warps): below this a K = 2 schedule leaves the GPU idle
 constexpr int kDeviceParts = 2;        // row bands e2e_render_frame renders concurrently (they share no pixel)
-constexpr int kHostBands = 8;          // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
+#ifndef E2E_HOST_BANDS
+#define E2E_HOST_BANDS 8
+#endif
+#ifndef E2E_HOST_BANDS16
+#define E2E_HOST_BANDS16 3
+#endif
+constexpr int kHostBands = E2E_HOST_BANDS;       // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
+constexpr int kHostBands16 = E2E_HOST_BANDS16;   // the same for the uint16 output: the copy is 4x shorter, fewer and larger bands pay
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -137,7 +144,7 @@ e2e_plan::~e2e_plan()
     if (d_succ_off) cudaFree(d_succ_off);
     if (d_succ_idx) cudaFree(d_succ_idx);
     if (d_ctrl_init) cudaFree(d_ctrl_init);
-    for (BandPart* bp : {&host, &halves}) {
+    for (BandPart* bp : {&host, &halves, &host16}) {
         if (bp->d_items) cudaFree(bp->d_items);
         if (bp->d_strips) cudaFree(bp->d_strips);
         if (bp->d_queue) cudaFree(bp->d_queue);
@@ -852,6 +859,8 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         if (rc) return rc;
         rc = build_part(kDeviceParts, false, pl->halves);
         if (rc) return rc;
+        rc = build_part(std::min(kHostBands16, want), false, pl->host16);
+        if (rc) return rc;
     }
     *out = pl.get();
     F->plans.push_back(std::move(pl));
@@ -1307,7 +1316,8 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
         return E2E_OK;
     };
     HostPipe* hp = host_pipe();
-    if (pl->host.n_bands <= 1 || !hp) {
+    const e2e_plan::BandPart& part = out16 ? pl->host16 : pl->host;   // the 2-byte output travels 4x faster: fewer, larger bands
+    if (part.n_bands <= 1 || !hp) {
         // one pass: render, detector, copy
         rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
         if (rc) return rc;
@@ -1325,7 +1335,7 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     double* d_y = (double*)(p + per);
     double* d_w = (double*)(p + 2 * per);
     unsigned* d_ctrl = (unsigned*)(p + 3 * per);
-    if (pl->host.n_bands > kCtrlHeads) return fail(E2E_ERR_UNSUPPORTED, w + ": too many row bands");
+    if (part.n_bands > kCtrlHeads) return fail(E2E_ERR_UNSUPPORTED, w + ": too many row bands");
     std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
     E2E_CUDA(cudaMemsetAsync(d_frame, 0, npix * 8, stream));
     E2E_CUDA(ctrl_reset(pl, d_ctrl, stream));
@@ -1335,18 +1345,18 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     // from here on work is forked: every exit goes through the join below (errors are remembered, not returned at once)
     cudaError_t ce = cudaSuccess;
     int row0 = 0;
-    for (int b = 0; b < pl->host.n_bands && !rc && ce == cudaSuccess; ++b) {
+    for (int b = 0; b < part.n_bands && !rc && ce == cudaSuccess; ++b) {
         cudaStream_t cs = (b & 1) ? hp->aux : stream;
-        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &pl->host, b);   // a1-a3 of this band's strips only
+        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &part, b);   // a1-a3 of this band's strips only
         if (rc) break;
         QueueSel qs;
         qs.ctrl = d_ctrl; qs.head = b;
-        qs.queue = pl->host.d_queue + pl->host.queue_off[b];
-        qs.n = pl->host.queue_off[b + 1] - pl->host.queue_off[b];
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, qs, pl->host.d_items,
-                           pl->host.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        qs.queue = part.d_queue + part.queue_off[b];
+        qs.n = part.queue_off[b + 1] - part.queue_off[b];
+        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, qs, part.d_items,
+                           part.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
         if (rc) break;
-        const int row1 = std::max(row0, pl->host.fin_row[b]);
+        const int row1 = std::max(row0, part.fin_row[b]);
         if (row1 > row0) {
             rc = detector_rows(row0, row1, cs);
             if (rc) break;
@@ -1498,19 +1508,23 @@ int e2e_plan_check(const e2e_format_t* fmt, const e2e_psf_t* psf, e2e_plan_check
         out->claimed_px = (int64_t)h.claimed;
         E2E_PC(reset(true));
         E2E_PC(ctrl_reset(pl, d_ctrl, nullptr));
-        for (int b = 0; b < pl->host.n_bands && b < kCtrlHeads; ++b) {
-            W.queue = pl->host.d_queue + pl->host.queue_off[b];
-            W.n = pl->host.queue_off[b + 1] - pl->host.queue_off[b];
-            W.head = b;
-            stamp(pl->d_items, W.n, 2, 0, 0, W);
+        for (const e2e_plan::BandPart* part : {&pl->host, &pl->host16}) {
+            E2E_PC(reset(true));
+            E2E_PC(ctrl_reset(pl, d_ctrl, nullptr));
+            for (int b = 0; b < part->n_bands && b < kCtrlHeads; ++b) {
+                W.queue = part->d_queue + part->queue_off[b];
+                W.n = part->queue_off[b + 1] - part->queue_off[b];
+                W.head = b;
+                stamp(pl->d_items, W.n, 2, 0, 0, W);
+            }
+            E2E_PC(fetch());
+            out->queue_conflicts += (int64_t)h.conflicts;
+            if ((int64_t)h.claimed != out->claimed_px) out->queue_conflicts += 1;  // the band queues must cover the same pixels
         }
-        E2E_PC(fetch());
-        out->queue_conflicts += (int64_t)h.conflicts;
-        if ((int64_t)h.claimed != out->claimed_px) out->queue_conflicts += 1;      // the band queues must cover the same pixels
     }
     // (3) row bands: no pixel in two bands; no row written after it was declared final
-    for (int which = 0; which < 2; ++which) {
-        const e2e_plan::BandPart& part = which == 0 ? pl->halves : pl->host;
+    for (int which = 0; which < 3; ++which) {
+        const e2e_plan::BandPart& part = which == 0 ? pl->halves : which == 1 ? pl->host : pl->host16;
         const int np1 = pl->n_phases_all + 1;
         E2E_PC(reset(true));
         for (int b = 0; b < part.n_bands; ++b) {
@@ -1519,8 +1533,8 @@ int e2e_plan_check(const e2e_format_t* fmt, const e2e_psf_t* psf, e2e_plan_check
         }
         E2E_PC(fetch());
         if (which == 0) out->device_band_conflicts = (int64_t)h.conflicts;
-        else { out->host_band_conflicts = (int64_t)h.conflicts; out->host_rows_not_final = (int64_t)h.early_rows; }
-        if ((int64_t)h.claimed != out->claimed_px) out->host_band_conflicts += which == 1, out->device_band_conflicts += which == 0;
+        else { out->host_band_conflicts += (int64_t)h.conflicts; out->host_rows_not_final += (int64_t)h.early_rows; }
+        if ((int64_t)h.claimed != out->claimed_px) out->host_band_conflicts += which >= 1, out->device_band_conflicts += which == 0;
     }
 #undef E2E_PC
     return done(E2E_OK);
@@ -1564,6 +1578,14 @@ int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, do
         const double np1 = (double)psf->moment_degree + 1.0;
         pc = (double)psf->mom.T * (8.0 * np1 * w + 8.0 * w * h);
         ps = 8.0 * np1;
+    } else if (choose_tabcell(psf)) {
+        // cell-deposit method (render_tabcell.cuh): one FMA per (field node, y-offset row, x-offset, window pixel) and cell --
+        // the samples of a cell sweep all os + 1 x-offsets and, on a trace flatter than 1/os px per px, 2 y-offset rows --
+        // and 4 deposit products per field node and sample
+        const TabParam& T = psf->tab;
+        const double nodes = (T.gx > 1 ? 2.0 : 1.0) * (T.gy > 1 ? 2.0 : 1.0);
+        pc = nodes * 2.0 * (double)(T.os + 1) * (double)(T.npix + 1) * (double)(T.npix + 1);
+        ps = 4.0 * nodes;
     }
     if (fma_cell) *fma_cell = pc;
     if (fma_sample) *fma_sample = ps;

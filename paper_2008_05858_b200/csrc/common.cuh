@@ -196,7 +196,7 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
         std::vector<int> queue_off;    // [n_bands + 1] into d_queue: the band's item ids in queue order (persistent launch)
         int* d_queue = nullptr;
     };
-    BandPart host, halves;
+    BandPart host, halves, host16;     // host16: fewer, equal bands for the host path's uint16 output (short copies)
     int n_phases_all = 0;          // phases before empty ones were dropped (colour x class)
     ~e2e_plan();
 };

@@ -132,6 +132,25 @@ def test_render_psf_variants(B, psf_kw):
     assert_frame_parity(G, O, str(psf_kw))
 
 
+def test_render_narrow_sigma_reaches_the_direct_kernel(B):
+    """sigma = 0.2 px: no polynomial degree up to 24 reproduces the pixel-phase factors to 1e-17, so e2e_psf_create builds no
+    tables and e2e_render_frame launches render_analytic_kernel (direct erfc / Psi evaluation) -- the kernel name is
+    asserted, so this test really covers that fallback.  Dense and sparse sampling, pure gaussian and with a fiber image"""
+    for spp, kw in ((6.0, dict(fiber_dx_px=0.0, fiber_dy_px=0.0, sigma_x=0.2, sigma_y=0.25)),
+                    (0.7, dict(fiber_dx_px=2.0, fiber_dy_px=2.0, sigma_x=0.22, sigma_y=0.22))):
+        s = with_psf(small_tiny(spp=spp, lam=(5010.0, 5012.0)), **kw)
+        r = B.Renderer(s)
+        try:
+            assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"] == "render_analytic_kernel"
+            G = r.render().cpu().numpy()
+        finally:
+            r.close()
+        O = oracle.render(s)
+        assert O.max() > 0
+        assert_frame_parity(G, O, f"direct kernel {kw}")
+        assert abs(G.sum() / oracle.total_weight(s) - 1.0) < 1e-12
+
+
 def test_render_single_sample_is_the_psf_itself(B):
     d = W.single_line_scene(x_pos=100.3173, y_pos=37.8641)
     G = gpu_render(B, d)
@@ -456,6 +475,52 @@ def test_render_frame_host_banded_pipeline(B):
         again = torch.empty_like(out)
         B.e2e_render_frame_host(r.fmt, r.psf, desc, again.data_ptr(), ws, det=det)
         assert torch.equal(again, out)
+    finally:
+        r.close()
+
+
+def test_render_frame_host_adu16_raw_frame(B):
+    """e2e_render_frame_host_adu16 / _ex: the host path with the full detector stage (PRNU + dark maps, full well, cross-talk,
+    ADC) delivering uint16 counts.  Bit-exact against the oracle's detector stage applied to the host path's own noise-free
+    frame, band by band (the stream is keyed by the pixel's index in the whole frame)"""
+    import torch
+    s = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    for sp in s.spectra:
+        sp.scale = sp.scale * 400.0                                   # bright enough to reach the well in line cores
+    rng = np.random.default_rng(12)
+    prnu = rng.normal(1.0, 0.02, (s.ny, s.nx))
+    dark = rng.uniform(0.0, 2.0, (s.ny, s.nx))
+    X = rng.uniform(0.0, 5e-4, (16, 16))
+    det = W.Detector(gain=1.0, dark_e=0.5, ron_e=3.0, bias=1000.0, seed=777)
+    r = B.Renderer(s)
+    try:
+        host_tabs = [np.ascontiguousarray(sp.flux, dtype=np.float64) for sp in s.spectra]
+        desc = B.spectra_array(s.spectra, [t.ctypes.data for t in host_tabs])
+        ws = torch.empty(B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc), dtype=torch.uint8, device="cuda")
+        clean = torch.empty((s.ny, s.nx), dtype=torch.float64).pin_memory()
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, clean.data_ptr(), ws)
+        H = clean.numpy().copy()
+        assert H.max() > 1e3
+        d_pr, d_dk = torch.from_numpy(prnu).cuda(), torch.from_numpy(dark).cuda()
+        kw = dict(full_well_e=2.0e4, e_per_adu=1.1, adu_max=65535.0)
+        okw = dict(full_well=2.0e4, e_per_adu=1.1, adu_max=65535.0)
+        for xt in (None, X):
+            d_ex, keep = B.detector_ex_desc(det, d_pr, d_dk, xtalk=xt, **kw)
+            out16 = torch.zeros((s.ny, s.nx), dtype=torch.uint16).pin_memory()
+            B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, out16.data_ptr(), ws, d_ex, adu16=True)
+            want = oracle.detector_adu16(H, det, prnu=prnu, dark=dark, xtalk=xt, **okw)
+            assert np.array_equal(out16.numpy(), want), "uint16 host path" + (" with cross-talk" if xt is not None else "")
+            out64 = torch.zeros((s.ny, s.nx), dtype=torch.float64).pin_memory()
+            B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, out64.data_ptr(), ws, d_ex)
+            assert np.array_equal(out64.numpy(), want.astype(np.float64))
+        assert want.max() > 1.9e4 / 1.1 and want.min() >= 900
+        # reproducible call to call, and refused without an ADC
+        again = torch.zeros_like(out16)
+        B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, again.data_ptr(), ws, d_ex, adu16=True)
+        assert np.array_equal(again.numpy(), out16.numpy())
+        bad, _ = B.detector_ex_desc(det)
+        with pytest.raises(B.E2EError):
+            B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, again.data_ptr(), ws, bad, adu16=True)
     finally:
         r.close()
 

@@ -46,7 +46,8 @@ class _Psf(C.Structure):
     _fields_ = [("kind", C.c_int32), ("fiber_dx_px", C.c_double), ("fiber_dy_px", C.c_double),
                 ("sigma_x", C.c_double), ("sigma_y", C.c_double), ("support_nsigma", C.c_double),
                 ("n_nodes", C.c_int32), ("tab_npix", C.c_int32), ("tab_os", C.c_int32),
-                ("tab_gx", C.c_int32), ("tab_gy", C.c_int32), ("tab", C.c_void_p)]
+                ("tab_gx", C.c_int32), ("tab_gy", C.c_int32), ("tab", C.c_void_p),
+                ("an_gx", C.c_int32), ("an_gy", C.c_int32), ("an_sigma_x", C.c_void_p), ("an_sigma_y", C.c_void_p)]
 
 
 class _Spectrum(C.Structure):
@@ -75,6 +76,8 @@ def lib():
         L.orc_psf_pixel.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.orc_psf_tab_pixel.restype = C.c_double
         L.orc_psf_tab_pixel.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32]
+        L.orc_psf_map_pixel.restype = C.c_double
+        L.orc_psf_map_pixel.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32]
         L.orc_footprint.restype = None
         L.orc_footprint.argtypes = [C.c_void_p, C.c_double, C.c_double] + [C.c_void_p] * 4
         L.orc_render.restype = C.c_int64
@@ -151,6 +154,12 @@ class Handles:
         p.n_nodes = 32                       # the oracle's own quadrature order, not the CUDA path's
         p.tab_npix, p.tab_os, p.tab_gx, p.tab_gy = q.tab_npix, q.tab_os, q.tab_gx, q.tab_gy
         p.tab = k(q.tab) if q.tab is not None else None
+        if getattr(q, "an_sigma_x", None) is not None:      # G21 analytic PSF map
+            p.an_gx, p.an_gy = int(q.an_gx), int(q.an_gy)
+            p.an_sigma_x, p.an_sigma_y = k(q.an_sigma_x), k(q.an_sigma_y)
+            assert np.asarray(q.an_sigma_x).size == p.an_gx * p.an_gy == np.asarray(q.an_sigma_y).size
+        else:
+            p.an_gx, p.an_gy, p.an_sigma_x, p.an_sigma_y = 0, 0, None, None
         self.psf = p
 
         arr = (_Spectrum * s.n_fibers)()
@@ -186,12 +195,19 @@ def psf_pixel(psf, u: float, v: float, n_nodes: int = 32) -> float:
     p.kind = 0
     p.fiber_dx_px, p.fiber_dy_px = psf.fiber_dx_px, psf.fiber_dy_px
     p.sigma_x, p.sigma_y, p.support_nsigma, p.n_nodes = psf.sigma_x, psf.sigma_y, psf.support_nsigma, n_nodes
+    p.an_gx, p.an_gy, p.an_sigma_x, p.an_sigma_y = 0, 0, None, None
     return float(lib().orc_psf_pixel(C.addressof(p), u, v))
 
 
 def psf_tab_pixel(scene, xk: float, yk: float, i: int, j: int) -> float:
     h = Handles(scene)
     return float(lib().orc_psf_tab_pixel(C.addressof(h.psf), scene.nx, scene.ny, xk, yk, i, j))
+
+
+def psf_map_pixel(scene, xk: float, yk: float, i: int, j: int) -> float:
+    """pixel (i, j) of the blended PSF of a sample at (xk, yk) for an analytic PSF map (G21)"""
+    h = Handles(scene)
+    return float(lib().orc_psf_map_pixel(C.addressof(h.psf), scene.nx, scene.ny, xk, yk, i, j))
 
 
 def footprint(scene, xk: float, yk: float):

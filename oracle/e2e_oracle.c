@@ -25,7 +25,9 @@
  * definition, P2 pure-gaussian closed form, P3 flux conservation, P4/P5 photocenter, P6 second
  * moment, P7 symmetries, P8 linearity, P9 integer translation, P10 tabulated == analytic limit and
  * == summed-area form, P11 the paper's own 0.1-px sub-pixel scheme, blaze closed forms,
- * Philox known-answer vectors and noise moments (P12).  Nothing here is "parity unpinned".
+ * Philox known-answer vectors and noise moments (P12); G21 PSF map: reduction to the constant PSF, mixture of the pinned
+ * constant-sigma pixels with independently computed bilinear weights, mixture second moments, box from the largest node
+ * sigma, clamping.  Nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -61,6 +63,10 @@ typedef struct {
     int32_t n_nodes;                         /* Q of O4 (oracle: 32) */
     int32_t tab_npix, tab_os, tab_gx, tab_gy;
     const double *tab;                       /* [gy][gx][npix*os][npix*os] */
+    /* G21 ("PSF ... for each wavelength"): analytic PSF MAP.  an_gx * an_gy > 0: the optical PSF was evaluated at the
+     * nodes of an an_gx x an_gy grid over the detector (node positions as T3) and sigma_x, sigma_y above are ignored */
+    int32_t an_gx, an_gy;
+    const double *an_sigma_x, *an_sigma_y;   /* [an_gy][an_gx] */
 } orc_psf_t;
 
 typedef struct {
@@ -217,14 +223,24 @@ double orc_psf_pixel(const orc_psf_t *p, double u, double v) { return (double)or
 
 /* G9: footprint box.  Half-widths H = a + t*sigma (analytic) or npix/2 (tabulated); hb = H + 1/2;
  * columns ceil(x - hb) .. floor(x + hb)  (all pixels that touch [x-H, x+H]); same for rows. */
+static int psf_is_map(const orc_psf_t *p) { return p->kind == 0 && p->an_gx > 0 && p->an_gy > 0 && p->an_sigma_x && p->an_sigma_y; }
+
 void orc_support(const orc_psf_t *p, double *hbx, double *hby)
 {
     if (p->kind == 1) {
         *hbx = 0.5 * (double)p->tab_npix + 0.5;
         *hby = *hbx;
     } else {
-        double Hx = 0.5 * p->fiber_dx_px + p->support_nsigma * p->sigma_x;
-        double Hy = 0.5 * p->fiber_dy_px + p->support_nsigma * p->sigma_y;
+        double sx = p->sigma_x, sy = p->sigma_y;
+        if (psf_is_map(p)) {                 /* G21: ONE box for the whole frame, from the largest node sigma per axis */
+            sx = p->an_sigma_x[0]; sy = p->an_sigma_y[0];
+            for (int c = 1; c < p->an_gx * p->an_gy; ++c) {
+                if (p->an_sigma_x[c] > sx) sx = p->an_sigma_x[c];
+                if (p->an_sigma_y[c] > sy) sy = p->an_sigma_y[c];
+            }
+        }
+        double Hx = 0.5 * p->fiber_dx_px + p->support_nsigma * sx;
+        double Hy = 0.5 * p->fiber_dy_px + p->support_nsigma * sy;
         *hbx = Hx + 0.5;
         *hby = Hy + 0.5;
     }
@@ -242,27 +258,62 @@ void orc_footprint(const orc_psf_t *p, double xk, double yk, int32_t *ilo, int32
  * ------------------------------------------------------------------------------------------ */
 /* T3: bilinear blend weights of the 4 surrounding node kernels at detector position (xk, yk);
  * nodes at X_g = g (nx-1)/(gx-1), Y_h = h (ny-1)/(gy-1); weights clamped outside the grid */
-static void field_weights(const orc_psf_t *p, int nx, int ny, double xk, double yk,
-                          int *g0, int *h0, long double *fx, long double *fy)
+static void grid_weights(int gx, int gy, int nx, int ny, double xk, double yk,
+                         int *g0, int *h0, long double *fx, long double *fy)
 {
     long double tx = 0.0L, ty = 0.0L;
     *g0 = 0; *h0 = 0;
-    if (p->tab_gx > 1) {
-        tx = (long double)xk * (long double)(p->tab_gx - 1) / (long double)(nx - 1);
+    if (gx > 1) {
+        tx = (long double)xk * (long double)(gx - 1) / (long double)(nx - 1);
         if (tx < 0.0L) tx = 0.0L;
-        if (tx > (long double)(p->tab_gx - 1)) tx = (long double)(p->tab_gx - 1);
-        *g0 = (int)floorl(tx); if (*g0 > p->tab_gx - 2) *g0 = p->tab_gx - 2;
+        if (tx > (long double)(gx - 1)) tx = (long double)(gx - 1);
+        *g0 = (int)floorl(tx); if (*g0 > gx - 2) *g0 = gx - 2;
         tx -= (long double)*g0;
     }
-    if (p->tab_gy > 1) {
-        ty = (long double)yk * (long double)(p->tab_gy - 1) / (long double)(ny - 1);
+    if (gy > 1) {
+        ty = (long double)yk * (long double)(gy - 1) / (long double)(ny - 1);
         if (ty < 0.0L) ty = 0.0L;
-        if (ty > (long double)(p->tab_gy - 1)) ty = (long double)(p->tab_gy - 1);
-        *h0 = (int)floorl(ty); if (*h0 > p->tab_gy - 2) *h0 = p->tab_gy - 2;
+        if (ty > (long double)(gy - 1)) ty = (long double)(gy - 1);
+        *h0 = (int)floorl(ty); if (*h0 > gy - 2) *h0 = gy - 2;
         ty -= (long double)*h0;
     }
     *fx = tx; *fy = ty;
 }
+static void field_weights(const orc_psf_t *p, int nx, int ny, double xk, double yk,
+                          int *g0, int *h0, long double *fx, long double *fy)
+{
+    grid_weights(p->tab_gx, p->tab_gy, nx, ny, xk, yk, g0, h0, fx, fy);
+}
+
+/* G21: the 4 nodes of the analytic PSF map around (xk, yk) and their bilinear weights (same node positions and clamping
+ * as T3); node[c] indexes an_sigma_x / an_sigma_y, c = 2 (row) + (column) */
+static void map_nodes(const orc_psf_t *p, int nx, int ny, double xk, double yk, int node[4], long double beta[4])
+{
+    int g0, h0; long double fx, fy;
+    grid_weights(p->an_gx, p->an_gy, nx, ny, xk, yk, &g0, &h0, &fx, &fy);
+    int g1 = p->an_gx > 1 ? g0 + 1 : g0, h1 = p->an_gy > 1 ? h0 + 1 : h0;
+    node[0] = h0 * p->an_gx + g0; node[1] = h0 * p->an_gx + g1; node[2] = h1 * p->an_gx + g0; node[3] = h1 * p->an_gx + g1;
+    beta[0] = (1.0L - fy) * (1.0L - fx); beta[1] = (1.0L - fy) * fx; beta[2] = fy * (1.0L - fx); beta[3] = fy * fx;
+}
+
+/* G21: pixel integral of the blended PSF of a sample at (xk, yk): sum over the 4 surrounding nodes of
+ * beta_c * P(u, v; sigma_x[c], sigma_y[c]) -- the PSF itself is interpolated between the field points where it was evaluated */
+long double orc_psf_map_pixel_l(const orc_psf_t *p, int nx, int ny, double xk, double yk, int i, int j)
+{
+    int node[4]; long double beta[4];
+    map_nodes(p, nx, ny, xk, yk, node, beta);
+    long double sum = 0.0L;
+    for (int c = 0; c < 4; ++c) {
+        if (beta[c] == 0.0L) continue;
+        orc_psf_t q = *p;
+        q.an_gx = q.an_gy = 0;
+        q.sigma_x = p->an_sigma_x[node[c]]; q.sigma_y = p->an_sigma_y[node[c]];
+        sum += beta[c] * orc_psf_pixel_l(&q, (long double)i - (long double)xk, (long double)j - (long double)yk);
+    }
+    return sum;
+}
+double orc_psf_map_pixel(const orc_psf_t *p, int32_t nx, int32_t ny, double xk, double yk, int32_t i, int32_t j)
+{ return (double)orc_psf_map_pixel_l(p, nx, ny, xk, yk, i, j); }
 
 static long double overlap(long double a0, long double a1, long double b0, long double b1)
 {
@@ -324,6 +375,16 @@ static void scatter_sample(const orc_format_t *f, const orc_psf_t *p, double xk,
             for (int i = ilo; i <= ihi; ++i) {
                 if (i < 0 || i >= f->nx || i < bi0 || i >= bi0 + bw) continue;
                 box[(size_t)(j - bj0) * bw + (i - bi0)] += (long double)wk * orc_psf_tab_pixel_l(p, f->nx, f->ny, xk, yk, i, j);
+            }
+        }
+        return;
+    }
+    if (psf_is_map(p)) {                     /* G21: blend of the 4 surrounding node PSFs, the box is the common one */
+        for (int j = jlo; j <= jhi; ++j) {
+            if (j < 0 || j >= f->ny || j < bj0 || j >= bj0 + bh) continue;
+            for (int i = ilo; i <= ihi; ++i) {
+                if (i < 0 || i >= f->nx || i < bi0 || i >= bi0 + bw) continue;
+                box[(size_t)(j - bj0) * bw + (i - bi0)] += (long double)wk * orc_psf_map_pixel_l(p, f->nx, f->ny, xk, yk, i, j);
             }
         }
         return;

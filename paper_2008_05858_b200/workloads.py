@@ -45,6 +45,12 @@ class Psf:
     tab_gx: int = 0
     tab_gy: int = 0
     tab: Optional[np.ndarray] = None   # float64 [gy][gx][npix*os][npix*os]
+    # analytic PSF map (G21; "PSF ... for each wavelength"): sigma_x, sigma_y at the nodes of an
+    # an_gx x an_gy grid over the detector; None = one PSF for the whole frame (sigma_x, sigma_y above)
+    an_gx: int = 0
+    an_gy: int = 0
+    an_sigma_x: Optional[np.ndarray] = None   # float64 [an_gy][an_gx]
+    an_sigma_y: Optional[np.ndarray] = None
 
 
 @dataclass
@@ -348,6 +354,26 @@ def field_psf(seed: int = 4004, samples_per_px: float = 32.0, base: Optional[Sce
 # --------------------------------------------------------------------------------------
 # configs[4]  precision / RV sweep
 # --------------------------------------------------------------------------------------
+def psf_map(base: Scene, gx: int = 3, gy: int = 3, seed: int = 6006, growth: float = 0.25, jitter: float = 0.03) -> Scene:
+    """Analytic PSF map (G21; "evaluate the optical PSF ... for each wavelength"): the base scene with
+    sigma_x, sigma_y given at the nodes of a gx x gy grid over the detector.  Input recipe only: the image quality of a camera
+    degrades towards the corners of the field, so sigma grows with the squared normalised distance from the detector centre
+    (by `growth` at the corners, differently in x and y) with a few per cent of node-to-node scatter."""
+    rng = np.random.default_rng(seed)
+    s = copy.copy(base)
+    s.name = base.name + "_psf_map"
+    gxs = np.linspace(-1.0, 1.0, gx) if gx > 1 else np.zeros(1)
+    gys = np.linspace(-1.0, 1.0, gy) if gy > 1 else np.zeros(1)
+    X, Y = np.meshgrid(gxs, gys)                                    # [gy][gx]
+    r2 = 0.5 * (X * X + Y * Y)
+    p = copy.copy(base.psf)
+    p.an_gx, p.an_gy = gx, gy
+    p.an_sigma_x = base.psf.sigma_x * (1.0 + growth * (r2 + 0.2 * X)) * (1.0 + jitter * rng.uniform(-1.0, 1.0, (gy, gx)))
+    p.an_sigma_y = base.psf.sigma_y * (1.0 + 0.6 * growth * (r2 - 0.25 * Y)) * (1.0 + jitter * rng.uniform(-1.0, 1.0, (gy, gx)))
+    s.psf = p
+    return s
+
+
 RV_SWEEP_V = (0.0, 0.01, 0.1, 1.0, 10.0)   # m/s
 
 

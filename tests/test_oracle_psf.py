@@ -8,6 +8,7 @@ import pytest
 from scipy import special
 
 import oracle
+from paper_2008_05858_b200 import workloads as W
 from paper_2008_05858_b200.workloads import Psf
 
 GOLD = Path(__file__).parent / "golden"
@@ -134,3 +135,91 @@ def test_p11_papers_subpixel_scheme():
     cx_p = np.sum(papers * i[None, :]) / papers.sum()
     cx_o = np.sum(P * i[None, :]) / P.sum()
     assert abs(cx_p - cx_o) < 1e-11
+
+
+# ------------------------------------------------------------------------------------------ G21: analytic PSF map
+def _map_scene(gx=3, gy=2, nx=200, ny=80, x_pos=100.3173, y_pos=37.8641):
+    d = W.single_line_scene(x_pos=x_pos, y_pos=y_pos, nx=nx, ny=ny)
+    return W.psf_map(d, gx=gx, gy=gy, seed=6)
+
+
+def _bilinear_nodes(gx, gy, nx, ny, x, y):
+    """independent restatement of the node rule (T3 / G21): nodes at g (nx-1)/(gx-1), weights clamped outside"""
+    tx = min(max(x * (gx - 1) / (nx - 1), 0.0), gx - 1.0) if gx > 1 else 0.0
+    ty = min(max(y * (gy - 1) / (ny - 1), 0.0), gy - 1.0) if gy > 1 else 0.0
+    g0 = min(int(np.floor(tx)), max(gx - 2, 0)); h0 = min(int(np.floor(ty)), max(gy - 2, 0))
+    fx, fy = tx - g0, ty - h0
+    g1, h1 = (g0 + 1 if gx > 1 else g0), (h0 + 1 if gy > 1 else h0)
+    return [((h0, g0), (1 - fy) * (1 - fx)), ((h0, g1), (1 - fy) * fx), ((h1, g0), fy * (1 - fx)), ((h1, g1), fy * fx)]
+
+
+def test_g21_map_pixel_is_the_mixture_of_the_pinned_constant_psfs():
+    """G21: the blended PSF = sum over the 4 surrounding nodes of beta_c P(u, v; sigma_c).  Right-hand side: the constant-sigma
+    pixel integral (pinned by P1, P2, P6) per node and bilinear weights restated here in numpy.  Asymmetric maps (sigma_x !=
+    sigma_y, gx != gy): a transposed grid, swapped weights or a swapped axis fails"""
+    import copy
+    for (xp, yp) in [(100.3173, 37.8641), (12.9, 70.2), (199.0, 0.0), (150.0, 79.0), (-3.5, 40.0), (57.25, 95.0)]:
+        d = _map_scene(x_pos=xp, y_pos=yp)
+        q = d.psf
+        nodes = _bilinear_nodes(q.an_gx, q.an_gy, d.nx, d.ny, xp, yp)
+        assert abs(sum(b for _, b in nodes) - 1.0) < 1e-15
+        for (i, j) in [(int(round(xp)), int(round(yp))), (int(round(xp)) + 3, int(round(yp)) - 2), (int(round(xp)) - 6, int(round(yp)) + 1)]:
+            want = 0.0
+            for (h, g), beta in nodes:
+                c = copy.copy(q)
+                c.an_sigma_x = c.an_sigma_y = None
+                c.sigma_x, c.sigma_y = float(q.an_sigma_x[h, g]), float(q.an_sigma_y[h, g])
+                want += beta * oracle.psf_pixel(c, i - xp, j - yp)
+            assert oracle.psf_map_pixel(d, xp, yp, i, j) == pytest.approx(want, rel=2e-15, abs=1e-300)
+
+
+def test_g21_map_with_equal_nodes_is_the_constant_psf():
+    d = W.single_line_scene(x_pos=100.3173, y_pos=37.8641)
+    m = W.psf_map(d, gx=3, gy=3, growth=0.0, jitter=0.0)
+    assert np.all(m.psf.an_sigma_x == d.psf.sigma_x) and np.all(m.psf.an_sigma_y == d.psf.sigma_y)
+    A, Bm = oracle.render(d), oracle.render(m)
+    assert A.max() > 0 and np.allclose(Bm, A, rtol=1e-15, atol=0.0)
+
+
+def test_g21_map_moments_box_and_flux():
+    """per-sample second moments of a mixture = sum beta (sigma^2) + a^2/4 + 1/12 per axis (P6 for every node), the footprint box
+    comes from the LARGEST node sigma (one box for the frame), flux = 1 - tail"""
+    d = _map_scene(gx=3, gy=2)
+    q = d.psf
+    xp, yp = 100.3173, 37.8641
+    fr = oracle.render(d)
+    w = oracle.total_weight(d)
+    P = fr / w
+    assert abs(P.sum() - 1.0) < 2e-13
+    jj, ii = np.mgrid[0:d.ny, 0:d.nx]
+    nodes = _bilinear_nodes(q.an_gx, q.an_gy, d.nx, d.ny, xp, yp)
+    a = 0.5 * q.fiber_dx_px
+    vx = sum(b * q.an_sigma_x[h, g] ** 2 for (h, g), b in nodes) + a * a / 4 + 1 / 12
+    vy = sum(b * q.an_sigma_y[h, g] ** 2 for (h, g), b in nodes) + (0.5 * q.fiber_dy_px) ** 2 / 4 + 1 / 12
+    assert abs((P * (ii - xp) ** 2).sum() - vx) < 1e-9
+    assert abs((P * (jj - yp) ** 2).sum() - vy) < 1e-9
+    assert abs(vx - vy) > 1e-3                                         # the map is asymmetric: an x/y swap would show
+    hbx = 0.5 * q.fiber_dx_px + q.support_nsigma * q.an_sigma_x.max() + 0.5
+    hby = 0.5 * q.fiber_dy_px + q.support_nsigma * q.an_sigma_y.max() + 0.5
+    nz = np.nonzero(fr)
+    assert (nz[1].min(), nz[1].max()) == (int(np.ceil(xp - hbx)), int(np.floor(xp + hbx)))
+    assert (nz[0].min(), nz[0].max()) == (int(np.ceil(yp - hby)), int(np.floor(yp + hby)))
+    assert oracle.footprint(d, xp, yp) == (int(np.ceil(xp - hbx)), int(np.floor(xp + hbx)), int(np.ceil(yp - hby)), int(np.floor(yp + hby)))
+
+
+def test_g21_map_render_is_linear_in_the_node_psfs():
+    """frame(map) = sum_c frame(weights beta_c, constant sigma_c): checked by rendering a multi-sample strip whose samples
+    cross a node boundary, against the per-pixel mixture"""
+    s = W.tiny(samples_per_px=2.0)
+    s.lam_min = np.array([5020.0]); s.lam_max = np.array([5030.0])          # x = 824 .. 1224: crosses the node at x = 1023.5
+    m = W.psf_map(s, gx=3, gy=2, seed=9)
+    fr = oracle.render(m)
+    lam, x, y, w = oracle.samples(m, 0, 0)
+    g0s = {_bilinear_nodes(3, 2, m.nx, m.ny, xx, yy)[0][0][1] for xx, yy in zip(x, y)}
+    assert g0s == {0, 1}
+    rng = np.random.default_rng(0)
+    for _ in range(6):
+        i = int(rng.integers(int(x.min()) + 12, int(x.max()) - 12)); j = int(round(128 + 0.01 * i)) + int(rng.integers(-3, 4))
+        want = sum(wk * oracle.psf_map_pixel(m, xk, yk, i, j) for xk, yk, wk in zip(x, y, w)
+                   if oracle.footprint(m, xk, yk)[0] <= i <= oracle.footprint(m, xk, yk)[1])
+        assert fr[j, i] == pytest.approx(want, rel=1e-13)

@@ -112,6 +112,14 @@ typedef struct {
     int32_t tab_npix, tab_os;       /* kind 1: kernel size in px (e.g. 11) and cells per px (e.g. 8) */
     int32_t tab_gx, tab_gy;         /* kind 1: field grid of kernels across the detector (e.g. 5 x 5), each >= 1 */
     const double* tab;              /* kind 1: [gy][gx][npix*os][npix*os] cell values, every kernel sums to 1 */
+    /* kind 0, analytic PSF MAP ("evaluate the optical PSF ... for each wavelength"; G21): when an_sigma_x and
+     * an_sigma_y are not NULL they hold sigma at the nodes of an an_gx x an_gy grid over the detector (node (g, h) at
+     * x = g (nx-1)/(an_gx-1), y = h (ny-1)/(an_gy-1)) and sigma_x / sigma_y above are ignored: the PSF of a sample is the
+     * bilinear blend, at the sample's position, of the 4 surrounding node PSFs (weights clamped outside the grid); the
+     * footprint box uses the largest node sigma per axis.  At most 64 nodes; rendered by the cell-moment kernel whatever the sampling. */
+    int32_t an_gx, an_gy;
+    const double* an_sigma_x;       /* HOST [an_gy][an_gx] */
+    const double* an_sigma_y;
 } e2e_psf_desc_t;
 
 /* Limits (E2E_ERR_UNSUPPORTED beyond them): footprint (2H+2) <= 96 px per axis; Q <= 64; tab_npix*tab_os <= 256. */

@@ -49,7 +49,8 @@ class PsfDesc(C.Structure):
     _fields_ = [("kind", C.c_int32), ("fiber_dx_px", C.c_double), ("fiber_dy_px", C.c_double),
                 ("sigma_x", C.c_double), ("sigma_y", C.c_double), ("support_nsigma", C.c_double),
                 ("n_nodes", C.c_int32), ("tab_npix", C.c_int32), ("tab_os", C.c_int32), ("tab_gx", C.c_int32),
-                ("tab_gy", C.c_int32), ("tab", C.c_void_p)]
+                ("tab_gy", C.c_int32), ("tab", C.c_void_p), ("an_gx", C.c_int32), ("an_gy", C.c_int32),
+                ("an_sigma_x", C.c_void_p), ("an_sigma_y", C.c_void_p)]
 
 
 class SpectrumDesc(C.Structure):
@@ -237,6 +238,11 @@ class Psf:
         d.tab_npix, d.tab_os, d.tab_gx, d.tab_gy = int(psf.tab_npix), int(psf.tab_os), int(psf.tab_gx), int(psf.tab_gy)
         tab = _host(psf.tab) if psf.tab is not None else None
         d.tab = tab.ctypes.data if tab is not None else None
+        sx = _host(psf.an_sigma_x) if getattr(psf, "an_sigma_x", None) is not None else None
+        sy = _host(psf.an_sigma_y) if getattr(psf, "an_sigma_y", None) is not None else None
+        d.an_gx, d.an_gy = (int(psf.an_gx), int(psf.an_gy)) if sx is not None else (0, 0)
+        d.an_sigma_x = sx.ctypes.data if sx is not None else None
+        d.an_sigma_y = sy.ctypes.data if sy is not None else None
         self.handle = C.c_void_p()
         _check(load().e2e_psf_create(C.byref(self.handle), C.byref(d), int(nx), int(ny)))
 

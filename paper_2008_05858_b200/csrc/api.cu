@@ -375,7 +375,17 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
     memset(&P->mom, 0, sizeof(P->mom));
     P->kind = d->kind; P->nx = nx; P->ny = ny; P->Q = 0;
     if (d->kind == 0) {
-        if (!(d->sigma_x > 0.0) || !(d->sigma_y > 0.0) || !is_fin(d->sigma_x) || !is_fin(d->sigma_y))
+        const bool is_map = d->an_sigma_x != nullptr || d->an_sigma_y != nullptr;
+        int n_map = 1;
+        if (is_map) {
+            if (!d->an_sigma_x || !d->an_sigma_y || d->an_gx < 1 || d->an_gy < 1)
+                return fail(E2E_ERR_INVALID_ARG, "psf_create: bad analytic PSF map description");
+            if ((long long)d->an_gx * d->an_gy > 64) return fail(E2E_ERR_UNSUPPORTED, "psf_create: more than 64 nodes in the analytic PSF map");
+            n_map = d->an_gx * d->an_gy;
+            for (int c = 0; c < n_map; ++c)
+                if (!(d->an_sigma_x[c] > 0.0) || !(d->an_sigma_y[c] > 0.0) || !is_fin(d->an_sigma_x[c]) || !is_fin(d->an_sigma_y[c]))
+                    return fail(E2E_ERR_INVALID_ARG, "psf_create: sigma must be > 0 at every node");
+        } else if (!(d->sigma_x > 0.0) || !(d->sigma_y > 0.0) || !is_fin(d->sigma_x) || !is_fin(d->sigma_y))
             return fail(E2E_ERR_INVALID_ARG, "psf_create: sigma must be > 0");
         if (!(d->fiber_dx_px >= 0.0) || !(d->fiber_dy_px >= 0.0) || !is_fin(d->fiber_dx_px) || !is_fin(d->fiber_dy_px))
             return fail(E2E_ERR_INVALID_ARG, "psf_create: fiber widths must be >= 0");
@@ -384,47 +394,108 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
         if (d->n_nodes > 2 * kMaxTerms) return fail(E2E_ERR_UNSUPPORTED, "psf_create: n_nodes > 64");
         const double t = d->support_nsigma > 0.0 ? d->support_nsigma : 7.5;
         const double a = 0.5 * d->fiber_dx_px, b = 0.5 * d->fiber_dy_px;
-        // G9: H = D/2 + t sigma; footprint = all pixels touching [x - H, x + H]
-        const double Hx = 0.5 * d->fiber_dx_px + t * d->sigma_x, Hy = 0.5 * d->fiber_dy_px + t * d->sigma_y;
+        // G9: H = D/2 + t sigma; footprint = all pixels touching [x - H, x + H].  G21: ONE box from the largest node sigma
+        double sx_box = d->sigma_x, sy_box = d->sigma_y, sx_min = d->sigma_x, sy_min = d->sigma_y;
+        if (is_map) {
+            sx_box = sx_min = d->an_sigma_x[0]; sy_box = sy_min = d->an_sigma_y[0];
+            for (int c = 1; c < n_map; ++c) {
+                sx_box = std::max(sx_box, d->an_sigma_x[c]); sy_box = std::max(sy_box, d->an_sigma_y[c]);
+                sx_min = std::min(sx_min, d->an_sigma_x[c]); sy_min = std::min(sy_min, d->an_sigma_y[c]);
+            }
+        }
+        const double Hx = 0.5 * d->fiber_dx_px + t * sx_box, Hy = 0.5 * d->fiber_dy_px + t * sy_box;
         P->hbx = Hx + 0.5; P->hby = Hy + 0.5;
         if (2.0 * P->hbx + 1.0 > 96.0 || 2.0 * P->hby + 1.0 > 96.0)
             return fail(E2E_ERR_UNSUPPORTED, "psf_create: footprint larger than 96 px");
-        AnalyticParam& A = P->an;
-        A.inv_sx = 1.0 / d->sigma_x; A.inv_sy = 1.0 / d->sigma_y;
-        A.hbx = P->hbx; A.hby = P->hby;
-        A.by_gauss = !(b > 0.0);
-        A.paired = 0;
-        if (!(a > 0.0) && !(b > 0.0)) {           // P2: pure gaussian, one term
-            P->Q = 1; A.n_terms = 1; A.s[0] = 0.0; A.cs[0] = 0.0; A.wq[0] = 1.0; A.g[0] = 1.0;
-        } else {
-            const int Q = d->n_nodes > 0 ? d->n_nodes : auto_nodes(a, b, d->sigma_x, d->sigma_y);
-            P->Q = Q;
+        // chord terms of one (sigma_x, sigma_y): nodes q and Q+1-q share |s|, c and the weight -> one term with
+        // F(d) = Phi(d - s) + Phi(d + s).  Q = the caller's, else chosen for the narrowest sigma of the map
+        const bool pure_gauss = !(a > 0.0) && !(b > 0.0);
+        const int Qn = pure_gauss ? 1 : (d->n_nodes > 0 ? d->n_nodes : auto_nodes(a, b, sx_min, sy_min));
+        P->Q = Qn;
+        auto chord_terms = [&](double sy, AnalyticParam& A) {
+            A.by_gauss = !(b > 0.0);
+            A.paired = 0;
+            if (pure_gauss) {                     // P2: pure gaussian, one term
+                A.n_terms = 1; A.s[0] = 0.0; A.cs[0] = 0.0; A.wq[0] = 1.0; A.g[0] = 1.0;
+                return;
+            }
             int nt = 0;
-            // nodes q and Q+1-q share |s|, c and the weight: one term with F(d) = Phi(d - s) + Phi(d + s)
-            for (int q = 1; 2 * q <= Q + 1; ++q) {
-                const long double th = (long double)q * 3.14159265358979323846264338327950288L / (long double)(Q + 1);
+            for (int q = 1; 2 * q <= Qn + 1; ++q) {
+                const long double th = (long double)q * 3.14159265358979323846264338327950288L / (long double)(Qn + 1);
                 const long double sn = sinl(th), cn = cosl(th);
                 A.s[nt] = (double)((long double)a * cn);
                 const long double c = (long double)b * sn;
-                A.cs[nt] = (double)(c / (long double)d->sigma_y);
-                A.wq[nt] = (double)((2.0L / (long double)(Q + 1)) * sn * sn);
-                A.g[nt] = b > 0.0 ? (double)((long double)d->sigma_y / (2.0L * c)) : 1.0;
-                if (2 * q != Q + 1) A.paired |= 1u << nt;
+                A.cs[nt] = (double)(c / (long double)sy);
+                A.wq[nt] = (double)((2.0L / (long double)(Qn + 1)) * sn * sn);
+                A.g[nt] = b > 0.0 ? (double)((long double)sy / (2.0L * c)) : 1.0;
+                if (2 * q != Qn + 1) A.paired |= 1u << nt;
                 else A.s[nt] = 0.0;               // middle node of an odd rule sits at s = 0
                 ++nt;
             }
             A.n_terms = nt;
-        }
-        // production path: pixel-phase polynomial tables (the direct special-function kernel stays as the fallback
-        // for PSFs whose tables do not converge: sigma below ~0.3 px)
-        {
+        };
+        auto shape_of = [&](double sx, double sy, const AnalyticParam& A) {
             PsfShape shape;
-            shape.sx = d->sigma_x; shape.sy = d->sigma_y; shape.by_gauss = A.by_gauss != 0;
+            shape.sx = sx; shape.sy = sy; shape.by_gauss = A.by_gauss != 0;
             for (int i = 0; i < A.n_terms; ++i) {
                 ChordTerm ct;
                 ct.s = A.s[i]; ct.cs = A.cs[i]; ct.wq = A.wq[i]; ct.g = A.g[i]; ct.paired = (A.paired >> i) & 1u;
                 shape.terms.push_back(ct);
             }
+            return shape;
+        };
+        AnalyticParam& A = P->an;
+        A.inv_sx = 1.0 / sx_box; A.inv_sy = 1.0 / sy_box;
+        A.hbx = P->hbx; A.hby = P->hby;
+        chord_terms(is_map ? sy_box : d->sigma_y, A);
+        if (is_map) {
+            // analytic PSF map: one moment-table set per node, all with the same layout (x degree, y windows) = the
+            // finest any node needs.  No per-sample-polynomial or direct fallback: the map needs the cell-moment kernel.
+            P->is_map = true;
+            std::vector<MomentTables> tabs(n_map);
+            std::vector<AnalyticParam> An(n_map);
+            int Pmax = 0, nybmax = 0;
+            for (int c = 0; c < n_map; ++c) {
+                memset(&An[c], 0, sizeof(AnalyticParam));
+                chord_terms(d->an_sigma_y[c], An[c]);
+                if (!build_moment_tables(shape_of(d->an_sigma_x[c], d->an_sigma_y[c], An[c]), P->hbx, P->hby, tabs[c]))
+                    return fail(E2E_ERR_UNSUPPORTED, "psf_create: no converged moment tables for a node of the PSF map (sigma too small)");
+                Pmax = std::max(Pmax, tabs[c].P); nybmax = std::max(nybmax, tabs[c].nyb);
+            }
+            for (int c = 0; c < n_map; ++c)
+                if (tabs[c].P != Pmax || tabs[c].nyb != nybmax) {
+                    tabs[c] = MomentTables();
+                    if (!build_moment_tables(shape_of(d->an_sigma_x[c], d->an_sigma_y[c], An[c]), P->hbx, P->hby, tabs[c], Pmax, nybmax))
+                        return fail(E2E_ERR_UNSUPPORTED, "psf_create: PSF map nodes do not share a table layout");
+                }
+            if (tabs[0].npt > 4) return fail(E2E_ERR_UNSUPPORTED, "psf_create: PSF map needs an x degree above 31");
+            const size_t nfx = tabs[0].fx.size(), nfy = tabs[0].fy.size();
+            for (int c = 1; c < n_map; ++c)
+                if (tabs[c].fx.size() != nfx || tabs[c].fy.size() != nfy) return fail(E2E_ERR_UNSUPPORTED, "psf_create: PSF map table sizes differ");
+            E2E_CUDA(cudaMalloc(&P->d_mom, 8 * (nfx + nfy) * (size_t)n_map));
+            cudaError_t ce = cudaSuccess;
+            for (int c = 0; c < n_map && ce == cudaSuccess; ++c) {
+                ce = cudaMemcpy(P->d_mom + nfx * c, tabs[c].fx.data(), 8 * nfx, cudaMemcpyHostToDevice);
+                if (ce == cudaSuccess) ce = cudaMemcpy(P->d_mom + nfx * n_map + nfy * c, tabs[c].fy.data(), 8 * nfy, cudaMemcpyHostToDevice);
+            }
+            if (ce != cudaSuccess) { cudaFree(P->d_mom); P->d_mom = nullptr; return fail_cuda(ce, "psf_create: PSF map table upload"); }
+            const MomentTables& mom = tabs[0];
+            MomentParam& M = P->mom;
+            M.T = mom.T; M.ncol = mom.ncol; M.nrow = mom.nrow; M.nit = mom.nit; M.njt = mom.njt;
+            M.hbx = P->hbx; M.hby = P->hby; M.c0x = mom.c0x; M.c0y = mom.c0y; M.nyb = mom.nyb;
+            M.fx = reinterpret_cast<const double2*>(P->d_mom);
+            M.fy = reinterpret_cast<const double2*>(P->d_mom + nfx * n_map);
+            M.gx = d->an_gx; M.gy = d->an_gy;
+            M.fsx = nx > 1 ? (double)(d->an_gx - 1) / (double)(nx - 1) : 0.0;
+            M.fsy = ny > 1 ? (double)(d->an_gy - 1) / (double)(ny - 1) : 0.0;
+            M.fx_node_stride = nfx / 2; M.fy_node_stride = nfy / 2;
+            P->moment_npt = mom.npt;
+            P->moment_degree = mom.P;
+        } else {
+            // production path: pixel-phase polynomial tables (the direct special-function kernel stays as the fallback
+            // for PSFs whose tables do not converge: sigma below ~0.3 px)
+            const PsfShape shape = shape_of(d->sigma_x, d->sigma_y, A);
+            A.inv_sx = 1.0 / d->sigma_x; A.inv_sy = 1.0 / d->sigma_y;
             PolyTables tabs;
             if (build_poly_tables(shape, P->hbx, P->hby, tabs) && tabs.ncol_pad <= kMaxWin && tabs.nrow_pad <= kMaxWin) {
                 const size_t nx_ = tabs.tx.size(), ny_ = tabs.ty.size();
@@ -907,7 +978,7 @@ static int launch_setup(const e2e_format* F, const e2e_plan* pl, const e2e_spect
 // dense sampling -> per-cell moments; sparse sampling (few samples per footprint cell) -> per-sample polynomials
 static bool choose_moment(const e2e_format* F, const e2e_psf* P)
 {
-    return P->kind == 0 && P->moment_npt > 0 && F->samples_per_px >= kMomentMinSpp;
+    return P->kind == 0 && P->moment_npt > 0 && (F->samples_per_px >= kMomentMinSpp || P->is_map);
 }
 
 // tabulated PSF: cell-deposit kernel unless the oversampling is too fine for its weight array
@@ -932,7 +1003,7 @@ struct QueueSel {
 };
 
 // dynamic shared memory attribute of the moment kernel: per device, set once
-template <int NPT>
+template <int NPT, bool MAP>
 static int moment_kernel_attr(size_t smem)
 {
     static bool set[64] = {};
@@ -940,7 +1011,7 @@ static int moment_kernel_attr(size_t smem)
     E2E_CUDA(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return fail(E2E_ERR_UNSUPPORTED, "render: device index above 63");
     if (!set[dev]) {
-        E2E_CUDA(cudaFuncSetAttribute(render_moment_kernel<NPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        E2E_CUDA(cudaFuncSetAttribute(render_moment_kernel<NPT, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         set[dev] = true;
     }
     return E2E_OK;
@@ -960,19 +1031,26 @@ static int launch_render(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
         W.queue = qs.queue; W.n = qs.n; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
         W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx;
         W.ctrl = qs.ctrl; W.head = qs.head; W.ctrl_stride = (long long)(ctrl_bytes(pl) / sizeof(unsigned));
-#define E2E_MOM_CASE(NPT)                                                                                               \
+#define E2E_MOM_CASE(NPT, MAP)                                                                                          \
     case NPT: {                                                                                                         \
-        const size_t sm = sizeof(MomentWarpSmem<NPT>) * kMomWarps;                                                      \
-        int rc = moment_kernel_attr<NPT>(sm);                                                                           \
+        const size_t sm = sizeof(MomentWarpSmem<NPT, MAP>) * kMomWarps;                                                 \
+        int rc = moment_kernel_attr<NPT, MAP>(sm);                                                                      \
         if (rc) return rc;                                                                                              \
         const unsigned pb = (unsigned)((qs.n + kMomWarps - 1) / kMomWarps);                                             \
-        render_moment_kernel<NPT><<<dim3(pb, n_frames), kMomWarps * 32, sm, stream>>>(                                  \
+        render_moment_kernel<NPT, MAP><<<dim3(pb, n_frames), kMomWarps * 32, sm, stream>>>(                             \
             d_x, d_y, d_w, pl->d_strips, pl->d_items, W, P->mom, d_frame, F->view.nx, F->view.ny, w_stride,             \
             n_frames > 1 ? d_frames : nullptr);                                                                          \
     } break;
-        switch (P->moment_npt) {
-            E2E_MOM_CASE(2) E2E_MOM_CASE(3) E2E_MOM_CASE(4)
-            default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+        if (P->is_map) {
+            switch (P->moment_npt) {
+                E2E_MOM_CASE(2, true) E2E_MOM_CASE(3, true) E2E_MOM_CASE(4, true)
+                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+            }
+        } else {
+            switch (P->moment_npt) {
+                E2E_MOM_CASE(2, false) E2E_MOM_CASE(3, false) E2E_MOM_CASE(4, false)
+                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+            }
         }
 #undef E2E_MOM_CASE
         count_launch();
@@ -1547,12 +1625,14 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
     double pc = 0.0, ps = 0.0;
     if (choose_moment(fmt, psf)) {
         static const char* names[] = {"", "", "render_moment_kernel<2>", "render_moment_kernel<3>", "render_moment_kernel<4>"};
+        static const char* map_names[] = {"", "", "render_moment_kernel<2, map>", "render_moment_kernel<3, map>", "render_moment_kernel<4, map>"};
         const MomentParam& M = psf->mom;
         const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
-        nm = names[npt];
+        nm = psf->is_map ? map_names[npt] : names[npt];
+        const double nodes = psf->is_map ? (M.gx > 1 ? 2.0 : 1.0) * (M.gy > 1 ? 2.0 : 1.0) : 1.0;
         // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
-        pc = 256.0 * M.T * (2.0 * npt * M.nit * jp + 2.0 * M.nit * M.njt);         // step 2 (redone per row panel) + step 3
-        ps = 64.0 * npt + 8.0 * npt + 8.0;                     // step 1 (npt DMMAs per 4 samples) + powers
+        pc = nodes * 256.0 * M.T * (2.0 * npt * M.nit * jp + 2.0 * M.nit * M.njt);         // step 2 (redone per row panel) + step 3
+        ps = nodes * 64.0 * npt + 8.0 * npt + 8.0;             // step 1 (npt DMMAs per 4 samples and node) + powers
         (void)ip;
     } else if (psf->kind == 0 && psf->poly_degree > 0) {
         static thread_local char buf[40];
@@ -1576,8 +1656,9 @@ int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, do
     if (choose_moment(fmt, psf)) {
         const double w = std::floor(2.0 * psf->hbx), h = std::floor(2.0 * psf->hby);   // nominal footprint (2 H + 1 per axis, G9)
         const double np1 = (double)psf->moment_degree + 1.0;
-        pc = (double)psf->mom.T * (8.0 * np1 * w + 8.0 * w * h);
-        ps = 8.0 * np1;
+        const double nodes = psf->is_map ? (psf->mom.gx > 1 ? 2.0 : 1.0) * (psf->mom.gy > 1 ? 2.0 : 1.0) : 1.0;   // G21: one moment set per node
+        pc = nodes * (double)psf->mom.T * (8.0 * np1 * w + 8.0 * w * h);
+        ps = nodes * 8.0 * np1;
     } else if (choose_tabcell(psf)) {
         // cell-deposit method (render_tabcell.cuh): one FMA per (field node, y-offset row, x-offset, window pixel) and cell --
         // the samples of a cell sweep all os + 1 x-offsets and, on a trace flatter than 1/os px per px, 2 y-offset rows --

@@ -126,6 +126,10 @@ struct MomentParam {
     const double2* fx;                 // [T][nit][npt][32] fragment-ordered coefficient pairs
     const double2* fy;                 // [nyb][T][njt][32]   y-phase windows, degree 7 (one power tile)
     int nyb;                           // windows: centres -1/2 + (b + 1/2)/nyb, valid for |dy - centre| <= 1/nyb
+    // analytic PSF map (G21): gx x gy nodes, node n's tables at fx + n * fx_node_stride, fy + n * fy_node_stride (0 x 0: one PSF)
+    int gx, gy;
+    double fsx, fsy;                   // (gx-1)/(nx-1), (gy-1)/(ny-1)
+    size_t fx_node_stride, fy_node_stride;
 };
 
 struct TabParam {
@@ -162,6 +166,7 @@ struct e2e_psf {
     int moment_degree = 0;         // x-phase degree of the moment tables
     e2e::MomentParam mom;
     double* d_mom = nullptr;       // one allocation: fx then fy
+    bool is_map = false;           // analytic PSF map (G21): mom holds one table set per node
 };
 
 struct e2e_plan {                  // schedule for one (format, footprint) pair; cached in the format handle

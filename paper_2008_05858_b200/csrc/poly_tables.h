@@ -193,7 +193,8 @@ constexpr int kMomYBins[] = {16, 32, 64, 128, 256};
 // valid for +-1/nyb around its centre) and each window gets its own degree-7 Chebyshev fit -- 8 coefficients = one DMMA
 // power tile instead of two or three.  A cell takes the window whose centre is nearest to its first sample (|delta| <=
 // 1/(2 nyb)) and keeps it while |delta| <= 1/nyb (render_moment.cuh).  nyb = the coarsest of kMomYBins that reaches kPolyTol.
-inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, MomentTables& out)
+// force_P / force_nyb > 0: use exactly that x degree / that number of y windows (a PSF map needs one layout for all its nodes)
+inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, MomentTables& out, int force_P = 0, int force_nyb = 0)
 {
     out.c0x = hbx - 0.5;
     out.c0y = hby - 0.5;
@@ -208,6 +209,7 @@ inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, Momen
     long double worst_x = 0.0L;
     for (int di = 0; di < kNumPolyDegrees && !okx; ++di) {
         const int P = kPolyDegrees[di];
+        if (force_P > 0 && P != force_P) continue;
         const int npt = (P + 1 + 7) / 8;
         std::vector<long double> mono(P + 1);
         std::vector<double> fx((size_t)out.T * out.nit * npt * 64, 0.0);
@@ -229,7 +231,7 @@ inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, Momen
                 }
             }
         }
-        if (worst <= kPolyTol || di == kNumPolyDegrees - 1) {
+        if (worst <= kPolyTol || di == kNumPolyDegrees - 1 || force_P > 0) {
             out.P = P;
             out.npt = npt;
             out.fx.swap(fx);
@@ -241,6 +243,7 @@ inline bool build_moment_tables(const PsfShape& S, double hbx, double hby, Momen
     if (!okx) return false;
     // ---- y: windows
     for (int nyb : kMomYBins) {
+        if (force_nyb > 0 && nyb != force_nyb) continue;
         const long double hw = 1.0L / (long double)nyb;
         std::vector<long double> mono(kMomYDegree + 1);
         std::vector<double> fy((size_t)nyb * out.T * out.njt * 64, 0.0);

@@ -54,10 +54,11 @@ constexpr int kMomWarps = 1;           // warps per CTA: one item per CTA, so a 
                                        // (4 / 2 / 1 warps per CTA: 6.18 / 6.17 / 6.13 ms)
 constexpr int kMomLdk = 36;            // pitch of the power arrays V[power][sample] (36 mod 16 = 4: conflict-free fragments)
 
-template <int NPT>
+template <int NPT, bool MAP = false>
 struct MomentWarpSmem {
     double vx[8 * NPT * kMomLdk];      // w_k dx_k^q
     double vy[8 * kMomLdk];            // delta_k^p, p = 0..7 (rewritten for every cell: delta is relative to the cell's window)
+    double beta[MAP ? 4 * kMomLdk : 1];// PSF map (G21): bilinear weight of each of the cell's 4 nodes at every sample
 };
 
 // work queue of one render launch
@@ -115,8 +116,11 @@ __device__ __forceinline__ void queue_done(const QueueParam& W, unsigned* ctrl, 
     for (int d = W.succ_off[item_id] + lane; d < s1; d += 32) red_release_dec_u32(pend + W.succ_idx[d]);
 }
 
-template <int NPT>
-__global__ void __launch_bounds__(kMomWarps * 32, NPT == 2 ? E2E_MOM_MINB : 1)
+// MAP (G21, analytic PSF map): the PSF of a sample is the bilinear blend of 4 node PSFs, and the blend is linear, so
+// a cell (now also: one node cell of the map) keeps ONE weighted moment set per node, M_c = sum_k (w_k beta_c,k) delta^p dx^q, and
+// its contribution is sum_c cy_c^T M_c cx_c with node c's own tables -- steps 2 + 3 run once per node into the same window.
+template <int NPT, bool MAP>
+__global__ void __launch_bounds__(kMomWarps * 32, MAP ? 12 : (NPT == 2 ? E2E_MOM_MINB : 1))
 render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                      const Strip* __restrict__ strips, const Item* __restrict__ items, QueueParam W, MomentParam Q,
                      double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)
@@ -127,7 +131,8 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         frame = frames[blockIdx.y];                           // same geometry, its own weights, target and control block
         ws += (long long)blockIdx.y * w_stride;
     }
-    MomentWarpSmem<NPT>& S = reinterpret_cast<MomentWarpSmem<NPT>*>(smem_raw)[warp];
+    MomentWarpSmem<NPT, MAP>& S = reinterpret_cast<MomentWarpSmem<NPT, MAP>*>(smem_raw)[warp];
+    constexpr int NC = MAP ? 4 : 1;                           // moment sets per cell
     const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
     constexpr int NP = 8 * NPT;
     const double ywin = 1.0 / (double)Q.nyb;
@@ -141,9 +146,10 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
     long long kend = k + (long long)it.nchunks * 32;
     if (kend > st.n) kend = st.n;
 
-    double mt[NPT][2];                                         // M tiles [qt]: lane holds M[p = l/4][q = 8qt + 2(l%4) + e]
+    double mt[NC][NPT][2];                                     // M tiles [node][qt]: lane holds M[p = l/4][q = 8qt + 2(l%4) + e]
     bool have = false;
     int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
+    int cG = 0, cH = 0;                                        // MAP: its node cell (first node column / row)
     double cYc = 0.0;                                          // its centre
 
     // steps 2 + 3 + a5 for the open cell
@@ -159,10 +165,24 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
                     for (int b = 0; b < 3; ++b) { out[a][b][0] = 0.0; out[a][b][1] = 0.0; }
+#pragma unroll 1
+              for (int c = 0; c < NC; ++c) {
+                size_t node = 0;
+                if (MAP) {                                     // node c = 2 (row) + (column) of the cell's 4; absent on 1-wide grids
+                    if (((c & 1) && Q.gx == 1) || ((c & 2) && Q.gy == 1)) continue;
+                    node = (size_t)(cH + (c >> 1)) * Q.gx + (cG + (c & 1));
+                }
+                double mc[NPT][2];                             // this node's moment set (static register indices only)
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc)
+                    if (cc == c) {
+#pragma unroll
+                        for (int qt = 0; qt < NPT; ++qt) { mc[qt][0] = mt[cc][qt][0]; mc[qt][1] = mt[cc][qt][1]; }
+                    }
 #pragma unroll 2                                        // two terms in flight: step 2 of one overlaps step 3 of the other
                 for (int t = 0; t < Q.T; ++t) {
-                    const double2* fy = Q.fy + ((size_t)(cYb * Q.T + t) * Q.njt + jp) * 32 + lane;
-                    const double2* fx = Q.fx + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
+                    const double2* fy = Q.fy + node * Q.fy_node_stride + ((size_t)(cYb * Q.T + t) * Q.njt + jp) * 32 + lane;
+                    const double2* fx = Q.fx + node * Q.fx_node_stride + ((size_t)(t * Q.nit + ip) * NPT) * 32 + lane;
                     double2 cy[3], cx[3][NPT];
 #pragma unroll
                     for (int jt = 0; jt < 3; ++jt) cy[jt] = (jp + jt < Q.njt) ? __ldg(fy + jt * 32) : make_double2(0.0, 0.0);
@@ -178,9 +198,9 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
 #pragma unroll
                     for (int qt = 0; qt < NPT; ++qt) {
 #pragma unroll
-                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].x, mt[qt][0]);
+                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].x, mc[qt][0]);
 #pragma unroll
-                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].y, mt[qt][1]);
+                        for (int it = 0; it < 3; ++it) dmma_m8n8k4(yt[it][0], yt[it][1], cx[it][qt].y, mc[qt][1]);
                     }
                     // ---- step 3: out^T += Y_t^T cy_t  (contraction over the 8 powers of delta: two k-slots)
 #pragma unroll
@@ -192,6 +212,7 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
 #pragma unroll
                         for (int jt = 0; jt < 3; ++jt) dmma_m8n8k4(out[it][jt][0], out[it][jt][1], yt[it][1], cy[jt].y);
                 }
+              }
                 // ---- a5: add the panel to the frame by L2 reductions (red.global.add.f64): the same IEEE sum as load + add +
                 // store without a round trip to wait for.  Order per pixel: items of one launch never share a pixel, and
                 // inside the warp the __syncwarp() that closes every flush orders this cell's reductions before the next
@@ -226,7 +247,28 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         const int jlo = __double2int_ru(__dsub_rn(yk, Q.hby)), jhi = __double2int_rd(__dadd_rn(yk, Q.hby));
         const double dx = __dsub_rn(__dsub_rn(xk, (double)ilo), Q.c0x);
         const double dy = __dsub_rn(__dsub_rn(yk, (double)jlo), Q.c0y);
+        // MAP: node cell and bilinear weights of the sample (T3's rule: nodes at g (nx-1)/(gx-1), clamped outside the grid)
+        int g0 = 0, h0 = 0;
+        double bfx = 0.0, bfy = 0.0;
+        if (MAP) {
+            if (Q.gx > 1) {
+                const double t = fmin(fmax(xk * Q.fsx, 0.0), (double)(Q.gx - 1));
+                g0 = min((int)floor(t), Q.gx - 2);
+                bfx = t - (double)g0;
+            }
+            if (Q.gy > 1) {
+                const double t = fmin(fmax(yk * Q.fsy, 0.0), (double)(Q.gy - 1));
+                h0 = min((int)floor(t), Q.gy - 2);
+                bfy = t - (double)h0;
+            }
+        }
         __syncwarp();                                          // previous batch's readers are done
+        if (MAP) {
+            S.beta[0 * kMomLdk + lane] = (1.0 - bfy) * (1.0 - bfx);
+            S.beta[1 * kMomLdk + lane] = (1.0 - bfy) * bfx;
+            S.beta[2 * kMomLdk + lane] = bfy * (1.0 - bfx);
+            S.beta[3 * kMomLdk + lane] = bfy * bfx;
+        }
         {
             // w dx^p by repeated squaring: the same number of multiplications, dependency depth log2(NP) instead of NP
             double v[NP];
@@ -248,22 +290,25 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
             const int kI0 = __shfl_sync(0xffffffffu, ilo, pos), kI1 = __shfl_sync(0xffffffffu, ihi, pos);
             const int kJ0 = __shfl_sync(0xffffffffu, jlo, pos), kJ1 = __shfl_sync(0xffffffffu, jhi, pos);
             const double kdy = __shfl_sync(0xffffffffu, dy, pos);
-            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1 || !(fabs(kdy - cYc) <= ywin))) {
+            const int kG = MAP ? __shfl_sync(0xffffffffu, g0, pos) : 0, kH = MAP ? __shfl_sync(0xffffffffu, h0, pos) : 0;
+            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1 || !(fabs(kdy - cYc) <= ywin) || kG != cG || kH != cH)) {
                 flush();
                 have = false;
             }
             if (!have) {
                 have = true;
-                cI0 = kI0; cI1 = kI1; cJ0 = kJ0; cJ1 = kJ1;
+                cI0 = kI0; cI1 = kI1; cJ0 = kJ0; cJ1 = kJ1; cG = kG; cH = kH;
                 // window whose centre is nearest to the first sample: |delta| <= ywin / 2, kept while |delta| <= ywin
                 cYb = min(max((int)floor((kdy + 0.5) * (double)Q.nyb), 0), Q.nyb - 1);
                 cYc = ((double)cYb + 0.5) * ywin - 0.5;
 #pragma unroll
-                for (int a = 0; a < NPT; ++a) { mt[a][0] = 0.0; mt[a][1] = 0.0; }
+                for (int c = 0; c < NC; ++c)
+#pragma unroll
+                    for (int a = 0; a < NPT; ++a) { mt[c][a][0] = 0.0; mt[c][a][1] = 0.0; }
             }
             const double dl = dy - cYc;
             const unsigned same = __ballot_sync(0xffffffffu, valid && ilo == cI0 && ihi == cI1 && jlo == cJ0 && jhi == cJ1 &&
-                                                                 fabs(dl) <= ywin);
+                                                                 fabs(dl) <= ywin && g0 == cG && h0 == cH);
             const unsigned rest = ~(same >> pos);              // bit r: sample pos + r is NOT in the cell
             const int run = rest ? (__ffs(rest) - 1) : 32;     // >= 1: sample pos is in
             const int pend = min(pos + run, nb);
@@ -291,7 +336,11 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
 #pragma unroll
                 for (int qt = 0; qt < NPT; ++qt) b[qt] = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
 #pragma unroll
-                for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[qt][0], mt[qt][1], a, b[qt]);
+                for (int c = 0; c < NC; ++c) {
+                    const double ac = MAP ? a * S.beta[c * kMomLdk + ksamp] : a;   // the node weight rides on the delta powers
+#pragma unroll
+                    for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[c][qt][0], mt[c][qt][1], ac, b[qt]);
+                }
             }
             pos = pend;
         }

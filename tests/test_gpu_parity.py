@@ -151,6 +151,54 @@ def test_render_narrow_sigma_reaches_the_direct_kernel(B):
         assert abs(G.sum() / oracle.total_weight(s) - 1.0) < 1e-12
 
 
+@pytest.mark.parametrize("grid", [(2, 2), (3, 2), (1, 3), (4, 1)])
+def test_render_psf_map(B, grid):
+    """S8(f) 3 / DESIGN.md G21 (P:61 'PSF ... for each wavelength'): analytic PSF map, the PSF of a sample = bilinear blend of
+    the 4 surrounding node PSFs.  Whole frame against the oracle per pixel: strips that cross node boundaries in x, a steep
+    two-fiber scene that crosses them in y, and the single-sample scene (box from the largest node sigma)"""
+    gx, gy = grid
+    s = small_tiny(spp=8.0, lam=(5010.0, 5030.0))                      # x = 424 .. 1224 on 2048 columns
+    s.fiber_dx = np.array([0.0, 0.4]); s.fiber_dy = np.array([-30.0, 41.5])
+    s.spectra = [s.spectra[0], s.spectra[0]]
+    s.coef_y = np.array([128.0, 150.0, 0.0, 0.0])                      # rows 68 .. 158 (+ fibers): crosses the y node at 127.5
+    m = W.psf_map(s, gx=gx, gy=gy, seed=60 + gx)
+    r = B.Renderer(m)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"].endswith("map>")
+        G = r.render().cpu().numpy()
+        again = r.render().cpu().numpy()
+        c = B.e2e_plan_check(r.fmt, r.psf)
+    finally:
+        r.close()
+    assert np.array_equal(G, again)
+    assert c["queue_conflicts"] == 0 and c["phase_conflicts"] == 0
+    O = oracle.render(m)
+    assert O.max() > 0
+    e = assert_frame_parity(G, O, f"psf map {grid}")
+    assert e["max_rel_core"] < 1e-11
+    assert abs(G.sum() / oracle.total_weight(m) - 1.0) < 1e-12
+    d = W.psf_map(W.single_line_scene(x_pos=100.3173, y_pos=37.8641), gx=gx, gy=gy, seed=6)
+    Gd, Od = gpu_render(B, d), oracle.render(d)
+    assert_frame_parity(Gd, Od, "psf map, single sample")
+    assert np.array_equal(Gd != 0.0, Od != 0.0)                        # the common box (largest node sigma)
+
+
+def test_render_psf_map_espresso_windows(B):
+    """the ESPRESSO-like frame (7 orders of it) with a 3 x 3 PSF map: oracle windows at strip ends and inside, both fibers"""
+    s = W.psf_map(W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 40, 41, 42, 83, 84]), gx=3, gy=3)
+    G = gpu_render(B, s)
+    assert np.isfinite(G).all()
+    for o, frac in ((0, 0.002), (1, 0.5), (3, 0.4999), (4, 0.75), (6, 0.998)):
+        n = oracle.order_nsamples(s, o)
+        k = int(frac * (n - 1))
+        lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
+        i0, j0 = max(0, int(x[0]) - 16), max(0, int(y[0]) - 22)
+        O = oracle.render(s, window=(i0, j0, 32, 44))
+        assert O.max() > 0
+        assert_frame_parity(G[j0:j0 + 44, i0:i0 + 32], O, f"psf map window {i0},{j0}")
+    assert abs(float(G.sum(dtype=np.longdouble)) / oracle.total_weight(s) - 1.0) < 1e-12
+
+
 def test_render_single_sample_is_the_psf_itself(B):
     d = W.single_line_scene(x_pos=100.3173, y_pos=37.8641)
     G = gpu_render(B, d)

@@ -98,6 +98,57 @@ E2E_API void e2e_format_destroy(e2e_format_t* fmt);
 E2E_API int e2e_format_num_samples(const e2e_format_t* fmt, int64_t* n_per_order, int64_t* n_total);
 
 /* ------------------------------------------------------------------------------------------------
+ * Parametric Spectrograph Unit ("the Parametric Version ... requires only geometrical parameters (such as dispersing
+ * elements working angle, optical elements working F-Number) to recover the expected spectral format required for rendering
+ * the image"; P:165 blaze "for each order"; P:59 / P:155 line tilt).  HOST code, no device call: fills the arrays an
+ * e2e_format_desc_t / e2e_psf_desc_t needs from the relations of a cross-dispersed echelle spectrograph (G22):
+ *   echelle   m lam = d cos(gamma) (sin alpha + sin beta), alpha = blaze + theta, blaze peak at beta_c = blaze - theta,
+ *             lam_c(m) = K / m with K = 2 d cos(gamma) sin(blaze) cos(theta); one free spectral range per order,
+ *             lam in [K / (m + 1/2), K / (m - 1/2)]; x = x_c + F tan(beta - beta_c), F = f_cam / pixel
+ *   cross-disperser  first-order grating in Littrow at xd_lam_ref: sin beta_x = lam / d_x - sin alpha_x;
+ *             y = y_c + F tan(beta_x - alpha_x)
+ *   fibers    image widths Dy = core f_cam / (f_coll pixel), Dx = Dy cos(alpha) / cos(beta_c); fiber at height h along the
+ *             pseudo-slit: dy = h f_cam / (f_coll pixel), dx = tan(chi) dy, tan(chi) = tan(gamma) (sin alpha + sin beta_c) / cos(beta_c)
+ *   blaze     amplitude min(1, cos(alpha) / cos(beta_c)) (groove shadowing), sinc^2 profile of e2e_format_desc_t
+ * x and y are delivered as the degree-(5, 5) tensor polynomials of e2e_format_desc_t (x depends on (lam, m) through
+ * m lam / K - 1 only, bilinear in (L, M): its degree-5 Chebyshev interpolant is expanded exactly; y: degree-5 interpolant in
+ * L); residual_x_px / residual_y_px = largest deviation of the stored polynomials from the closed forms over all orders.
+ * Output arrays are owned by the caller: order arrays of capacity_orders >= m_hi - m_lo + 1 entries, coef_x / coef_y of 36,
+ * fiber_dx / fiber_dy of n_fibers.  Errors: NULL / non-finite / non-positive parameters -> E2E_ERR_INVALID_ARG; a diffraction
+ * angle beyond 90 degrees -> E2E_ERR_UNSUPPORTED.
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    double groove_um;               /* echelle groove spacing d (1000 / grooves per mm) */
+    double blaze_deg;               /* blaze angle */
+    double theta_deg;               /* in-plane angle between the incident beam and the blaze normal (quasi-Littrow: small) */
+    double gamma_deg;               /* off-plane angle (gives the line tilt) */
+    double xd_groove_um;            /* cross-disperser groove spacing */
+    double xd_lam_ref;              /* Angstrom: cross-disperser in Littrow here; this wavelength lands on row y_c */
+    double f_cam_mm, f_coll_mm;     /* camera and collimator focal lengths */
+    double pixel_um;
+    double fiber_core_um;           /* diameter of the fiber core as seen at the spectrograph entrance */
+    int32_t m_lo, m_hi;             /* echelle orders to generate */
+    double x_c, y_c;                /* column of the blaze peaks, row of xd_lam_ref */
+    int32_t n_fibers;
+    const double* fiber_height_um;  /* [n_fibers] positions along the pseudo-slit */
+} e2e_spectrograph_t;
+
+typedef struct {
+    int32_t capacity_orders;        /* in: length of the order arrays below */
+    int32_t n_orders, deg_l, deg_m; /* out */
+    int32_t* order_m;               /* out [n_orders] */
+    double *lam_min, *lam_max, *blaze_lam_c, *blaze_amp;   /* out [n_orders] */
+    double *coef_x, *coef_y;        /* out [36] */
+    double lam0, inv_dlam, m0, inv_dm;
+    double *fiber_dx, *fiber_dy;    /* out [n_fibers] */
+    double fiber_dx_px, fiber_dy_px;/* out: full widths of the fiber image (e2e_psf_desc_t) */
+    double residual_x_px, residual_y_px;
+    double x_min, x_max, y_min, y_max;   /* extent of the traces (base trace, no fiber offset) */
+    double tilt_tan, K, px_per_radian;
+} e2e_spectrograph_format_t;
+E2E_API int e2e_spectrograph_format(const e2e_spectrograph_t* sp, e2e_spectrograph_format_t* out);
+
+/* ------------------------------------------------------------------------------------------------
  * Instrument PSF = fiber image (x) optical PSF
  * ------------------------------------------------------------------------------------------------ */
 typedef struct e2e_psf e2e_psf_t; /* opaque; immutable after create */

@@ -26,7 +26,7 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_apply_detector_adu16", "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
            "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames",
-           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check"]
+           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check", "e2e_spectrograph_format"]
 
 
 class E2EError(RuntimeError):
@@ -71,6 +71,24 @@ class DetectorDesc(C.Structure):
 class DetectorExDesc(C.Structure):
     _fields_ = [("base", DetectorDesc), ("d_prnu", C.c_void_p), ("d_dark", C.c_void_p), ("full_well_e", C.c_double),
                 ("e_per_adu", C.c_double), ("adu_max", C.c_double), ("n_ports", C.c_int32), ("xtalk", C.c_void_p)]
+
+
+class SpectrographDesc(C.Structure):
+    _fields_ = [("groove_um", C.c_double), ("blaze_deg", C.c_double), ("theta_deg", C.c_double), ("gamma_deg", C.c_double),
+                ("xd_groove_um", C.c_double), ("xd_lam_ref", C.c_double), ("f_cam_mm", C.c_double), ("f_coll_mm", C.c_double),
+                ("pixel_um", C.c_double), ("fiber_core_um", C.c_double), ("m_lo", C.c_int32), ("m_hi", C.c_int32),
+                ("x_c", C.c_double), ("y_c", C.c_double), ("n_fibers", C.c_int32), ("fiber_height_um", C.c_void_p)]
+
+
+class SpectrographFormatDesc(C.Structure):
+    _fields_ = [("capacity_orders", C.c_int32), ("n_orders", C.c_int32), ("deg_l", C.c_int32), ("deg_m", C.c_int32),
+                ("order_m", C.c_void_p), ("lam_min", C.c_void_p), ("lam_max", C.c_void_p), ("blaze_lam_c", C.c_void_p),
+                ("blaze_amp", C.c_void_p), ("coef_x", C.c_void_p), ("coef_y", C.c_void_p), ("lam0", C.c_double),
+                ("inv_dlam", C.c_double), ("m0", C.c_double), ("inv_dm", C.c_double), ("fiber_dx", C.c_void_p),
+                ("fiber_dy", C.c_void_p), ("fiber_dx_px", C.c_double), ("fiber_dy_px", C.c_double),
+                ("residual_x_px", C.c_double), ("residual_y_px", C.c_double), ("x_min", C.c_double), ("x_max", C.c_double),
+                ("y_min", C.c_double), ("y_max", C.c_double), ("tilt_tan", C.c_double), ("K", C.c_double),
+                ("px_per_radian", C.c_double)]
 
 
 class PlanCheckDesc(C.Structure):
@@ -125,6 +143,8 @@ def load():
     L.e2e_render_frame_host_adu16.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(DetectorExDesc), vp, vp, C.c_size_t, vp]
     L.e2e_plan_check.restype = C.c_int
     L.e2e_plan_check.argtypes = [vp, vp, C.POINTER(PlanCheckDesc)]
+    L.e2e_spectrograph_format.restype = C.c_int
+    L.e2e_spectrograph_format.argtypes = [C.POINTER(SpectrographDesc), C.POINTER(SpectrographFormatDesc)]
     L.e2e_apply_detector.restype = C.c_int
     L.e2e_apply_detector.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorDesc), vp]
     L.e2e_apply_detector_ex.restype = C.c_int
@@ -350,6 +370,32 @@ def e2e_render_frame_host_ex(fmt: Format, psf: Psf, spectra_desc, h_frame_ptr: i
     fn = load().e2e_render_frame_host_adu16 if adu16 else load().e2e_render_frame_host_ex
     _check(fn(fmt.handle, psf.handle, spectra_desc, C.byref(det_ex_desc), int(h_frame_ptr), int(d_workspace.data_ptr()),
               int(d_workspace.numel() * d_workspace.element_size()), _stream_ptr(stream)))
+
+
+def e2e_spectrograph_format(groove_um: float, blaze_deg: float, theta_deg: float, gamma_deg: float, xd_groove_um: float,
+                            xd_lam_ref: float, f_cam_mm: float, f_coll_mm: float, pixel_um: float, fiber_core_um: float,
+                            m_lo: int, m_hi: int, x_c: float, y_c: float, fiber_height_um: Sequence[float] = (0.0,)) -> dict:
+    """parametric Spectrograph Unit (e2e.h): the arrays of a spectral format from the geometrical parameters of a
+    cross-dispersed echelle spectrograph.  Host call, needs no GPU.  Returns a dict of numpy arrays / floats."""
+    n = int(m_hi) - int(m_lo) + 1
+    hf = _host(fiber_height_um)
+    d = SpectrographDesc(groove_um, blaze_deg, theta_deg, gamma_deg, xd_groove_um, xd_lam_ref, f_cam_mm, f_coll_mm, pixel_um,
+                         fiber_core_um, int(m_lo), int(m_hi), x_c, y_c, int(hf.shape[0]), hf.ctypes.data)
+    arr = {"order_m": np.zeros(max(n, 1), dtype=np.int32)}
+    for k in ("lam_min", "lam_max", "blaze_lam_c", "blaze_amp"):
+        arr[k] = np.zeros(max(n, 1))
+    arr["coef_x"], arr["coef_y"] = np.zeros(36), np.zeros(36)
+    arr["fiber_dx"], arr["fiber_dy"] = np.zeros(hf.shape[0]), np.zeros(hf.shape[0])
+    o = SpectrographFormatDesc()
+    o.capacity_orders = max(n, 1)
+    for k, a in arr.items():
+        setattr(o, k, a.ctypes.data)
+    _check(load().e2e_spectrograph_format(C.byref(d), C.byref(o)))
+    res = {k: a[:o.n_orders] if k in ("order_m", "lam_min", "lam_max", "blaze_lam_c", "blaze_amp") else a for k, a in arr.items()}
+    for k in ("n_orders", "deg_l", "deg_m", "lam0", "inv_dlam", "m0", "inv_dm", "fiber_dx_px", "fiber_dy_px", "residual_x_px",
+              "residual_y_px", "x_min", "x_max", "y_min", "y_max", "tilt_tan", "K", "px_per_radian"):
+        res[k] = getattr(o, k)
+    return res
 
 
 def e2e_plan_check(fmt: Format, psf: Psf) -> dict:

@@ -17,7 +17,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden",
           "-Xptxas", "-v"]
 # per translation unit: extra flags.  detector.cu must not contract a*b+c (bit-exact noise stage, G12).
-UNITS = {"api.cu": [], "peak.cu": [], "detector.cu": ["--fmad=false"]}
+UNITS = {"api.cu": [], "peak.cu": [], "detector.cu": ["--fmad=false"], "spectrograph.cu": []}
 
 
 def _nvcc() -> str:
@@ -31,7 +31,7 @@ def _stale() -> bool:
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime
-    deps = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "e2e.h", Path(__file__)]
+    deps = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + [PKG.parent / "include" / "e2e.h", Path(__file__)]
     return any(d.stat().st_mtime > t for d in deps)
 
 

@@ -892,3 +892,41 @@ def test_schedule_invariants_full_size(B, which):
                 assert r.torch.equal(r.render(), a)
         finally:
             r.close()
+
+
+# ------------------------------------------------------------------------------------------ parametric spectrograph unit
+def test_render_from_the_parametric_spectrograph_unit(B):
+    """S8(f) 4: a frame rendered from a spectral format that e2e_spectrograph_format generated from geometrical
+    parameters (R2 echelle, three orders, a tilted 3-fiber pseudo-slit).  The mapped sample positions follow the oracle's
+    closed-form grating relations within the residual the generator reports, and the frame matches the oracle per pixel"""
+    from oracle import spectrograph as OS
+    kw = dict(groove_um=1000.0 / 52.6, blaze_deg=63.4, theta_deg=0.7, gamma_deg=0.9, xd_groove_um=1000.0 / 300.0, xd_lam_ref=5500.0,
+              f_cam_mm=300.0, f_coll_mm=1200.0, pixel_um=15.0, fiber_core_um=200.0, m_lo=60, m_hi=62, x_c=1024.0, y_c=300.0,
+              fiber_height_um=(-400.0, 0.0, 400.0))
+    g = B.e2e_spectrograph_format(**kw)
+    assert g["residual_x_px"] < 1e-4 and g["residual_y_px"] < 1e-4
+    assert 0 < g["x_min"] and g["x_max"] < 2048 and 0 < g["y_min"] and g["y_max"] < 600
+    rng = np.random.default_rng(61)
+    lam_lo, lam_hi = float(g["lam_min"].min()) - 1.0, float(g["lam_max"].max()) + 1.0
+    flux = 1.0 + 0.5 * rng.random(int((lam_hi - lam_lo) / 0.02) + 2)
+    spectra = [W.Spectrum(flux=flux, lam0=lam_lo, dlam=0.02, scale=sc) for sc in (800.0, 1000.0, 700.0)]
+    s = W.Scene(name="parametric_r2", nx=2048, ny=600, order_m=g["order_m"].copy(), lam_min=g["lam_min"].copy(), lam_max=g["lam_max"].copy(),
+                fiber_dx=g["fiber_dx"].copy(), fiber_dy=g["fiber_dy"].copy(), deg_l=5, deg_m=5, coef_x=g["coef_x"].copy(),
+                coef_y=g["coef_y"].copy(), lam0=g["lam0"], inv_dlam=g["inv_dlam"], m0=g["m0"], inv_dm=g["inv_dm"],
+                blaze_lam_c=g["blaze_lam_c"].copy(), blaze_amp=g["blaze_amp"].copy(), samples_per_px=8.0,
+                psf=W.Psf(kind=0, fiber_dx_px=g["fiber_dx_px"], fiber_dy_px=g["fiber_dy_px"], sigma_x=1.1, sigma_y=1.1), spectra=spectra)
+    p = OS.Spectrograph(**kw)
+    r = B.Renderer(s)
+    try:
+        for o in range(3):
+            lam, x, y, w = r.samples(1, o)                                # the middle fiber sits on the base trace
+            assert np.abs(x - OS.position_x(p, lam, int(g["order_m"][o]))).max() < 1.02 * g["residual_x_px"] + 1e-8
+            assert np.abs(y - OS.position_y(p, lam)).max() < 1.02 * g["residual_y_px"] + 1e-8
+            assert np.array_equal(x, oracle.samples(s, 1, o)[1])
+        G = r.render().cpu().numpy()
+    finally:
+        r.close()
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, "parametric spectrograph unit")
+    assert abs(G.sum() / oracle.total_weight(s) - 1.0) < 1e-12

@@ -135,6 +135,14 @@ static HostPipe* host_pipe()
     return pipes[dev];
 }
 
+e2e_psf::~e2e_psf()
+{
+    if (d_sat) cudaFree(d_sat);
+    if (d_pi) cudaFree(d_pi);
+    if (d_poly) cudaFree(d_poly);
+    if (d_mom) cudaFree(d_mom);
+}
+
 e2e_plan::~e2e_plan()
 {
     if (d_strips) cudaFree(d_strips);
@@ -561,7 +569,7 @@ int e2e_psf_create(e2e_psf_t** out, const e2e_psf_desc_t* d, int32_t nx, int32_t
         }
         E2E_CUDA(cudaMalloc(&P->d_sat, 8 * sat.size()));
         cudaError_t ce = cudaMemcpy(P->d_sat, sat.data(), 8 * sat.size(), cudaMemcpyHostToDevice);
-        if (ce != cudaSuccess) { cudaFree(P->d_sat); return fail_cuda(ce, "psf_create: table upload"); }
+        if (ce != cudaSuccess) { cudaFree(P->d_sat); P->d_sat = nullptr; return fail_cuda(ce, "psf_create: table upload"); }
         T.sat = P->d_sat;
         // production path (render_tabcell.cuh): PI[ry][rx][J][I] = sum of the kernel cells inside the pixel whose
         // lower-left corner is the fine-grid point (os I + rx - os, os J + ry - os), from a long double SAT
@@ -617,15 +625,7 @@ int e2e_psf_info(const e2e_psf_t* psf, int32_t* n_nodes, int32_t* footprint_cols
     return E2E_OK;
 }
 
-void e2e_psf_destroy(e2e_psf_t* psf)
-{
-    if (!psf) return;
-    if (psf->d_sat) cudaFree(psf->d_sat);
-    if (psf->d_pi) cudaFree(psf->d_pi);
-    if (psf->d_poly) cudaFree(psf->d_poly);
-    if (psf->d_mom) cudaFree(psf->d_mom);
-    delete psf;
-}
+void e2e_psf_destroy(e2e_psf_t* psf) { delete psf; }      // ~e2e_psf frees the device tables
 
 }  // extern "C"
 
@@ -1138,24 +1138,16 @@ int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spectrum, i
     const long long N = fmt->nsamp[order_index];
     if (capacity < N) return fail(E2E_ERR_INVALID_ARG, "setup_samples: capacity smaller than the order's sample count");
     if (N == 0) return E2E_OK;
-    // a one-strip launch: the strip table travels through a small device allocation owned by this call's stream order
-    Strip st{0, N};
-    Strip* d_st = nullptr;
-    E2E_CUDA(cudaMalloc(&d_st, sizeof(Strip)));
-    cudaError_t ce = cudaMemcpy(d_st, &st, sizeof(Strip), cudaMemcpyHostToDevice);
-    if (ce != cudaSuccess) { cudaFree(d_st); return fail_cuda(ce, "setup_samples: strip upload"); }
+    // a one-strip launch: the strip travels as a kernel parameter, nothing is allocated and nothing synchronises
     SpectraParam sp;
     memset(&sp, 0, sizeof(sp));
     sp.s[fiber] = *spectrum;
     dim3 grid((unsigned)((N + 255) / 256), 1);
-    setup_samples_kernel<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(fmt->view, sp, d_st, fiber * fmt->view.n_orders + order_index,
-                                                                      d_lam, d_x, d_y, d_w);
+    setup_samples_kernel<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(fmt->view, sp, nullptr, fiber * fmt->view.n_orders + order_index,
+                                                                      d_lam, d_x, d_y, d_w, nullptr, Strip{0, N});
     count_launch();
-    ce = cudaGetLastError();
-    cudaError_t ce2 = cudaStreamSynchronize((cudaStream_t)cuda_stream);
-    cudaFree(d_st);
+    cudaError_t ce = cudaGetLastError();
     if (ce != cudaSuccess) return fail_cuda(ce, "setup_samples_kernel launch");
-    if (ce2 != cudaSuccess) return fail_cuda(ce2, "setup_samples_kernel");
     return E2E_OK;
 }
 

@@ -167,6 +167,7 @@ struct e2e_psf {
     e2e::MomentParam mom;
     double* d_mom = nullptr;       // one allocation: fx then fy
     bool is_map = false;           // analytic PSF map (G21): mom holds one table set per node
+    ~e2e_psf();                    // frees the device tables (also on the early returns of e2e_psf_create)
 };
 
 struct e2e_plan {                  // schedule for one (format, footprint) pair; cached in the format handle

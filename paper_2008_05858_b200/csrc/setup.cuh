@@ -127,11 +127,12 @@ __device__ __forceinline__ double eff_at(const FormatView& f, double lam)
 __global__ void setup_samples_kernel(FormatView f, SpectraParam sp, const Strip* __restrict__ strips,
                                      int strip0, double* __restrict__ out_lam, double* __restrict__ out_x,
                                      double* __restrict__ out_y, double* __restrict__ out_w,
-                                     const int* __restrict__ strip_ids = nullptr)
+                                     const int* __restrict__ strip_ids = nullptr, Strip single = Strip{0, -1})
 {
     int sidx = strip_ids ? strip_ids[blockIdx.y] : strip0 + blockIdx.y;
     int fiber = sidx / f.n_orders, o = sidx - fiber * f.n_orders;
-    Strip st = strips[strip_ids ? sidx : blockIdx.y];
+    // single.n >= 0: a one-strip launch whose strip travels as a kernel parameter (e2e_setup_samples: no device table)
+    Strip st = single.n >= 0 ? single : strips[strip_ids ? sidx : blockIdx.y];
     long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= st.n) return;
     double lam, X, Y;

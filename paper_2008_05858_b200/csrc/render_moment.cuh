@@ -240,8 +240,9 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
         const int nb = (int)min((long long)32, kend - k);
         const bool valid = lane < nb;
         const long long kidx = st.off + k + (valid ? lane : nb - 1);
-        const double xk = xs[kidx], yk = ys[kidx];
-        const double wk = valid ? ws[kidx] : 0.0;
+        // streamed once: evict-first loads keep the L1 for the tables
+        const double xk = __ldcs(xs + kidx), yk = __ldcs(ys + kidx);
+        const double wk = valid ? __ldcs(ws + kidx) : 0.0;
         // G9 footprint box (same operations as the oracle's box)
         const int ilo = __double2int_ru(__dsub_rn(xk, Q.hbx)), ihi = __double2int_rd(__dadd_rn(xk, Q.hbx));
         const int jlo = __double2int_ru(__dsub_rn(yk, Q.hby)), jhi = __double2int_rd(__dadd_rn(yk, Q.hby));

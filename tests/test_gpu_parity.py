@@ -333,6 +333,12 @@ def test_render_espresso_full_frame_windows(B, espresso_gpu):
             k = int(frac * (n - 1))
             lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
             wins.append((max(0, int(x[0]) - 24), max(0, int(y[0]) - 20), 48, 40))
+    # windows centred on the Fabry-Perot fiber (fiber 1), on one of its lines: found from the oracle's own weights
+    for o in (17, 63):
+        lam, x, y, w = oracle.samples(s, 1, o)
+        k = int(np.argmax(w[len(w) // 3:]) + len(w) // 3)
+        assert w[k] > 0
+        wins.append((max(0, int(x[k]) - 24), max(0, int(y[k]) - 20), 48, 40))
     worst = 0.0
     for (i0, j0, wnx, wny) in wins:
         O = oracle.render(s, window=(i0, j0, wnx, wny))
@@ -373,7 +379,7 @@ def test_render_hires_full_frame_windows(B):
     s = W.hires_like()
     G = gpu_render(B, s)
     assert np.isfinite(G).all()
-    for o, f, frac in ((0, 0, 0.0008), (30, 4, 0.41), (59, 9, 0.9992)):
+    for o, f, frac in ((0, 0, 0.0008), (30, 4, 0.41), (59, 9, 0.9992), (12, 9, 0.27), (45, 0, 0.66), (58, 5, 0.05)):
         n = oracle.order_nsamples(s, o)
         k = int(frac * (n - 1))
         lam, x, y, w = oracle.samples(s, f, o, k, k + 1)
@@ -442,11 +448,10 @@ def test_render_tabulated_steep_trace_and_fibers(B):
 
 def test_render_field_psf_full_frame_windows(B):
     """BASELINE.json configs[3] at full size; oracle on sampled windows"""
-    base = W.espresso_like(n_obj_lines=500, table_dlam=0.005)
-    s = W.field_psf(base=base)
+    s = W.field_psf()                                             # the scene bench.py --workload field_psf times
     G = gpu_render(B, s)
     assert np.isfinite(G).all()
-    for o, frac in ((0, 0.3), (42, 0.77), (84, 0.5)):
+    for o, frac in ((0, 0.3), (42, 0.77), (84, 0.5), (21, 0.0007), (66, 0.9993)):
         n = oracle.order_nsamples(s, o)
         k = int(frac * (n - 1))
         lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)

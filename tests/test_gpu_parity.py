@@ -935,3 +935,64 @@ def test_render_from_the_parametric_spectrograph_unit(B):
     assert O.max() > 0
     assert_frame_parity(G, O, "parametric spectrograph unit")
     assert abs(G.sum() / oracle.total_weight(s) - 1.0) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------ degenerate inputs
+def test_degenerate_inputs_and_limits(B):
+    """edge cases of the boundary (include/e2e.h): orders wholly off the detector, an order of a single sample, 64 fibers (the
+    limit) and 65 (refused), PSFs beyond the footprint / chord-order limits (refused), NaN parameters (refused), a misaligned
+    workspace (refused), zero frames in a batch (refused) -- and the frames that ARE rendered match the oracle"""
+    import torch
+    # (1) one order on the detector, one wholly below it, one reduced to a single sample
+    s = small_tiny(spp=4.0, lam=(5010.0, 5012.0))
+    s.order_m = np.array([100, 101, 102], dtype=np.int32)
+    s.lam_min = np.array([5010.0, 5010.0, 5011.0]); s.lam_max = np.array([5012.0, 5012.0, 5011.0 + 1e-5])
+    s.blaze_lam_c = np.array([5025.0, 5025.0, 5025.0]); s.blaze_amp = np.ones(3)
+    s.deg_m = 1
+    s.coef_x = np.array([1024.0, 0.0, 1000.0, 0.0, 1.0, 0.0, 0.0, 0.0])
+    s.coef_y = np.array([100.0, 900.0, 10.0, 0.0, 0.0, 0.0, 0.0, 0.0])        # m = 101 lands on row 1000 of a 256-row detector
+    s.m0, s.inv_dm = 100.0, 1.0
+    assert oracle.order_nsamples(s, 2) == 1
+    G, O = gpu_render(B, s), oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, "off-detector order + single-sample order")
+    # (2) 64 fibers render, 65 are refused
+    s = small_tiny(spp=2.0, lam=(5010.0, 5010.5))
+    s.fiber_dx = np.linspace(-1.0, 1.0, 64); s.fiber_dy = np.linspace(-100.0, 100.0, 64)
+    s.spectra = [s.spectra[0]] * 64
+    assert_frame_parity(gpu_render(B, s), oracle.render(s), "64 fibers")
+    s.fiber_dx = np.zeros(65); s.fiber_dy = np.zeros(65); s.spectra = [s.spectra[0]] * 65
+    with pytest.raises(B.E2EError) as ei:
+        B.Format(s)
+    assert ei.value.code == -5
+    # (3) PSF limits and bad parameters
+    base = small_tiny(spp=2.0)
+    for kw, code in ((dict(fiber_dx_px=3.0, fiber_dy_px=3.0, sigma_x=7.0, sigma_y=1.0), -5),          # footprint > 96 px
+                     (dict(fiber_dx_px=3.0, fiber_dy_px=3.0, sigma_x=1.0, sigma_y=1.0, n_nodes=65), -5),
+                     (dict(fiber_dx_px=3.0, fiber_dy_px=3.0, sigma_x=float("nan"), sigma_y=1.0), -1),
+                     (dict(fiber_dx_px=-1.0, fiber_dy_px=3.0, sigma_x=1.0, sigma_y=1.0), -1),
+                     (dict(fiber_dx_px=3.0, fiber_dy_px=3.0, sigma_x=0.0, sigma_y=1.0), -1)):
+        with pytest.raises(B.E2EError) as ei:
+            B.Psf(with_psf(base, **kw).psf, base.nx, base.ny)
+        assert ei.value.code == code, kw
+    bad = copy.copy(base); bad.coef_x = base.coef_x.copy(); bad.coef_x[1] = np.inf
+    with pytest.raises(B.E2EError):
+        B.Format(bad)
+    # (4) workspace misaligned / batch of zero frames / spectrum descriptor with a non-positive step
+    r = B.Renderer(base)
+    try:
+        fr = torch.empty((base.ny, base.nx), dtype=torch.float64, device="cuda")
+        with pytest.raises(B.E2EError) as ei:
+            B.e2e_render_frame(r.fmt, r.psf, r.spectra, fr, False, r.workspace[8:])
+        assert ei.value.code == -6
+        with pytest.raises(B.E2EError):
+            B.e2e_render_frames_workspace_bytes(r.fmt, r.psf, 0)
+        d = B.spectra_array(base.spectra, [t.data_ptr() for t in r.flux])
+        d[0].dlam = 0.0
+        with pytest.raises(B.E2EError) as ei:
+            B.e2e_render_frame(r.fmt, r.psf, d, fr, False, r.workspace)
+        assert ei.value.code == -1
+        # the handle still renders after the refused calls
+        assert_frame_parity(r.render().cpu().numpy(), oracle.render(base), "after refused calls")
+    finally:
+        r.close()

@@ -208,8 +208,10 @@ E2E_API int e2e_setup_samples(const e2e_format_t* fmt, const e2e_spectrum_t* spe
  * (a cudaStream_t, NULL = default stream); launch errors are returned, later device faults surface at the
  * caller's next synchronisation.  The call allocates nothing on the device except, the first time a
  * (format, psf) pair is seen, the cached schedule (a few hundred KB). 
- * Part of the work is enqueued on a stream owned by the library that forks from and joins cuda_stream (two row bands
- * that share no pixel are rendered concurrently); to the caller the call is ordered on cuda_stream as a whole. */
+ * The analytic PSF under dense sampling renders with ONE kernel launch on cuda_stream.  The other kernels (sparse sampling,
+ * sigma < ~0.3 px, tabulated PSF) enqueue part of their launches on a stream owned by the (format, psf) pair that forks from
+ * and joins cuda_stream (two row bands that share no pixel are rendered concurrently); to the caller the call is ordered on
+ * cuda_stream as a whole, and renders of different pairs never wait on each other's forked work. */
 E2E_API int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                      double* d_frame, int32_t accumulate, void* d_workspace, size_t workspace_bytes,
                      void* cuda_stream);
@@ -236,7 +238,7 @@ E2E_API int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int
  * cuda_stream, odd bands on a second stream owned by the library, and as soon as a band is done a6 runs on its rows
  * and they travel to the host on the library's copy stream.  The frame is bit-reproducible call to call; against
  * e2e_render_frame it can differ in the last bit where strips overlap (the additions happen band by band).  Calls
- * on one device are serialised. */
+ * on one (format, psf) pair are serialised. */
 E2E_API int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
                                     size_t* bytes);
 struct e2e_detector;

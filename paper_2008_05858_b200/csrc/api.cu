@@ -101,38 +101,38 @@ static double host_x_of_lambda(const e2e_format_desc_t& d, int o, double lam)
 
 using namespace e2e;
 
-// copy stream + events of the banded host path; created on first use, one per device (kept until exit)
+// second compute stream, copy stream and events of one plan (fork / join around the caller's stream); created on first use
 struct HostPipe {
     static constexpr int kEvents = 16;
     cudaStream_t copy = nullptr;
     cudaStream_t aux = nullptr;        // second compute stream: odd bands render here while even bands render on the caller's
-    cudaStream_t aux2[2] = {};         // device path with 3 / 4 concurrent parts
-    cudaEvent_t ev_aux2_done[2] = {};
     cudaEvent_t ev[kEvents] = {};
     cudaEvent_t ev_start = nullptr, ev_aux_done = nullptr;
-    std::mutex mu;
+    std::mutex mu;                     // one call at a time enqueues on these streams
+    ~HostPipe()
+    {
+        if (copy) cudaStreamDestroy(copy);
+        if (aux) cudaStreamDestroy(aux);
+        for (cudaEvent_t e : ev)
+            if (e) cudaEventDestroy(e);
+        if (ev_start) cudaEventDestroy(ev_start);
+        if (ev_aux_done) cudaEventDestroy(ev_aux_done);
+    }
 };
-static HostPipe* host_pipe()
+static HostPipe* host_pipe(e2e_plan* pl)
 {
-    static std::mutex mu;
-    static HostPipe* pipes[64] = {};
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
-    std::lock_guard<std::mutex> lk(mu);
-    if (!pipes[dev]) {
+    std::lock_guard<std::mutex> lk(pl->pipe_mu);
+    if (!pl->pipe) {
         HostPipe* h = new HostPipe;
         bool ok = cudaStreamCreateWithFlags(&h->copy, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaStreamCreateWithFlags(&h->aux, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) == cudaSuccess &&
                   cudaEventCreateWithFlags(&h->ev_aux_done, cudaEventDisableTiming) == cudaSuccess;
-        for (int i = 0; ok && i < 2; ++i)
-            ok = cudaStreamCreateWithFlags(&h->aux2[i], cudaStreamNonBlocking) == cudaSuccess &&
-                 cudaEventCreateWithFlags(&h->ev_aux2_done[i], cudaEventDisableTiming) == cudaSuccess;
         for (int i = 0; ok && i < HostPipe::kEvents; ++i) ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { delete h; return nullptr; }
-        pipes[dev] = h;
+        pl->pipe = h;
     }
-    return pipes[dev];
+    return static_cast<HostPipe*>(pl->pipe);
 }
 
 e2e_psf::~e2e_psf()
@@ -145,6 +145,7 @@ e2e_psf::~e2e_psf()
 
 e2e_plan::~e2e_plan()
 {
+    delete static_cast<HostPipe*>(pipe);
     if (d_strips) cudaFree(d_strips);
     if (d_items) cudaFree(d_items);
     if (d_dep_off) cudaFree(d_dep_off);
@@ -1189,7 +1190,7 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
         StageTimer tm(kStageRender, stream);
         const long long before = g_launches.load();
         const int nparts = persistent ? 1 : pl->halves.n_bands;
-        HostPipe* hp = nparts >= 2 ? host_pipe() : nullptr;
+        HostPipe* hp = nparts >= 2 ? host_pipe(pl) : nullptr;
         if (hp) {
             // phase-launched kernels: two row bands that share no pixel, rendered concurrently: the tail of one band's launch
             // (a few long items on otherwise idle SMs) overlaps the other band's work.  Fork to the library's stream and join.
@@ -1385,7 +1386,7 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
         if (det) return launch_detector(d_frame + off, d_frame + off, n, *det, cs, (long long)off);
         return E2E_OK;
     };
-    HostPipe* hp = host_pipe();
+    HostPipe* hp = host_pipe(pl);
     const e2e_plan::BandPart& part = out16 ? pl->host16 : pl->host;   // the 2-byte output travels 4x faster: fewer, larger bands
     if (part.n_bands <= 1 || !hp) {
         // one pass: render, detector, copy

@@ -204,6 +204,10 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     };
     BandPart host, halves, host16;     // host16: fewer, equal bands for the host path's uint16 output (short copies)
     int n_phases_all = 0;          // phases before empty ones were dropped (colour x class)
+    // streams and events the library adds to the caller's stream (second compute stream, copy stream of the host path): owned by
+    // the plan, so renders of different (format, psf) pairs never wait on each other's forked work; created on first use
+    void* pipe = nullptr;
+    std::mutex pipe_mu;
     ~e2e_plan();
 };
 

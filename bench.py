@@ -488,6 +488,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     burst, sustained = B.e2e_measure_fp64_peak(80)
     peak_tf, burst_tf = 2.0 * sustained / 1e12, 2.0 * burst / 1e12
     stages = stage_rooflines(m, args.workload, peak_tf, burst_tf)
+    if "render" in stages:
+        stages["render"]["fp64_pipe_probe"] = B.e2e_probe_fp64_pipe()        # why the mix stops short of the peak
     if args.others and world == 1 and nbatch == 1:
         for name in ("tiny", "espresso_like", "hires_like", "field_psf", "rv_sweep"):
             if name == args.workload:

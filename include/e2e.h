@@ -324,6 +324,14 @@ E2E_API int e2e_apply_detector_adu16(const double* d_frame_in, uint16_t* d_frame
  * launch, *sustained = total work / total time of the second half of the launches.  Synchronous. */
 E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s);
 
+/* Probes of one SM's FP64 pipe under the render kernel's instruction mix; results6[0] cycles per
+ * mma.sync.m8n8k4.f64 (DMMA) in one dependent accumulator chain, [1] cycles per DMMA with two independent chains in one warp
+ * (= the issue interval: one warp can keep its scheduler's pipe busy), [2] DMMAs per clock and SM with 16 DMMA warps (0.25 =
+ * 64 fused multiply-adds per clock), [3] scalar DFMA warp instructions per clock and SM from 4 warps of independent chains
+ * alone, [4] from the same 4 warps while 16 DMMA warps run next to them (scalar fp64 starves behind a saturated pipe),
+ * [5] what the DMMA warps got in that mix.  Synchronous, a few milliseconds. */
+E2E_API int e2e_probe_fp64_pipe(double* results6);
+
 /* Which a4+a5 kernel e2e_render_frame launches for this (format, psf) pair and what it executes: *name is a static
  * string ("render_moment_kernel<2>", "render_poly_kernel<14>", "render_analytic_kernel", "render_tabulated_kernel");
  * *executed_fma_per_cell / *executed_fma_per_sample are the fp64 fused multiply-adds the kernel issues per footprint

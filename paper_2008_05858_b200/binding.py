@@ -26,7 +26,7 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_apply_detector_adu16", "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
            "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames",
-           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check", "e2e_spectrograph_format"]
+           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check", "e2e_spectrograph_format", "e2e_probe_fp64_pipe"]
 
 
 class E2EError(RuntimeError):
@@ -153,6 +153,8 @@ def load():
     L.e2e_apply_detector_adu16.argtypes = [vp, vp, i32, i32, C.POINTER(DetectorExDesc), vp]
     L.e2e_measure_fp64_peak.restype = C.c_int
     L.e2e_measure_fp64_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
+    L.e2e_probe_fp64_pipe.restype = C.c_int
+    L.e2e_probe_fp64_pipe.argtypes = [C.POINTER(dbl)]
     L.e2e_render_kernel_info.restype = C.c_int
     L.e2e_render_kernel_info.argtypes = [vp, vp, C.POINTER(C.c_char_p), C.POINTER(dbl), C.POINTER(dbl)]
     L.e2e_render_frames_workspace_bytes.restype = C.c_int
@@ -444,6 +446,14 @@ def e2e_measure_fp64_peak(repeats: int = 60):
     burst, sus = C.c_double(), C.c_double()
     _check(load().e2e_measure_fp64_peak(int(repeats), C.byref(burst), C.byref(sus)))
     return float(burst.value), float(sus.value)
+
+
+def e2e_probe_fp64_pipe() -> dict:
+    """probes of one SM's FP64 pipe (e2e.h): DMMA latency / issue interval, DMMA and scalar DFMA rates alone and mixed"""
+    r = (C.c_double * 6)()
+    _check(load().e2e_probe_fp64_pipe(r))
+    return {"dmma_cycles_dependent_chain": r[0], "dmma_cycles_two_chains": r[1], "dmma_per_clk_sm_alone": r[2],
+            "dfma_per_clk_sm_alone": r[3], "dfma_per_clk_sm_next_to_dmma": r[4], "dmma_per_clk_sm_in_mix": r[5]}
 
 
 def e2e_render_kernel_info(fmt, psf) -> dict:

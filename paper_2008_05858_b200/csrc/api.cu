@@ -34,6 +34,7 @@ int launch_detector(const double* d_in, double* d_out, long long n, const e2e_de
 int launch_detector_ex(const double* d_in, void* d_out, bool out16, long long n, int nx, const e2e_detector_ex_t& det,
                        cudaStream_t stream, long long p0 = 0);
 int measure_fp64_peak(int repeats, double* burst, double* sustained);
+int probe_fp64_pipe(double* r);
 
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
@@ -1669,6 +1670,12 @@ int e2e_render_algorithmic_fma(const e2e_format_t* fmt, const e2e_psf_t* psf, do
 int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, double* sustained_dfma_per_s)
 {
     return measure_fp64_peak(repeats, burst_dfma_per_s, sustained_dfma_per_s);
+}
+
+int e2e_probe_fp64_pipe(double* results6)
+{
+    if (!results6) return fail(E2E_ERR_INVALID_ARG, "probe_fp64_pipe: NULL argument");
+    return probe_fp64_pipe(results6);
 }
 
 int e2e_profile_enable(int32_t on)

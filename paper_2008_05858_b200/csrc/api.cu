@@ -7,6 +7,7 @@
 #include "render_poly.cuh"
 #include "render_moment.cuh"
 #include "plan_check.cuh"
+#include "render_cells.cuh"
 #include "poly_tables.h"
 
 #include <algorithm>
@@ -39,6 +40,9 @@ int probe_fp64_pipe(double* r);
 // samples per pixel from which the per-cell moment kernel beats the per-sample polynomial kernel
 constexpr double kMomentMinSpp = 8.0;
 constexpr long long kSmallFrameItems = 4736;   // 2 x (148 SMs x 16 resident warps): below this a K = 2 schedule leaves the GPU idle
+#ifndef E2E_SPLIT
+#define E2E_SPLIT 1                    // 1: e2e_render_frame renders the analytic PSF with the two kernels of render_cells.cuh
+#endif
 constexpr int kDeviceParts = 2;        // row bands e2e_render_frame renders concurrently (they share no pixel)
 #ifndef E2E_HOST_BANDS
 #define E2E_HOST_BANDS 8
@@ -154,6 +158,7 @@ e2e_plan::~e2e_plan()
     if (d_succ_off) cudaFree(d_succ_off);
     if (d_succ_idx) cudaFree(d_succ_idx);
     if (d_ctrl_init) cudaFree(d_ctrl_init);
+    if (d_cell_off) cudaFree(d_cell_off);
     for (BandPart* bp : {&host, &halves, &host16}) {
         if (bp->d_items) cudaFree(bp->d_items);
         if (bp->d_strips) cudaFree(bp->d_strips);
@@ -641,10 +646,12 @@ struct Interval { int lo, hi, strip; };
 static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
 {
     std::lock_guard<std::mutex> lock(F->plan_mu);
+    // the cell ranges of the two-kernel render depend on the y-phase windows of the PSF's tables as well
+    const int nyb_key = (P->kind == 0 && P->moment_npt > 0 && !P->is_map) ? P->mom.nyb : 0;
     for (auto& p : F->plans)
-        if (p->hbx == P->hbx && p->hby == P->hby) { *out = p.get(); return E2E_OK; }
+        if (p->hbx == P->hbx && p->hby == P->hby && p->nyb == nyb_key) { *out = p.get(); return E2E_OK; }
     std::unique_ptr<e2e_plan> pl(new e2e_plan);
-    pl->hbx = P->hbx; pl->hby = P->hby;
+    pl->hbx = P->hbx; pl->hby = P->hby; pl->nyb = nyb_key;
     const int no = F->view.n_orders, nf = F->view.n_fibers, nx = F->view.nx;
     const int n_strips = no * nf;
     if (n_strips > 65535) return fail(E2E_ERR_UNSUPPORTED, "render: more than 65535 (fiber, order) strips");
@@ -838,6 +845,31 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
     E2E_CUDA(cudaMemcpy(pl->d_strips, pl->strips.data(), sizeof(Strip) * n_strips, cudaMemcpyHostToDevice));
     E2E_CUDA(cudaMalloc(&pl->d_items, sizeof(Item) * std::max<size_t>(1, flat.size())));
     if (!flat.empty()) E2E_CUDA(cudaMemcpy(pl->d_items, flat.data(), sizeof(Item) * flat.size(), cudaMemcpyHostToDevice));
+    // ---- cells of every item (two-kernel render): the render's own cell walk, positions straight from the format
+    if (nyb_key > 0 && !flat.empty()) {
+        const int ni = (int)flat.size();
+        int* d_counts = nullptr;
+        E2E_CUDA(cudaMalloc(&d_counts, sizeof(int) * ni));
+        CellStore none;
+        memset(&none, 0, sizeof(none));
+        static SpectraParam no_spectra;
+        const unsigned blocks = (unsigned)((ni + kCellWarps - 1) / kCellWarps);
+        switch (P->moment_npt) {
+            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+        }
+        count_launch();
+        std::vector<int> counts(ni);
+        cudaError_t ce = cudaMemcpy(counts.data(), d_counts, sizeof(int) * ni, cudaMemcpyDeviceToHost);
+        cudaFree(d_counts);
+        if (ce != cudaSuccess) return fail_cuda(ce, "render: cell count");
+        std::vector<long long> off(ni + 1, 0);
+        for (int i = 0; i < ni; ++i) off[i + 1] = off[i] + counts[i];
+        pl->n_cells = off[ni];
+        E2E_CUDA(cudaMalloc(&pl->d_cell_off, sizeof(long long) * (ni + 1)));
+        E2E_CUDA(cudaMemcpy(pl->d_cell_off, off.data(), sizeof(long long) * (ni + 1), cudaMemcpyHostToDevice));
+    }
     // ---- row bands: strips sorted by their first row, split into bands by sample count, bands starting only at gaps
     {
         const int ny = F->view.ny;
@@ -989,6 +1021,21 @@ static bool choose_tabcell(const e2e_psf* P) { return P->kind == 1 && P->tab.pi 
 // control block of the persistent render launch: kCtrlHeads head counters + one flag per item (zeroed before the launch)
 static size_t ctrl_bytes(const e2e_plan* pl) { return align_up(sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)), 256); }
 
+// two-kernel render (render_cells.cuh): is it the path of this pair, and the bytes of its per-cell records in the workspace
+static bool use_split(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl)
+{
+    return E2E_SPLIT != 0 && choose_moment(F, P) && !P->is_map && pl->d_cell_off != nullptr && pl->n_cells > 0;
+}
+static size_t cell_hdr_bytes(const e2e_plan* pl) { return align_up(sizeof(CellHeader) * (size_t)std::max<long long>(pl->n_cells, 1), 256); }
+static size_t cell_mom_bytes(const e2e_plan* pl, const e2e_psf* P)
+{
+    return align_up(sizeof(double) * 64 * (size_t)P->moment_npt * (size_t)std::max<long long>(pl->n_cells, 1), 256);
+}
+static size_t cell_bytes(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl)
+{
+    return use_split(F, P, pl) ? cell_hdr_bytes(pl) + cell_mom_bytes(pl, P) : 0;
+}
+
 // (re)initialise a control block in the caller's workspace for one launch: head counters 0, dependency counters from the plan
 static cudaError_t ctrl_reset(const e2e_plan* pl, unsigned* ctrl, cudaStream_t stream)
 {
@@ -1125,7 +1172,7 @@ int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, si
     e2e_plan* pl = nullptr;
     int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
-    *bytes = 3 * sample_array_bytes(pl->total_samples) + ctrl_bytes(pl);
+    *bytes = 3 * sample_array_bytes(pl->total_samples) + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl);
     return E2E_OK;
 }
 
@@ -1166,7 +1213,7 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     if (rc) return rc;
     const size_t per = sample_array_bytes(pl->total_samples);
     if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace NULL or not 256-byte aligned");
-    if (workspace_bytes < 3 * per + ctrl_bytes(pl)) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
+    if (workspace_bytes < 3 * per + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     double* d_x = (double*)d_workspace;
     double* d_y = (double*)((char*)d_workspace + per);
@@ -1183,7 +1230,7 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
         StageTimer tm(kStageSetup, stream);
         const long long before = g_launches.load();
         if (persistent) E2E_CUDA(ctrl_reset(pl, qs.ctrl, stream));
-        rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
+        if (!use_split(fmt, psf, pl)) rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);   // the two-kernel path fuses a1-a3
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
         if (rc) return rc;
     }
@@ -1208,6 +1255,36 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
             ce = cudaEventRecord(hp->ev_aux_done, hp->aux);
             if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, hp->ev_aux_done, 0);
             if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: join");
+        } else if (use_split(fmt, psf, pl)) {
+            // two kernels (render_cells.cuh): every cell's moments in any order, then the contraction under the ticket queue
+            CellStore cs;
+            cs.cell_off = pl->d_cell_off;
+            cs.hdr = (CellHeader*)((char*)qs.ctrl + ctrl_bytes(pl));
+            cs.mom = (double*)((char*)cs.hdr + cell_hdr_bytes(pl));
+            QueueParam W;
+            memset(&W, 0, sizeof(W));
+            W.n = pl->n_items; W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
+            W.ctrl = qs.ctrl;
+            const unsigned ab = (unsigned)((pl->n_items + kCellWarps - 1) / kCellWarps);
+            SpectraParam sp_call;                                // a1-a3 run inside cell_moment_kernel: no setup launch on this path
+            memset(&sp_call, 0, sizeof(sp_call));
+            for (int f = 0; f < fmt->view.n_fibers; ++f) sp_call.s[f] = spectra[f];
+#define E2E_SPLIT_CASE(NPT)                                                                                                     \
+    case NPT: {                                                                                                                 \
+        const size_t sm = sizeof(MomentWarpSmem<NPT, false>) * kCellWarps;                                                      \
+        cell_moment_kernel<NPT, false, true><<<ab, kCellWarps * 32, sm, stream>>>(nullptr, nullptr, nullptr, pl->d_strips,       \
+                                                                                  pl->d_items, pl->n_items, psf->mom, cs,       \
+                                                                                  nullptr, fmt->view, sp_call);                 \
+        cell_flush_kernel<NPT><<<(unsigned)pl->n_items, 32, 0, stream>>>(W, psf->mom, cs, d_frame, fmt->view.nx, fmt->view.ny);  \
+    } break;
+            switch (psf->moment_npt) {
+                E2E_SPLIT_CASE(2) E2E_SPLIT_CASE(3) E2E_SPLIT_CASE(4)
+                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+            }
+#undef E2E_SPLIT_CASE
+            count_launch(2);
+            cudaError_t ce = cudaGetLastError();
+            if (ce != cudaSuccess) return fail_cuda(ce, "cell_moment_kernel / cell_flush_kernel launch");
         } else {
             rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, qs);
         }

@@ -172,6 +172,9 @@ struct e2e_psf {
 
 struct e2e_plan {                  // schedule for one (format, footprint) pair; cached in the format handle
     double hbx, hby;
+    int nyb = 0;                   // y-phase windows of the PSF's moment tables the cell ranges below were counted for (0: none)
+    long long n_cells = 0;         // footprint cells of the whole frame
+    long long* d_cell_off = nullptr;   // [n_items + 1] first cell of every item (two-kernel render, render_cells.cuh)
     int win_cols, win_rows;        // window capacity the schedule was built for
     int n_strips = 0;
     long long total_samples = 0;

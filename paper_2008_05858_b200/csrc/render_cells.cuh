@@ -1,0 +1,206 @@
+// render_cells.cuh -- the cell-moment render in two kernels (round 2).
+//
+// render_moment_kernel does everything for a cell in one warp: batch prologue (sample loads, footprint boxes, phase powers),
+// step 1 (the cell's weighted phase moments M), steps 2 + 3 (the contraction with the pixel-phase tables) and the write-out.
+// On sm_100a the scalar fp64 instructions of one warp's prologue STARVE while other warps of its scheduler stream DMMAs
+// (e2e_probe_fp64_pipe: 0.0008 instead of 1.22 warp instructions per clock), so the prologues and the contraction do not
+// overlap the way five warps per scheduler suggest.  Here the two halves run as two kernels:
+//
+//   cell_moment_kernel  prologue + step 1 for every cell of every item, in any order (a cell's moments depend on nothing but
+//                       its own samples); writes per cell a 32-byte header (footprint box, y-phase window) and the moment
+//                       tiles in DMMA fragment order (32 lanes x 2 NPT doubles: 1 KB for NPT = 2) to the workspace.
+//                       COUNT = true: the same walk without arithmetic, counting the cells of each item (once per plan).
+//   cell_flush_kernel   steps 2 + 3 + a5 for the cells of an item in order, under the ticket queue and dependency counters of
+//                       render_moment.cuh: DMMAs, table loads and the frame reductions only -- no scalar fp64 at all.
+//
+// The cell walk (where a cell ends) and the arithmetic are those of render_moment_kernel, operation for operation, so the frame
+// has the same bits; tests compare the two paths with torch.equal (the batch call still runs the one-kernel path).
+#pragma once
+#include "common.cuh"
+#include "render_moment.cuh"
+
+namespace e2e {
+
+constexpr int kCellWarps = 4;          // warps per CTA of cell_moment_kernel (one item per warp)
+
+struct CellHeader {                    // 32 bytes
+    int i0, i1, j0, j1;                // footprint box of the cell (G9)
+    int yb;                            // y-phase window
+    int pad[3];
+};
+
+// per-item cell ranges and the record arrays in the workspace
+struct CellStore {
+    const long long* cell_off;         // [n_items + 1] first cell of every item (from the counting pass of the plan)
+    CellHeader* hdr;                   // [n_cells]
+    double* mom;                       // [n_cells][32 lanes][2 NPT]
+};
+
+// FUSED: steps a1-a3 run here (setup.cuh's device functions: the oracle's operation sequence, the same bits as
+// setup_samples_kernel) and the samples are never materialised; else they are read from the arrays setup_samples_kernel wrote
+template <int NPT, bool COUNT, bool FUSED>
+__global__ void __launch_bounds__(kCellWarps * 32)
+cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
+                   const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q, CellStore C,
+                   int* __restrict__ counts, const __grid_constant__ FormatView F, const __grid_constant__ SpectraParam SP)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int item_id = blockIdx.x * kCellWarps + warp;
+    if (item_id >= n_items) return;
+    MomentWarpSmem<NPT, false>& S = reinterpret_cast<MomentWarpSmem<NPT, false>*>(smem_raw)[warp];
+    const int lq = lane >> 2, lr = lane & 3;
+    constexpr int NP = 8 * NPT;
+    const double ywin = 1.0 / (double)Q.nyb;
+    const Item it = items[item_id];
+    const Strip st = strips[it.strip];
+    long long k = (long long)it.chunk0 * 32;
+    long long kend = k + (long long)it.nchunks * 32;
+    if (kend > st.n) kend = st.n;
+
+    double mt[NPT][2];
+    bool have = false;
+    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;
+    double cYc = 0.0;
+    long long cell = COUNT ? 0 : C.cell_off[item_id];
+    int n_cells = 0;
+
+    // the open cell is complete: hand it to the flush kernel
+    auto emit = [&]() {
+        if (!COUNT) {
+            if (lane == 0) {
+                CellHeader h;
+                h.i0 = cI0; h.i1 = cI1; h.j0 = cJ0; h.j1 = cJ1; h.yb = cYb; h.pad[0] = h.pad[1] = h.pad[2] = 0;
+                C.hdr[cell] = h;
+            }
+            double* dst = C.mom + ((size_t)cell * 32 + lane) * (2 * NPT);
+#pragma unroll
+            for (int qt = 0; qt < NPT; ++qt) *reinterpret_cast<double2*>(dst + 2 * qt) = make_double2(mt[qt][0], mt[qt][1]);
+            cell += 1;
+        }
+        n_cells += 1;
+    };
+
+    while (k < kend) {
+        const int nb = (int)min((long long)32, kend - k);
+        const bool valid = lane < nb;
+        double xk, yk, wk = 0.0;
+        if (COUNT || FUSED) {
+            // positions straight from the format (a1, a3: the setup kernel's operations, so the cells are the render's)
+            const int fiber = it.strip / F.n_orders, o = it.strip - fiber * F.n_orders;
+            double lam, X, Y;
+            sample_position_fast(F, o, k + (valid ? lane : nb - 1), lam, X, Y);
+            xk = __dadd_rn(X, F.fiber_dx[fiber]);
+            yk = __dadd_rn(Y, F.fiber_dy[fiber]);
+            if (FUSED && !COUNT) {                              // a2: the photon weight, setup_samples_kernel's expression
+                const e2e_spectrum_t& sf = SP.s[fiber];
+                const double wv = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(sf.scale, spectrum_at(sf, lam)), blaze_at(F, o, lam)),
+                                                      eff_at(F, lam)), F.dl[o]);
+                wk = valid ? wv : 0.0;
+            }
+        } else {
+            const long long kidx = st.off + k + (valid ? lane : nb - 1);
+            xk = __ldcs(xs + kidx); yk = __ldcs(ys + kidx);
+            wk = valid ? __ldcs(ws + kidx) : 0.0;
+        }
+        // G9 footprint box (same operations as the oracle's box)
+        const int ilo = __double2int_ru(__dsub_rn(xk, Q.hbx)), ihi = __double2int_rd(__dadd_rn(xk, Q.hbx));
+        const int jlo = __double2int_ru(__dsub_rn(yk, Q.hby)), jhi = __double2int_rd(__dadd_rn(yk, Q.hby));
+        const double dx = __dsub_rn(__dsub_rn(xk, (double)ilo), Q.c0x);
+        const double dy = __dsub_rn(__dsub_rn(yk, (double)jlo), Q.c0y);
+        if (!COUNT) {
+            __syncwarp();                                      // previous batch's readers are done
+            double v[NP];
+            v[0] = wk;
+            double sq = dx;
+#pragma unroll
+            for (int h = 1; h < NP; h *= 2) {
+#pragma unroll
+                for (int p = 0; p < h; ++p)
+                    if (h + p < NP) v[h + p] = v[p] * sq;
+                sq *= sq;
+            }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) S.vx[p * kMomLdk + lane] = v[p];
+            __syncwarp();
+        }
+        int pos = 0;
+        while (pos < nb) {
+            const int kI0 = __shfl_sync(0xffffffffu, ilo, pos), kI1 = __shfl_sync(0xffffffffu, ihi, pos);
+            const int kJ0 = __shfl_sync(0xffffffffu, jlo, pos), kJ1 = __shfl_sync(0xffffffffu, jhi, pos);
+            const double kdy = __shfl_sync(0xffffffffu, dy, pos);
+            if (have && (kI0 != cI0 || kI1 != cI1 || kJ0 != cJ0 || kJ1 != cJ1 || !(fabs(kdy - cYc) <= ywin))) {
+                emit();
+                have = false;
+            }
+            if (!have) {
+                have = true;
+                cI0 = kI0; cI1 = kI1; cJ0 = kJ0; cJ1 = kJ1;
+                cYb = min(max((int)floor((kdy + 0.5) * (double)Q.nyb), 0), Q.nyb - 1);
+                cYc = ((double)cYb + 0.5) * ywin - 0.5;
+#pragma unroll
+                for (int a = 0; a < NPT; ++a) { mt[a][0] = 0.0; mt[a][1] = 0.0; }
+            }
+            const double dl = dy - cYc;
+            const unsigned same = __ballot_sync(0xffffffffu, valid && ilo == cI0 && ihi == cI1 && jlo == cJ0 && jhi == cJ1 &&
+                                                                 fabs(dl) <= ywin);
+            const unsigned rest = ~(same >> pos);
+            const int run = rest ? (__ffs(rest) - 1) : 32;
+            const int pend = min(pos + run, nb);
+            if (!COUNT) {
+                __syncwarp();                                  // the previous run's step-1 reads of vy are done
+                const double d2 = dl * dl, d3 = d2 * dl, d4 = d2 * d2;
+                S.vy[0 * kMomLdk + lane] = 1.0;
+                S.vy[1 * kMomLdk + lane] = dl;
+                S.vy[2 * kMomLdk + lane] = d2;
+                S.vy[3 * kMomLdk + lane] = d3;
+                S.vy[4 * kMomLdk + lane] = d4;
+                S.vy[5 * kMomLdk + lane] = d4 * dl;
+                S.vy[6 * kMomLdk + lane] = d4 * d2;
+                S.vy[7 * kMomLdk + lane] = d4 * d3;
+                __syncwarp();
+                // ---- step 1: MT += VX VY^T over the samples [pos, pend)
+                for (int ks = pos >> 2; ks <= (pend - 1) >> 2; ++ks) {
+                    const int ksamp = 4 * ks + lr;
+                    const bool in = ksamp >= pos && ksamp < pend;
+                    const double vv = S.vy[lq * kMomLdk + ksamp];
+                    const double a = in ? vv : 0.0;
+                    double b[NPT];
+#pragma unroll
+                    for (int qt = 0; qt < NPT; ++qt) b[qt] = S.vx[(8 * qt + lq) * kMomLdk + ksamp];
+#pragma unroll
+                    for (int qt = 0; qt < NPT; ++qt) dmma_m8n8k4(mt[qt][0], mt[qt][1], a, b[qt]);
+                }
+            }
+            pos = pend;
+        }
+        k += nb;
+    }
+    if (have) emit();
+    if (COUNT && lane == 0) counts[item_id] = n_cells;
+}
+
+// steps 2 + 3 + a5 for the cells of one item, in order, under the ticket queue (render_moment.cuh queue_take / queue_done)
+template <int NPT>
+__global__ void __launch_bounds__(32, NPT == 2 ? E2E_MOM_MINB : 1)
+cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny)
+{
+    const int lane = threadIdx.x & 31;
+    const int item_id = queue_take(W, W.ctrl, lane);
+    if (item_id < 0) return;
+    const long long c0 = C.cell_off[item_id], c1 = C.cell_off[item_id + 1];
+    for (long long cell = c0; cell < c1; ++cell) {
+        const CellHeader h = C.hdr[cell];
+        double mt[1][NPT][2];
+        const double* src = C.mom + ((size_t)cell * 32 + lane) * (2 * NPT);
+#pragma unroll
+        for (int qt = 0; qt < NPT; ++qt) {
+            const double2 v = __ldcs(reinterpret_cast<const double2*>(src + 2 * qt));
+            mt[0][qt][0] = v.x; mt[0][qt][1] = v.y;
+        }
+        moment_flush_cell<NPT, false>(Q, mt, h.i0, h.i1, h.j0, h.j1, h.yb, 0, 0, frame, nx, ny, lane);
+    }
+    queue_done(W, W.ctrl, item_id, lane);
+}
+
+}  // namespace e2e

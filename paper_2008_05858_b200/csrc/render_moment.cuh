@@ -116,44 +116,15 @@ __device__ __forceinline__ void queue_done(const QueueParam& W, unsigned* ctrl, 
     for (int d = W.succ_off[item_id] + lane; d < s1; d += 32) red_release_dec_u32(pend + W.succ_idx[d]);
 }
 
-// MAP (DESIGN.md G21, analytic PSF map): the PSF of a sample is the bilinear blend of 4 node PSFs, and the blend is linear, so
-// a cell (now also: one node cell of the map) keeps ONE weighted moment set per node, M_c = sum_k (w_k beta_c,k) delta^p dx^q, and
-// its contribution is sum_c cy_c^T M_c cx_c with node c's own tables -- steps 2 + 3 run once per node into the same window.
+// steps 2 + 3 + a5 for one cell: its moment set(s) mt, footprint box, y-phase window and (MAP) node cell
 template <int NPT, bool MAP>
-__global__ void __launch_bounds__(kMomWarps * 32, MAP ? 12 : (NPT == 2 ? E2E_MOM_MINB : 1))
-render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
-                     const Strip* __restrict__ strips, const Item* __restrict__ items, QueueParam W, MomentParam Q,
-                     double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)
+__device__ __forceinline__ void moment_flush_cell(const MomentParam& Q, const double (&mt)[MAP ? 4 : 1][NPT][2], int cI0, int cI1, int cJ0,
+                                                  int cJ1, int cYb, int cG, int cH, double* __restrict__ frame, int nx, int ny, int lane)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (frames) {                                             // batch render (e2e_render_frames): blockIdx.y = frame,
-        frame = frames[blockIdx.y];                           // same geometry, its own weights, target and control block
-        ws += (long long)blockIdx.y * w_stride;
-    }
-    MomentWarpSmem<NPT, MAP>& S = reinterpret_cast<MomentWarpSmem<NPT, MAP>*>(smem_raw)[warp];
-    constexpr int NC = MAP ? 4 : 1;                           // moment sets per cell
-    const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
-    constexpr int NP = 8 * NPT;
-    const double ywin = 1.0 / (double)Q.nyb;
+    constexpr int NC = MAP ? 4 : 1;
+    const int lq = lane >> 2, lr = lane & 3;
+    (void)cG; (void)cH;
 
-    const int item_id = queue_take(W, W.ctrl + (frames ? (long long)blockIdx.y * W.ctrl_stride : 0), lane);
-    if (item_id < 0) return;
-    const Item it = items[item_id];
-    const Strip st = strips[it.strip];
-
-    long long k = (long long)it.chunk0 * 32;
-    long long kend = k + (long long)it.nchunks * 32;
-    if (kend > st.n) kend = st.n;
-
-    double mt[NC][NPT][2];                                     // M tiles [node][qt]: lane holds M[p = l/4][q = 8qt + 2(l%4) + e]
-    bool have = false;
-    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
-    int cG = 0, cH = 0;                                        // MAP: its node cell (first node column / row)
-    double cYc = 0.0;                                          // its centre
-
-    // steps 2 + 3 + a5 for the open cell
-    auto flush = [&]() {
         const bool dead = cI1 < 0 || cI0 >= nx || cJ1 < 0 || cJ0 >= ny || cI1 < cI0 || cJ1 < cJ0;
         if (dead) return;
         for (int jp = 0; jp < Q.njt; jp += 3) {
@@ -233,7 +204,46 @@ render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ y
             }
         }
         __syncwarp();                                          // the next cell's window overlaps this one
-    };
+    }
+
+// MAP (DESIGN.md G21, analytic PSF map): the PSF of a sample is the bilinear blend of 4 node PSFs, and the blend is linear, so
+// a cell (now also: one node cell of the map) keeps ONE weighted moment set per node, M_c = sum_k (w_k beta_c,k) delta^p dx^q, and
+// its contribution is sum_c cy_c^T M_c cx_c with node c's own tables -- steps 2 + 3 run once per node into the same window.
+template <int NPT, bool MAP>
+__global__ void __launch_bounds__(kMomWarps * 32, MAP ? 12 : (NPT == 2 ? E2E_MOM_MINB : 1))
+render_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
+                     const Strip* __restrict__ strips, const Item* __restrict__ items, QueueParam W, MomentParam Q,
+                     double* __restrict__ frame, int nx, int ny, long long w_stride, double* const* __restrict__ frames)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (frames) {                                             // batch render (e2e_render_frames): blockIdx.y = frame,
+        frame = frames[blockIdx.y];                           // same geometry, its own weights, target and control block
+        ws += (long long)blockIdx.y * w_stride;
+    }
+    MomentWarpSmem<NPT, MAP>& S = reinterpret_cast<MomentWarpSmem<NPT, MAP>*>(smem_raw)[warp];
+    constexpr int NC = MAP ? 4 : 1;                           // moment sets per cell
+    const int lq = lane >> 2, lr = lane & 3;                  // fragment coordinates: l/4 and l%4
+    constexpr int NP = 8 * NPT;
+    const double ywin = 1.0 / (double)Q.nyb;
+
+    const int item_id = queue_take(W, W.ctrl + (frames ? (long long)blockIdx.y * W.ctrl_stride : 0), lane);
+    if (item_id < 0) return;
+    const Item it = items[item_id];
+    const Strip st = strips[it.strip];
+
+    long long k = (long long)it.chunk0 * 32;
+    long long kend = k + (long long)it.nchunks * 32;
+    if (kend > st.n) kend = st.n;
+
+    double mt[NC][NPT][2];                                     // M tiles [node][qt]: lane holds M[p = l/4][q = 8qt + 2(l%4) + e]
+    bool have = false;
+    int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;           // footprint box and y-phase window of the open cell
+    int cG = 0, cH = 0;                                        // MAP: its node cell (first node column / row)
+    double cYc = 0.0;                                          // its centre
+
+    // steps 2 + 3 + a5 for the open cell
+    auto flush = [&]() { moment_flush_cell<NPT, MAP>(Q, mt, cI0, cI1, cJ0, cJ1, cYb, cG, cH, frame, nx, ny, lane); };
 
     while (k < kend) {
         // ---- next batch of up to 32 samples: footprint boxes, phases, power arrays

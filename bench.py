@@ -38,6 +38,7 @@ C_ERFC, C_PSI = 60.0, 90.0
 KERNEL_SOURCES = {"render_moment_kernel": "render_moment.cuh", "render_tabcell_kernel": "render_tabcell.cuh",
                   "render_poly_kernel": "render_poly.cuh", "render_analytic_kernel": "render_analytic.cuh",
                   "render_tabulated_kernel": "render_tabulated.cuh", "detector_kernel": "detector.cu",
+                  "cell_flush_kernel": "render_cells.cuh", "cell_moment_kernel": "render_cells.cuh",
                   "setup_samples_kernel": "setup.cuh"}
 
 
@@ -371,18 +372,31 @@ def stage_rooflines(m, name: str, peak_tf: float, burst_tf: float):
                       "peak_source": hbm_src}
 
     hbm("zero", m["stage_ms"]["ms_zero"], 8.0 * npx, "8 B per pixel written", None)
-    hbm("setup", m["stage_ms"]["ms_setup"], 24.0 * n_samples + table_bytes * m["nbatch"],
-        "24 B per sample written (x, y, w) + the spectrum tables read once", "setup_samples_kernel")
+    split = kinfo["name"].startswith("cell_flush_kernel")
+    if split:
+        # two-kernel analytic path: the setup stage is cell_moment_kernel (a1-a3 fused + step 1); it writes one record per cell
+        npt = int(kinfo["name"].split("<")[1].rstrip(">"))
+        rec = 32.0 + 512.0 * npt
+        hbm("setup", m["stage_ms"]["ms_setup"], rec * n_cells + table_bytes * m["nbatch"],
+            "cell_moment_kernel: %d B per footprint cell written (header + moment tiles) + the spectrum tables read once; its step 1 is "
+            "%.3g fp64 flop per frame (2 x 8 (P+1) per sample)" % (rec, 2.0 * n_samples * alg["fma_per_sample"]), "cell_moment_kernel<%d>" % npt)
+    else:
+        hbm("setup", m["stage_ms"]["ms_setup"], 24.0 * n_samples + table_bytes * m["nbatch"],
+            "24 B per sample written (x, y, w) + the spectrum tables read once", "setup_samples_kernel")
     hbm("detector", m["stage_ms"]["ms_detector"], 16.0 * npx, "16 B per pixel (fp64 frame read + fp64 frame written)", "detector_kernel<double, false>")
     ms_render = m["stage_ms"]["ms_render"]
     if ms_render > 0:
         sec = ms_render * 1e-3
-        alg_flops = 2.0 * (n_cells * alg["fma_per_cell"] + n_samples * alg["fma_per_sample"])
+        alg_flops = 2.0 * (n_cells * alg["fma_per_cell"] + (0 if split else n_samples * alg["fma_per_sample"]))
         executed = 2.0 * (n_cells * kinfo["executed_fma_per_cell"] + n_samples * kinfo["executed_fma_per_sample"])
         ncols, nrows = np.floor(2 * m["hbx"]), np.floor(2 * m["hby"])
         fma_flops, survey_flops = algorithmic_flops_per_sample(scene.psf, m["info"]["n_nodes"], ncols, nrows)
         definition = ("algorithmic = un-padded fp64 flops of the cell-moment method (DESIGN.md 5.3 'Roofline'): per cell "
                       "2 T (8 (P+1) w + 8 w h), per sample 2 * 8 (P+1); x measured cell / sample counts of the workload")
+        if split:
+            definition = ("algorithmic = un-padded fp64 flops of the contraction this kernel performs (steps 2 + 3 of the cell-moment method, "
+                          "DESIGN.md 5.3): per cell 2 T (8 (P+1) w + 8 w h) x the measured cell count; the moment update (2 * 8 (P+1) per "
+                          "sample) runs in cell_moment_kernel and is counted there (stage_roofline.setup)")
         if kinfo["name"].startswith("render_tabcell"):
             definition = ("algorithmic = fp64 flops of the cell-deposit method (DESIGN.md 5.5): per cell 2 x nodes x 2 y-offset rows x "
                           "(os+1) x-offsets x (npix+1)^2 window pixels, per sample 2 x 4 x nodes deposit products; x measured counts")

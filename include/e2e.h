@@ -193,8 +193,9 @@ typedef struct {
 } e2e_spectrum_t;
 
 /* bytes of device scratch e2e_render_frame needs for this (format, psf): the per-sample arrays x, y, w of
- * step a1-a3 (24 B per sample) plus the control block of the persistent render launch (4 B per work item).
- * 256-byte aligned workspace required. */
+ * step a1-a3 (24 B per sample; the kernels that materialise the samples), the control block of the render queue (4 B per
+ * work item) and, on the two-kernel analytic path, one record per footprint cell (32 B + 512 B per power tile: 1056 B per
+ * cell for the ESPRESSO-like PSF, 1.7 GB per frame).  256-byte aligned workspace required. */
 E2E_API int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, size_t* bytes);
 
 /* a1-a3 only, for one (fiber, order): writes lam, x, y, w of its samples to DEVICE arrays of length
@@ -333,15 +334,18 @@ E2E_API int e2e_measure_fp64_peak(int32_t repeats, double* burst_dfma_per_s, dou
 E2E_API int e2e_probe_fp64_pipe(double* results6);
 
 /* Which a4+a5 kernel e2e_render_frame launches for this (format, psf) pair and what it executes: *name is a static
- * string ("render_moment_kernel<2>", "render_poly_kernel<14>", "render_analytic_kernel", "render_tabulated_kernel");
- * *executed_fma_per_cell / *executed_fma_per_sample are the fp64 fused multiply-adds the kernel issues per footprint
+ * string ("cell_flush_kernel<2>" -- the dominant kernel of the two-kernel analytic path, whose first kernel is
+ * cell_moment_kernel --, "render_moment_kernel<2, map>", "render_poly_kernel<14>", "render_analytic_kernel",
+ * "render_tabcell_kernel", "render_tabulated_kernel"; the batch call and the PSF map run "render_moment_kernel<NPT>");
+ * *executed_fma_per_cell / *executed_fma_per_sample are the fp64 fused multiply-adds THAT kernel issues per footprint
  * cell and per sample (DMMA counted as 256), 0 where it does not apply.  Any output pointer may be NULL. */
 E2E_API int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const char** name,
                                    double* executed_fma_per_cell, double* executed_fma_per_sample);
 
 /* Algorithmic work of the a4+a5 method e2e_render_frame uses for this pair (DESIGN.md 5.3 "Roofline"), without the
  * padding of the DMMA tiles: fp64 fused multiply-adds per footprint cell, T (8 (P+1) w + 8 w h) with w x h the nominal
- * footprint (2 H + 1 pixels per axis, G9), P the x-phase degree, T the chord terms, and per sample, 8 (P+1) (moment update).
+ * footprint (2 H + 1 pixels per axis, G9), P the x-phase degree, T the chord terms, and per sample, 8 (P+1) (moment update;
+ * on the two-kernel path the per-cell part is cell_flush_kernel's work and the per-sample part cell_moment_kernel's).
  * Tabulated PSF (cell-deposit kernel): per cell nodes x 2 y-offset rows x (os+1) x-offsets x (npix+1)^2 window
  * pixels, per sample 4 x nodes deposit products (nodes = field nodes blended per sample: 1, 2 or 4).
  * 0 for the kernels that do not work cell by cell.  Output pointers may be NULL. */
@@ -377,8 +381,9 @@ E2E_API int64_t e2e_launch_count(void);
  * totals afterwards.  ms_* are summed device milliseconds, n_* the number of kernel launches in that stage. */
 typedef struct {
     double ms_zero;      /* zero-fill of the frame (cudaMemsetAsync) */
-    double ms_setup;     /* a1-a3 sample-setup kernel */
-    double ms_render;    /* a4-a5 render kernels (all phases) */
+    double ms_setup;     /* a1-a3 sample-setup kernel; on the two-kernel analytic path: cell_moment_kernel (a1-a3 fused with the
+                            weighted phase moments of every footprint cell) */
+    double ms_render;    /* a4-a5 render kernels (all phases); on the two-kernel path: cell_flush_kernel (the contraction + a5) */
     double ms_detector;  /* a6 */
     int64_t n_setup, n_render, n_detector;
     int64_t n_calls;     /* e2e_render_frame calls covered */

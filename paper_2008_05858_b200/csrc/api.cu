@@ -855,9 +855,9 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         static SpectraParam no_spectra;
         const unsigned blocks = (unsigned)((ni + kCellWarps - 1) / kCellWarps);
         switch (P->moment_npt) {
-            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
-            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
-            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
         }
         count_launch();
         std::vector<int> counts(ni);
@@ -1034,6 +1034,63 @@ static size_t cell_mom_bytes(const e2e_plan* pl, const e2e_psf* P)
 static size_t cell_bytes(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl)
 {
     return use_split(F, P, pl) ? cell_hdr_bytes(pl) + cell_mom_bytes(pl, P) : 0;
+}
+
+static CellStore cell_store(const e2e_plan* pl, unsigned* ctrl)
+{
+    CellStore cs;
+    cs.cell_off = pl->d_cell_off;
+    cs.hdr = (CellHeader*)((char*)ctrl + align_up(sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)), 256));
+    cs.mom = (double*)((char*)cs.hdr + cell_hdr_bytes(pl));
+    return cs;
+}
+
+// kernel A of the two-kernel render: a1-a3 + the moments of every cell of the items ids[0 .. n) (nullptr: all items)
+static int launch_cell_moments(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const e2e_spectrum_t* spectra, unsigned* ctrl,
+                               const int* ids, int n, cudaStream_t stream)
+{
+    if (n <= 0) return E2E_OK;
+    const CellStore cs = cell_store(pl, ctrl);
+    SpectraParam sp;
+    memset(&sp, 0, sizeof(sp));
+    for (int f = 0; f < F->view.n_fibers; ++f) sp.s[f] = spectra[f];
+    const unsigned blocks = (unsigned)((n + kCellWarps - 1) / kCellWarps);
+#define E2E_CELL_CASE(NPT)                                                                                                     \
+    case NPT:                                                                                                                   \
+        cell_moment_kernel<NPT, false, true><<<blocks, kCellWarps * 32, sizeof(MomentWarpSmem<NPT, false>) * kCellWarps, stream>>>( \
+            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ids, n, P->mom, cs, nullptr, F->view, sp);                    \
+        break;
+    switch (P->moment_npt) {
+        E2E_CELL_CASE(2) E2E_CELL_CASE(3) E2E_CELL_CASE(4)
+        default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+    }
+#undef E2E_CELL_CASE
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "cell_moment_kernel launch");
+    return E2E_OK;
+}
+
+// kernel B: the contraction of every cell of the queue's items, in queue order
+static int launch_cell_flush(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, double* d_frame, unsigned* ctrl, const int* queue,
+                             int n, int head, cudaStream_t stream)
+{
+    if (n <= 0) return E2E_OK;
+    const CellStore cs = cell_store(pl, ctrl);
+    QueueParam W;
+    memset(&W, 0, sizeof(W));
+    W.queue = queue; W.n = n; W.head = head; W.ctrl = ctrl;
+    W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
+    switch (P->moment_npt) {
+        case 2: cell_flush_kernel<2><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+        case 3: cell_flush_kernel<3><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+        case 4: cell_flush_kernel<4><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+        default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+    }
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "cell_flush_kernel launch");
+    return E2E_OK;
 }
 
 // (re)initialise a control block in the caller's workspace for one launch: head counters 0, dependency counters from the plan
@@ -1230,7 +1287,9 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
         StageTimer tm(kStageSetup, stream);
         const long long before = g_launches.load();
         if (persistent) E2E_CUDA(ctrl_reset(pl, qs.ctrl, stream));
-        if (!use_split(fmt, psf, pl)) rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);   // the two-kernel path fuses a1-a3
+        // the two-kernel path fuses a1-a3 into its first kernel, which is timed as this stage
+        if (use_split(fmt, psf, pl)) rc = launch_cell_moments(fmt, psf, pl, spectra, qs.ctrl, nullptr, pl->n_items, stream);
+        else rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
         if (rc) return rc;
     }
@@ -1256,35 +1315,8 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
             if (ce == cudaSuccess) ce = cudaStreamWaitEvent(stream, hp->ev_aux_done, 0);
             if (ce != cudaSuccess) return fail_cuda(ce, "render_frame: join");
         } else if (use_split(fmt, psf, pl)) {
-            // two kernels (render_cells.cuh): every cell's moments in any order, then the contraction under the ticket queue
-            CellStore cs;
-            cs.cell_off = pl->d_cell_off;
-            cs.hdr = (CellHeader*)((char*)qs.ctrl + ctrl_bytes(pl));
-            cs.mom = (double*)((char*)cs.hdr + cell_hdr_bytes(pl));
-            QueueParam W;
-            memset(&W, 0, sizeof(W));
-            W.n = pl->n_items; W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
-            W.ctrl = qs.ctrl;
-            const unsigned ab = (unsigned)((pl->n_items + kCellWarps - 1) / kCellWarps);
-            SpectraParam sp_call;                                // a1-a3 run inside cell_moment_kernel: no setup launch on this path
-            memset(&sp_call, 0, sizeof(sp_call));
-            for (int f = 0; f < fmt->view.n_fibers; ++f) sp_call.s[f] = spectra[f];
-#define E2E_SPLIT_CASE(NPT)                                                                                                     \
-    case NPT: {                                                                                                                 \
-        const size_t sm = sizeof(MomentWarpSmem<NPT, false>) * kCellWarps;                                                      \
-        cell_moment_kernel<NPT, false, true><<<ab, kCellWarps * 32, sm, stream>>>(nullptr, nullptr, nullptr, pl->d_strips,       \
-                                                                                  pl->d_items, pl->n_items, psf->mom, cs,       \
-                                                                                  nullptr, fmt->view, sp_call);                 \
-        cell_flush_kernel<NPT><<<(unsigned)pl->n_items, 32, 0, stream>>>(W, psf->mom, cs, d_frame, fmt->view.nx, fmt->view.ny);  \
-    } break;
-            switch (psf->moment_npt) {
-                E2E_SPLIT_CASE(2) E2E_SPLIT_CASE(3) E2E_SPLIT_CASE(4)
-                default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
-            }
-#undef E2E_SPLIT_CASE
-            count_launch(2);
-            cudaError_t ce = cudaGetLastError();
-            if (ce != cudaSuccess) return fail_cuda(ce, "cell_moment_kernel / cell_flush_kernel launch");
+            // second kernel of the two-kernel render: the contraction of every cell, under the ticket queue
+            rc = launch_cell_flush(fmt, psf, pl, d_frame, qs.ctrl, nullptr, pl->n_items, 0, stream);
         } else {
             rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, stream, qs);
         }
@@ -1479,7 +1511,8 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     // banded pipeline: per row band a1-a3 of its strips, a4 + a5, a6 on the rows that became final, then those rows travel
     // to the host on the library's copy stream while the next bands render
     const size_t per = sample_array_bytes(pl->total_samples);
-    if (workspace_bytes - used < 3 * per + ctrl_bytes(pl)) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
+    const bool split = use_split(fmt, psf, pl);
+    if (workspace_bytes - used < 3 * per + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
     double* d_x = (double*)p;
     double* d_y = (double*)(p + per);
     double* d_w = (double*)(p + 2 * per);
@@ -1496,14 +1529,20 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     int row0 = 0;
     for (int b = 0; b < part.n_bands && !rc && ce == cudaSuccess; ++b) {
         cudaStream_t cs = (b & 1) ? hp->aux : stream;
-        rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &part, b);   // a1-a3 of this band's strips only
-        if (rc) break;
         QueueSel qs;
         qs.ctrl = d_ctrl; qs.head = b;
         qs.queue = part.d_queue + part.queue_off[b];
         qs.n = part.queue_off[b + 1] - part.queue_off[b];
-        rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, qs, part.d_items,
-                           part.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        if (split) {
+            // two-kernel render of this band's items: a1-a3 + moments, then the contraction under the band's queue
+            rc = launch_cell_moments(fmt, psf, pl, dev.data(), d_ctrl, qs.queue, qs.n, cs);
+            if (!rc) rc = launch_cell_flush(fmt, psf, pl, d_frame, d_ctrl, qs.queue, qs.n, b, cs);
+        } else {
+            rc = launch_setup(fmt, pl, dev.data(), d_x, d_y, d_w, cs, &part, b);   // a1-a3 of this band's strips only
+            if (!rc)
+                rc = launch_render(fmt, psf, pl, d_x, d_y, d_w, d_frame, cs, qs, part.d_items,
+                                   part.phase_off.data() + (size_t)b * (pl->n_phases_all + 1), pl->n_phases_all);
+        }
         if (rc) break;
         const int row1 = std::max(row0, part.fin_row[b]);
         if (row1 > row0) {
@@ -1697,13 +1736,18 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
     if (choose_moment(fmt, psf)) {
         static const char* names[] = {"", "", "render_moment_kernel<2>", "render_moment_kernel<3>", "render_moment_kernel<4>"};
         static const char* map_names[] = {"", "", "render_moment_kernel<2, map>", "render_moment_kernel<3, map>", "render_moment_kernel<4, map>"};
+        static const char* split_names[] = {"", "", "cell_flush_kernel<2>", "cell_flush_kernel<3>", "cell_flush_kernel<4>"};
         const MomentParam& M = psf->mom;
         const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
-        nm = psf->is_map ? map_names[npt] : names[npt];
+        e2e_plan* pl = nullptr;
+        const bool split = build_plan(const_cast<e2e_format*>(fmt), psf, &pl) == E2E_OK && use_split(fmt, psf, pl);
+        nm = split ? split_names[npt] : psf->is_map ? map_names[npt] : names[npt];
         const double nodes = psf->is_map ? (M.gx > 1 ? 2.0 : 1.0) * (M.gy > 1 ? 2.0 : 1.0) : 1.0;
         // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
         pc = nodes * 256.0 * M.T * (2.0 * npt * M.nit * jp + 2.0 * M.nit * M.njt);         // step 2 (redone per row panel) + step 3
-        ps = nodes * 64.0 * npt + 8.0 * npt + 8.0;             // step 1 (npt DMMAs per 4 samples and node) + powers
+        // step 1 (npt DMMAs per 4 samples and node) + powers: on the two-kernel path they belong to cell_moment_kernel, not to the
+        // kernel named here
+        ps = split ? 0.0 : nodes * 64.0 * npt + 8.0 * npt + 8.0;
         (void)ip;
     } else if (psf->kind == 0 && psf->poly_degree > 0) {
         static thread_local char buf[40];

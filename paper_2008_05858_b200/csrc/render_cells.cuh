@@ -41,13 +41,15 @@ struct CellStore {
 template <int NPT, bool COUNT, bool FUSED>
 __global__ void __launch_bounds__(kCellWarps * 32)
 cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
-                   const Strip* __restrict__ strips, const Item* __restrict__ items, int n_items, MomentParam Q, CellStore C,
-                   int* __restrict__ counts, const __grid_constant__ FormatView F, const __grid_constant__ SpectraParam SP)
+                   const Strip* __restrict__ strips, const Item* __restrict__ items, const int* __restrict__ ids, int n_items,
+                   MomentParam Q, CellStore C, int* __restrict__ counts, const __grid_constant__ FormatView F,
+                   const __grid_constant__ SpectraParam SP)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int item_id = blockIdx.x * kCellWarps + warp;
-    if (item_id >= n_items) return;
+    const int slot = blockIdx.x * kCellWarps + warp;
+    if (slot >= n_items) return;
+    const int item_id = ids ? ids[slot] : slot;              // ids: the items of one row band (host path), else all of them
     MomentWarpSmem<NPT, false>& S = reinterpret_cast<MomentWarpSmem<NPT, false>*>(smem_raw)[warp];
     const int lq = lane >> 2, lr = lane & 3;
     constexpr int NP = 8 * NPT;

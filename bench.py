@@ -35,20 +35,27 @@ C_ERFC, C_PSI = 60.0, 90.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures: profiles/traffic.json
 # holds, per (workload, kernel), the bytes, the profile file they come from and the sha256 of the kernel's source file at
 # capture time.  A value is reported only while that hash still matches the source in the tree (else null + a note).
-KERNEL_SOURCES = {"render_moment_kernel": "render_moment.cuh", "render_tabcell_kernel": "render_tabcell.cuh",
-                  "render_poly_kernel": "render_poly.cuh", "render_analytic_kernel": "render_analytic.cuh",
-                  "render_tabulated_kernel": "render_tabulated.cuh", "detector_kernel": "detector.cu",
-                  "cell_flush_kernel": "render_cells.cuh", "cell_moment_kernel": "render_cells.cuh",
-                  "setup_samples_kernel": "setup.cuh"}
+# kernel -> the source files its device code comes from (a capture in profiles/traffic.json is stale once any of them changed)
+KERNEL_SOURCES = {"render_moment_kernel": ("render_moment.cuh",), "render_tabcell_kernel": ("render_tabcell.cuh",),
+                  "render_poly_kernel": ("render_poly.cuh",), "render_analytic_kernel": ("render_analytic.cuh",),
+                  "render_tabulated_kernel": ("render_tabulated.cuh",), "detector_kernel": ("detector.cu",),
+                  "cell_flush_kernel": ("render_cells.cuh", "render_moment.cuh"),
+                  "cell_moment_kernel": ("render_cells.cuh", "render_moment.cuh", "setup.cuh"),
+                  "setup_samples_kernel": ("setup.cuh",)}
 
 
 def source_hash(kernel: str):
     import hashlib
-    base = kernel.split("<")[0]
-    f = ROOT / "paper_2008_05858_b200" / "csrc" / KERNEL_SOURCES.get(base, "")
-    if not f.is_file():
+    files = KERNEL_SOURCES.get(kernel.split("<")[0])
+    if not files:
         return None
-    return hashlib.sha256(f.read_bytes()).hexdigest()
+    h = hashlib.sha256()
+    for name in files:
+        f = ROOT / "paper_2008_05858_b200" / "csrc" / name
+        if not f.is_file():
+            return None
+        h.update(f.read_bytes())
+    return h.hexdigest()
 
 
 def ncu_traffic(workload: str, kernel: str):
@@ -61,7 +68,7 @@ def ncu_traffic(workload: str, kernel: str):
     if not e:
         return None, "no ncu capture committed for this (workload, kernel)"
     if e.get("source_sha256") != source_hash(kernel):
-        return None, f"stale: {KERNEL_SOURCES.get(kernel.split('<')[0])} changed since {e.get('profile')}"
+        return None, f"stale: {' / '.join(KERNEL_SOURCES.get(kernel.split('<')[0], ()))} changed since {e.get('profile')}"
     return float(e["bytes_per_launch"]), f"{e.get('profile')} ({e.get('launches_per_step')} launches per step)"
 
 

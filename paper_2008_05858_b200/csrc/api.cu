@@ -48,7 +48,7 @@ constexpr int kDeviceParts = 2;        // row bands e2e_render_frame renders con
 #define E2E_HOST_BANDS 8
 #endif
 #ifndef E2E_HOST_BANDS16
-#define E2E_HOST_BANDS16 3
+#define E2E_HOST_BANDS16 5
 #endif
 constexpr int kHostBands = E2E_HOST_BANDS;       // row bands of e2e_render_frame_host (device-to-host copy overlapped with rendering)
 constexpr int kHostBands16 = E2E_HOST_BANDS16;   // the same for the uint16 output: the copy is 4x shorter, fewer and larger bands pay
@@ -110,18 +110,24 @@ using namespace e2e;
 struct HostPipe {
     static constexpr int kEvents = 16;
     cudaStream_t copy = nullptr;
+    cudaStream_t up = nullptr;         // host -> device: the spectrum tables travel in the order the bands need them
     cudaStream_t aux = nullptr;        // second compute stream: odd bands render here while even bands render on the caller's
     cudaEvent_t ev[kEvents] = {};
-    cudaEvent_t ev_start = nullptr, ev_aux_done = nullptr;
+    cudaEvent_t ev_up[kEvents] = {};
+    cudaEvent_t ev_start = nullptr, ev_aux_done = nullptr, ev_zero = nullptr;
     std::mutex mu;                     // one call at a time enqueues on these streams
     ~HostPipe()
     {
         if (copy) cudaStreamDestroy(copy);
+        if (up) cudaStreamDestroy(up);
         if (aux) cudaStreamDestroy(aux);
         for (cudaEvent_t e : ev)
             if (e) cudaEventDestroy(e);
+        for (cudaEvent_t e : ev_up)
+            if (e) cudaEventDestroy(e);
         if (ev_start) cudaEventDestroy(ev_start);
         if (ev_aux_done) cudaEventDestroy(ev_aux_done);
+        if (ev_zero) cudaEventDestroy(ev_zero);
     }
 };
 static HostPipe* host_pipe(e2e_plan* pl)
@@ -130,10 +136,14 @@ static HostPipe* host_pipe(e2e_plan* pl)
     if (!pl->pipe) {
         HostPipe* h = new HostPipe;
         bool ok = cudaStreamCreateWithFlags(&h->copy, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&h->up, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaStreamCreateWithFlags(&h->aux, cudaStreamNonBlocking) == cudaSuccess &&
                   cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) == cudaSuccess &&
-                  cudaEventCreateWithFlags(&h->ev_aux_done, cudaEventDisableTiming) == cudaSuccess;
-        for (int i = 0; ok && i < HostPipe::kEvents; ++i) ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess;
+                  cudaEventCreateWithFlags(&h->ev_aux_done, cudaEventDisableTiming) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&h->ev_zero, cudaEventDisableTiming) == cudaSuccess;
+        for (int i = 0; ok && i < HostPipe::kEvents; ++i)
+            ok = cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming) == cudaSuccess &&
+                 cudaEventCreateWithFlags(&h->ev_up[i], cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { delete h; return nullptr; }
         pl->pipe = h;
     }
@@ -940,6 +950,18 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
                     if (band_of[s] == b && pl->strips[s].n > 0) bstrips.push_back(s);
                 part.strip_off[b + 1] = (int)bstrips.size();
             }
+            // wavelength range each band reads from each fiber's spectrum (the host path uploads the tables in that order)
+            const int nf = F->view.n_fibers, no = F->view.n_orders;
+            part.lam_lo.assign((size_t)want * nf, INFINITY);
+            part.lam_hi.assign((size_t)want * nf, -INFINITY);
+            for (int s = 0; s < n_strips; ++s) {
+                if (pl->strips[s].n == 0) continue;
+                const int fiber = s / no, o = s - fiber * no;
+                double& lo = part.lam_lo[(size_t)band_of[s] * nf + fiber];
+                double& hi = part.lam_hi[(size_t)band_of[s] * nf + fiber];
+                lo = std::min(lo, std::min(F->lam_min[o], F->lam_max[o]));
+                hi = std::max(hi, std::max(F->lam_min[o], F->lam_max[o]));
+            }
             E2E_CUDA(cudaMalloc(&part.d_strips, sizeof(int) * std::max<size_t>(1, bstrips.size())));
             if (!bstrips.empty()) E2E_CUDA(cudaMemcpy(part.d_strips, bstrips.data(), sizeof(int) * bstrips.size(), cudaMemcpyHostToDevice));
             E2E_CUDA(cudaMalloc(&part.d_items, sizeof(Item) * std::max<size_t>(1, bflat.size())));
@@ -1471,17 +1493,23 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     }
     const size_t out_elem = out16 ? 2 : 8;
     const char* d_out = out16 ? (const char*)d_adu : (const char*)d_frame;
-    std::vector<e2e_spectrum_t> dev(spectra, spectra + fmt->view.n_fibers);
-    for (int f = 0; f < fmt->view.n_fibers; ++f) {
-        // fibers that share one host table share one device copy
+    const int nf = fmt->view.n_fibers;
+    std::vector<e2e_spectrum_t> dev(spectra, spectra + nf);
+    std::vector<int> tab_of(nf, 0);                    // fibers that share one host table share one device copy
+    for (int f = 0; f < nf; ++f) {
         int same = -1;
         for (int g = 0; g < f; ++g)
             if (spectra[g].d_flux == spectra[f].d_flux && spectra[g].n == spectra[f].n) { same = g; break; }
+        tab_of[f] = same >= 0 ? same : f;
         if (same >= 0) { dev[f].d_flux = dev[same].d_flux; continue; }
-        E2E_CUDA(cudaMemcpyAsync(p, spectra[f].d_flux, (size_t)spectra[f].n * 8, cudaMemcpyHostToDevice, stream));
         dev[f].d_flux = (const double*)p;
         p += align_up((size_t)spectra[f].n * 8, 256);
     }
+    // host -> device copy of the elements [lo, hi) of fiber f's table
+    auto upload = [&](int f, long long lo, long long hi, cudaStream_t cs) -> cudaError_t {
+        if (hi <= lo) return cudaSuccess;
+        return cudaMemcpyAsync(const_cast<double*>(dev[f].d_flux) + lo, spectra[f].d_flux + lo, (size_t)(hi - lo) * 8, cudaMemcpyHostToDevice, cs);
+    };
     const size_t used = (size_t)(p - (char*)d_workspace);
     e2e_plan* pl = nullptr;
     rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
@@ -1499,7 +1527,9 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     HostPipe* hp = host_pipe(pl);
     const e2e_plan::BandPart& part = out16 ? pl->host16 : pl->host;   // the 2-byte output travels 4x faster: fewer, larger bands
     if (part.n_bands <= 1 || !hp) {
-        // one pass: render, detector, copy
+        // one pass: tables, render, detector, copy
+        for (int f = 0; f < nf; ++f)
+            if (tab_of[f] == f) E2E_CUDA(upload(f, 0, spectra[f].n, stream));
         rc = e2e_render_frame(fmt, psf, dev.data(), d_frame, 0, p, workspace_bytes - used, stream);
         if (rc) return rc;
         rc = detector_rows(0, ny, stream);
@@ -1519,16 +1549,54 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     unsigned* d_ctrl = (unsigned*)(p + 3 * per);
     if (part.n_bands > kCtrlHeads) return fail(E2E_ERR_UNSUPPORTED, w + ": too many row bands");
     std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
-    E2E_CUDA(cudaMemsetAsync(d_frame, 0, npix * 8, stream));
-    E2E_CUDA(ctrl_reset(pl, d_ctrl, stream));
     // bands share no pixel (build_plan): even bands on the caller's stream, odd bands on the library's second stream
     E2E_CUDA(cudaEventRecord(hp->ev_start, stream));
     E2E_CUDA(cudaStreamWaitEvent(hp->aux, hp->ev_start, 0));
+    E2E_CUDA(cudaStreamWaitEvent(hp->up, hp->ev_start, 0));
     // from here on work is forked: every exit goes through the join below (errors are remembered, not returned at once)
     cudaError_t ce = cudaSuccess;
+    // a2 reads of a band's samples stay inside the wavelength range of its strips (spectrum_at: elements floor(t), floor(t) + 1,
+    // t = (lam / doppler - lam0) / dlam), so the tables travel on their own stream piece by piece in band order -- the part
+    // band 0 reads first, then what each later band adds to the uploaded interval, the unread rest last -- and band b
+    // waits only for its own pieces
+    {
+        std::vector<long long> ulo(nf, 0), uhi(nf, -1);          // uploaded interval [ulo, uhi) per table (uhi < 0: nothing yet)
+        for (int b = 0; b < part.n_bands && ce == cudaSuccess; ++b) {
+            for (int f = 0; f < nf && ce == cudaSuccess; ++f) {
+                const double la = part.lam_lo[(size_t)b * nf + f], lb = part.lam_hi[(size_t)b * nf + f];
+                if (!(la <= lb)) continue;
+                const e2e_spectrum_t& sp = spectra[f];
+                const int u = tab_of[f];
+                const double ta = (la / sp.doppler - sp.lam0) / sp.dlam, tb = (lb / sp.doppler - sp.lam0) / sp.dlam;
+                long long lo = 0, hi = sp.n;
+                if (is_fin(ta) && is_fin(tb) && std::fabs(ta) < 4e18 && std::fabs(tb) < 4e18) {
+                    lo = std::min<long long>(std::max<long long>((long long)std::floor(std::min(ta, tb)) - 2, 0), sp.n);
+                    hi = std::max<long long>(std::min<long long>((long long)std::floor(std::max(ta, tb)) + 4, sp.n), lo);
+                }
+                if (hi <= lo) continue;
+                if (uhi[u] < 0) { ce = upload(u, lo, hi, hp->up); ulo[u] = lo; uhi[u] = hi; continue; }
+                if (lo < ulo[u]) { ce = upload(u, lo, ulo[u], hp->up); ulo[u] = lo; }
+                if (hi > uhi[u] && ce == cudaSuccess) { ce = upload(u, uhi[u], hi, hp->up); uhi[u] = hi; }
+            }
+            if (ce == cudaSuccess) ce = cudaEventRecord(hp->ev_up[b % HostPipe::kEvents], hp->up);
+        }
+        for (int f = 0; f < nf && ce == cudaSuccess; ++f) {
+            if (tab_of[f] != f) continue;
+            if (uhi[f] < 0) { ce = upload(f, 0, spectra[f].n, hp->up); continue; }
+            ce = upload(f, 0, ulo[f], hp->up);
+            if (ce == cudaSuccess) ce = upload(f, uhi[f], spectra[f].n, hp->up);
+        }
+    }
+    if (ce == cudaSuccess) ce = cudaMemsetAsync(d_frame, 0, npix * 8, stream);
+    if (ce == cudaSuccess) ce = ctrl_reset(pl, d_ctrl, stream);
+    // the memset and the control block must be in place before the second stream's first band
+    if (ce == cudaSuccess) ce = cudaEventRecord(hp->ev_zero, stream);
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(hp->aux, hp->ev_zero, 0);
     int row0 = 0;
     for (int b = 0; b < part.n_bands && !rc && ce == cudaSuccess; ++b) {
         cudaStream_t cs = (b & 1) ? hp->aux : stream;
+        ce = cudaStreamWaitEvent(cs, hp->ev_up[b % HostPipe::kEvents], 0);
+        if (ce != cudaSuccess) break;
         QueueSel qs;
         qs.ctrl = d_ctrl; qs.head = b;
         qs.queue = part.d_queue + part.queue_off[b];
@@ -1561,9 +1629,10 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     // join: the caller's stream waits for the second stream, and the call for both and for the copies
     cudaError_t cj = cudaEventRecord(hp->ev_aux_done, hp->aux);
     if (cj == cudaSuccess) cj = cudaStreamWaitEvent(stream, hp->ev_aux_done, 0);
+    cudaError_t c0 = cudaStreamSynchronize(hp->up);
     cudaError_t c1 = cudaStreamSynchronize(hp->aux), c2 = cudaStreamSynchronize(stream), c3 = cudaStreamSynchronize(hp->copy);
     if (rc) return rc;
-    for (cudaError_t e : {ce, cj, c1, c2, c3})
+    for (cudaError_t e : {ce, cj, c0, c1, c2, c3})
         if (e != cudaSuccess) return fail_cuda(e, who);
     return E2E_OK;
 }

@@ -204,6 +204,7 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
         int* d_strips = nullptr;
         std::vector<int> queue_off;    // [n_bands + 1] into d_queue: the band's item ids in queue order (persistent launch)
         int* d_queue = nullptr;
+        std::vector<double> lam_lo, lam_hi;   // [n_bands][n_fibers] wavelength range of the band's samples of one fiber (lo > hi: none)
     };
     BandPart host, halves, host16;     // host16: fewer, equal bands for the host path's uint16 output (short copies)
     int n_phases_all = 0;          // phases before empty ones were dropped (colour x class)

@@ -234,10 +234,14 @@ E2E_API int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int
  * [ny*nx] array (pinned memory gives full PCIe speed).  The call copies the tables to the device, renders,
  * applies the detector stage a6 when det != NULL, copies the frame back and synchronises the stream before
  * returning.  Device scratch is taken from d_workspace, which must hold e2e_render_host_workspace_bytes() bytes.
- * The (fiber, order) strips are rendered in up to 8 row bands that share no pixel
+ * The (fiber, order) strips are rendered in up to 8 row bands (5 for the uint16 output) that share no pixel
  * (a band starts only where a strip's first row lies above every row of the strips before it): even bands run on
  * cuda_stream, odd bands on a second stream owned by the library, and as soon as a band is done a6 runs on its rows
- * and they travel to the host on the library's copy stream.  The frame is bit-reproducible call to call; against
+ * and they travel to the host on the library's copy stream.  The tables travel the other way on a fourth stream in
+ * the order the bands read them -- the wavelength range of band 0's strips first, then what each later band adds --
+ * and a band waits only for its own range; table elements no sample reads (outside every order's wavelength range
+ * after the Doppler factor) are not copied.  The host tables and h_frame must stay valid and unchanged until the
+ * call returns.  The frame is bit-reproducible call to call; against
  * e2e_render_frame it can differ in the last bit where strips overlap (the additions happen band by band).  Calls
  * on one (format, psf) pair are serialised. */
 E2E_API int e2e_render_host_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,

@@ -1557,8 +1557,8 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     cudaError_t ce = cudaSuccess;
     // a2 reads of a band's samples stay inside the wavelength range of its strips (spectrum_at: elements floor(t), floor(t) + 1,
     // t = (lam / doppler - lam0) / dlam), so the tables travel on their own stream piece by piece in band order -- the part
-    // band 0 reads first, then what each later band adds to the uploaded interval, the unread rest last -- and band b
-    // waits only for its own pieces
+    // band 0 reads first, then what each later band adds to the uploaded interval -- and band b waits only for its own
+    // pieces.  Elements outside every band's range are read by no sample and do not travel at all.
     {
         std::vector<long long> ulo(nf, 0), uhi(nf, -1);          // uploaded interval [ulo, uhi) per table (uhi < 0: nothing yet)
         for (int b = 0; b < part.n_bands && ce == cudaSuccess; ++b) {
@@ -1579,12 +1579,6 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
                 if (hi > uhi[u] && ce == cudaSuccess) { ce = upload(u, uhi[u], hi, hp->up); uhi[u] = hi; }
             }
             if (ce == cudaSuccess) ce = cudaEventRecord(hp->ev_up[b % HostPipe::kEvents], hp->up);
-        }
-        for (int f = 0; f < nf && ce == cudaSuccess; ++f) {
-            if (tab_of[f] != f) continue;
-            if (uhi[f] < 0) { ce = upload(f, 0, spectra[f].n, hp->up); continue; }
-            ce = upload(f, 0, ulo[f], hp->up);
-            if (ce == cudaSuccess) ce = upload(f, uhi[f], spectra[f].n, hp->up);
         }
     }
     if (ce == cudaSuccess) ce = cudaMemsetAsync(d_frame, 0, npix * 8, stream);

@@ -532,6 +532,62 @@ def test_render_frame_host_banded_pipeline(B):
         r.close()
 
 
+def test_render_frame_host_uploads_every_table_element_a_band_reads(B):
+    """the host path sends the spectrum tables piece by piece, in the order the row bands read them, and a band waits only
+    for its own wavelength range.  The workspace is poisoned with NaN before every call, so a band that read an element
+    before it arrived (or one that never travelled) shows up as NaN; cases: fibers that share one host table under
+    different Doppler factors, a table that covers only part of an order, a table shorter than any band's range, and a
+    Doppler factor that moves every sample off the table"""
+    import copy
+    import torch
+    base = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    sp0 = base.spectra[0]
+    n = sp0.flux.shape[0]
+    cases = []
+    # one host table, two Doppler factors (+-300 km/s).  A 33-MB table (the bench's grid step): the part no band reads travels
+    # last and takes ~0.6 ms, so an element a band needs that was left to that part is still NaN when the band reads it
+    big = W.espresso_like(n_obj_lines=300).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    a = copy.copy(big)
+    a.spectra = [Spectrum_like(big.spectra[0], doppler=1.0 + 1e-3), Spectrum_like(big.spectra[0], doppler=1.0 - 1e-3)]
+    cases.append(("shared table, two doppler factors", a))
+    b = copy.copy(base)                                              # tables that start / end inside the format's range
+    cut = n // 3
+    b.spectra = [Spectrum_like(sp0, flux=sp0.flux[cut:], lam0=sp0.lam0 + cut * sp0.dlam),
+                 Spectrum_like(base.spectra[1], flux=base.spectra[1].flux[:2 * cut])]
+    cases.append(("partial tables", b))
+    c = copy.copy(base)                                              # 2-element table; every sample of fiber 1 off its table
+    c.spectra = [Spectrum_like(sp0, flux=np.array([3.0, 5.0]), lam0=float(base.lam_min[3]), dlam=float(base.lam_max[3] - base.lam_min[3])),
+                 Spectrum_like(base.spectra[1], doppler=3.0)]
+    cases.append(("two-element table, fiber off its table", c))
+    for name, s in cases:
+        r = B.Renderer(s)
+        try:
+            dev = r.render().cpu().numpy()
+            tabs = {}
+            for sp in s.spectra:
+                tabs.setdefault(id(sp.flux), torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).pin_memory())
+            desc = B.spectra_array(s.spectra, [tabs[id(sp.flux)].data_ptr() for sp in s.spectra])
+            ws = torch.empty(B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc), dtype=torch.uint8, device="cuda")
+            for rep in range(2):
+                ws.view(torch.float64).fill_(float("nan"))
+                out = torch.full((s.ny, s.nx), float("nan"), dtype=torch.float64).pin_memory()
+                B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws)
+                H = out.numpy()
+                assert np.isfinite(H).all(), name
+                assert np.abs(H - dev).max() <= 1e-13 * max(dev.max(), 1e-300), name
+                assert np.array_equal(H == 0.0, dev == 0.0), name
+            if name.startswith("two-element"):
+                assert dev.max() > 0                                 # order 3 of fiber 0 is lit, nothing else
+        finally:
+            r.close()
+
+
+def Spectrum_like(sp, **kw):
+    d = dict(flux=sp.flux, lam0=sp.lam0, dlam=sp.dlam, scale=sp.scale, doppler=sp.doppler)
+    d.update(kw)
+    return W.Spectrum(**d)
+
+
 def test_render_frame_host_adu16_raw_frame(B):
     """e2e_render_frame_host_adu16 / _ex: the host path with the full detector stage (PRNU + dark maps, full well, cross-talk,
     ADC) delivering uint16 counts.  Bit-exact against the oracle's detector stage applied to the host path's own noise-free

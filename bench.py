@@ -384,9 +384,12 @@ def stage_rooflines(m, name: str, peak_tf: float, burst_tf: float):
         # two-kernel analytic path: the setup stage is cell_moment_kernel (a1-a3 fused + step 1); it writes one record per cell
         npt = int(kinfo["name"].split("<")[1].rstrip(">"))
         rec = 32.0 + 512.0 * npt
-        hbm("setup", m["stage_ms"]["ms_setup"], rec * n_cells + table_bytes * m["nbatch"],
-            "cell_moment_kernel: %d B per footprint cell written (header + moment tiles) + the spectrum tables read once; its step 1 is "
-            "%.3g fp64 flop per frame (2 x 8 (P+1) per sample)" % (rec, 2.0 * n_samples * alg["fma_per_sample"]), "cell_moment_kernel<%d>" % npt)
+        # large frames are zero-filled inside this kernel (no separate pass: ms_zero = 0), 8 B per pixel more
+        fused_zero = m["stage_ms"]["ms_zero"] <= 0
+        hbm("setup", m["stage_ms"]["ms_setup"], rec * n_cells + table_bytes * m["nbatch"] + (8.0 * npx if fused_zero else 0.0),
+            "cell_moment_kernel: %d B per footprint cell written (header + moment tiles) + the spectrum tables read once%s; its step 1 is "
+            "%.3g fp64 flop per frame (2 x 8 (P+1) per sample)" % (rec, " + the frame's zero-fill (8 B per pixel written)" if fused_zero else "",
+                                                                  2.0 * n_samples * alg["fma_per_sample"]), "cell_moment_kernel<%d>" % npt)
     else:
         hbm("setup", m["stage_ms"]["ms_setup"], 24.0 * n_samples + table_bytes * m["nbatch"],
             "24 B per sample written (x, y, w) + the spectrum tables read once", "setup_samples_kernel")

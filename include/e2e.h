@@ -384,7 +384,7 @@ E2E_API int64_t e2e_launch_count(void);
  * the recorded events, adds their elapsed times to the totals below and returns them; reset != 0 clears the
  * totals afterwards.  ms_* are summed device milliseconds, n_* the number of kernel launches in that stage. */
 typedef struct {
-    double ms_zero;      /* zero-fill of the frame (cudaMemsetAsync) */
+    double ms_zero;      /* zero-fill of the frame (cudaMemsetAsync); 0 where the two-kernel path zero-fills inside cell_moment_kernel (counted in ms_setup) */
     double ms_setup;     /* a1-a3 sample-setup kernel; on the two-kernel analytic path: cell_moment_kernel (a1-a3 fused with the
                             weighted phase moments of every footprint cell) */
     double ms_render;    /* a4-a5 render kernels (all phases); on the two-kernel path: cell_flush_kernel (the contraction + a5) */

@@ -865,9 +865,9 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         static SpectraParam no_spectra;
         const unsigned blocks = (unsigned)((ni + kCellWarps - 1) / kCellWarps);
         switch (P->moment_npt) {
-            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
-            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
-            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra); break;
+            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
+            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
+            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
         }
         count_launch();
         std::vector<int> counts(ni);
@@ -1068,10 +1068,13 @@ static CellStore cell_store(const e2e_plan* pl, unsigned* ctrl)
 }
 
 // kernel A of the two-kernel render: a1-a3 + the moments of every cell of the items ids[0 .. n) (nullptr: all items)
+// zero_frame (16-byte aligned, even pixel count; see fused_zero_ok): the kernel also zero-fills that frame
 static int launch_cell_moments(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, const e2e_spectrum_t* spectra, unsigned* ctrl,
-                               const int* ids, int n, cudaStream_t stream)
+                               const int* ids, int n, cudaStream_t stream, double* zero_frame = nullptr)
 {
     if (n <= 0) return E2E_OK;
+    double2* const zero = reinterpret_cast<double2*>(zero_frame);
+    const long long n_zero = zero_frame ? (long long)F->view.nx * F->view.ny / 2 : 0;
     const CellStore cs = cell_store(pl, ctrl);
     SpectraParam sp;
     memset(&sp, 0, sizeof(sp));
@@ -1080,7 +1083,7 @@ static int launch_cell_moments(const e2e_format* F, const e2e_psf* P, const e2e_
 #define E2E_CELL_CASE(NPT)                                                                                                     \
     case NPT:                                                                                                                   \
         cell_moment_kernel<NPT, false, true><<<blocks, kCellWarps * 32, sizeof(MomentWarpSmem<NPT, false>) * kCellWarps, stream>>>( \
-            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ids, n, P->mom, cs, nullptr, F->view, sp);                    \
+            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ids, n, P->mom, cs, nullptr, F->view, sp, zero, n_zero);      \
         break;
     switch (P->moment_npt) {
         E2E_CELL_CASE(2) E2E_CELL_CASE(3) E2E_CELL_CASE(4)
@@ -1301,7 +1304,11 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     qs.ctrl = (unsigned*)((char*)d_workspace + 3 * per);
     qs.n = pl->n_items;
     const bool persistent = choose_moment(fmt, psf);
-    if (!accumulate) {
+    // the two-kernel path zero-fills inside its first kernel (no separate pass over the frame) when the frame can be written
+    // in 16-byte elements and the kernel has enough CTAs to do it at speed
+    const bool fused_zero = !accumulate && use_split(fmt, psf, pl) && ((uintptr_t)d_frame & 15) == 0 &&
+                            ((size_t)fmt->view.nx * fmt->view.ny) % 2 == 0 && pl->n_items >= 4 * 148;
+    if (!accumulate && !fused_zero) {
         StageTimer tm(kStageZero, stream);
         E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
     }
@@ -1310,7 +1317,8 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
         const long long before = g_launches.load();
         if (persistent) E2E_CUDA(ctrl_reset(pl, qs.ctrl, stream));
         // the two-kernel path fuses a1-a3 into its first kernel, which is timed as this stage
-        if (use_split(fmt, psf, pl)) rc = launch_cell_moments(fmt, psf, pl, spectra, qs.ctrl, nullptr, pl->n_items, stream);
+        if (use_split(fmt, psf, pl))
+            rc = launch_cell_moments(fmt, psf, pl, spectra, qs.ctrl, nullptr, pl->n_items, stream, fused_zero ? d_frame : nullptr);
         else rc = launch_setup(fmt, pl, spectra, d_x, d_y, d_w, stream);
         if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_setup += g_launches.load() - before; }
         if (rc) return rc;

@@ -43,10 +43,15 @@ __global__ void __launch_bounds__(kCellWarps * 32)
 cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                    const Strip* __restrict__ strips, const Item* __restrict__ items, const int* __restrict__ ids, int n_items,
                    MomentParam Q, CellStore C, int* __restrict__ counts, const __grid_constant__ FormatView F,
-                   const __grid_constant__ SpectraParam SP)
+                   const __grid_constant__ SpectraParam SP, double2* __restrict__ zero, long long n_zero)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // zero-fill of the frame (accumulate = 0) rides along: this kernel leaves most of the HBM bandwidth unused and touches no
+    // pixel, and the flush kernel starts after it in stream order.  n_zero 16-byte elements, grid-stride.
+    if (!COUNT && zero)
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_zero; i += (long long)gridDim.x * blockDim.x)
+            __stcs(zero + i, make_double2(0.0, 0.0));
     const int slot = blockIdx.x * kCellWarps + warp;
     if (slot >= n_items) return;
     const int item_id = ids ? ids[slot] : slot;              // ids: the items of one row band (host path), else all of them

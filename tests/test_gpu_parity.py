@@ -115,6 +115,32 @@ def test_render_is_deterministic_and_accumulates(B):
         r.close()
 
 
+def test_render_overwrites_a_dirty_frame_on_every_zero_fill_path(B):
+    """accumulate = 0 must not depend on what the frame held.  Large frames of the two-kernel path are zero-filled inside
+    cell_moment_kernel (16-byte stores, grid-stride), small ones, frames that are not 16-byte aligned and every other kernel by
+    a memset: a NaN-poisoned frame must come out equal, bit for bit, to a render on top of an explicitly zeroed frame"""
+    import torch
+    big = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    for name, s in (("two-kernel path, fused zero-fill", big), ("small frame, memset", small_tiny(spp=8.0, lam=(5010.0, 5020.0)))):
+        r = B.Renderer(s)
+        try:
+            n = s.nx * s.ny
+            ref = torch.zeros((s.ny, s.nx), dtype=torch.float64, device="cuda")
+            r.render(frame=ref, accumulate=True)
+            buf = torch.full((n + 1,), float("nan"), dtype=torch.float64, device="cuda")
+            aligned = buf[:n].view(s.ny, s.nx)
+            r.render(frame=aligned)
+            assert torch.equal(aligned, ref), name
+            assert torch.isnan(buf[n]).item(), name                  # nothing written past the frame
+            buf.fill_(float("nan"))
+            odd = buf[1:].view(s.ny, s.nx)                           # 8-byte aligned only
+            r.render(frame=odd)
+            assert torch.equal(odd, ref), name + " (8-byte aligned frame)"
+            assert torch.isnan(buf[0]).item(), name
+        finally:
+            r.close()
+
+
 @pytest.mark.parametrize("psf_kw", [
     dict(fiber_dx_px=0.0, fiber_dy_px=0.0, sigma_x=0.9, sigma_y=1.3),      # P2: pure asymmetric gaussian
     dict(fiber_dx_px=4.0, fiber_dy_px=4.0, sigma_x=1.2, sigma_y=1.2),      # ESPRESSO-like PSF

@@ -39,7 +39,7 @@ C_ERFC, C_PSI = 60.0, 90.0
 KERNEL_SOURCES = {"render_moment_kernel": ("render_moment.cuh",), "render_tabcell_kernel": ("render_tabcell.cuh",),
                   "render_poly_kernel": ("render_poly.cuh",), "render_analytic_kernel": ("render_analytic.cuh",),
                   "render_tabulated_kernel": ("render_tabulated.cuh",), "detector_kernel": ("detector.cu",),
-                  "cell_flush_kernel": ("render_cells.cuh", "render_moment.cuh"),
+                  "cell_flush_kernel": ("render_cells.cuh", "render_moment.cuh"), "cell_flush_wide_kernel": ("render_cells.cuh", "render_moment.cuh"),
                   "cell_moment_kernel": ("render_cells.cuh", "render_moment.cuh", "setup.cuh"),
                   "setup_samples_kernel": ("setup.cuh",)}
 
@@ -379,7 +379,7 @@ def stage_rooflines(m, name: str, peak_tf: float, burst_tf: float):
                       "peak_source": hbm_src}
 
     hbm("zero", m["stage_ms"]["ms_zero"], 8.0 * npx, "8 B per pixel written", None)
-    split = kinfo["name"].startswith("cell_flush_kernel")
+    split = kinfo["name"].startswith("cell_flush_")
     if split:
         # two-kernel analytic path: the setup stage is cell_moment_kernel (a1-a3 fused + step 1); it writes one record per cell
         npt = int(kinfo["name"].split("<")[1].rstrip(">"))

@@ -752,7 +752,11 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         const long long nchunks = (N + 31) / 32;
         items_k2 += (nchunks + run_length(s % no, nchunks) - 1) / run_length(s % no, nchunks);
     }
-    const int K = items_k2 < kSmallFrameItems ? 4 : 2;
+#ifndef E2E_SMALL_K
+#define E2E_SMALL_K 8
+#endif
+    const int K = items_k2 < kSmallFrameItems ? ((P->kind == 0 && P->moment_npt > 0) ? E2E_SMALL_K : 4) : 2;
+    pl->small = K > 2;
     std::vector<std::vector<Item>> phases((size_t)n_colors * K);
     for (int s = 0; s < n_strips; ++s) {
         const int o = s % no;
@@ -1106,6 +1110,19 @@ static int launch_cell_flush(const e2e_format* F, const e2e_psf* P, const e2e_pl
     memset(&W, 0, sizeof(W));
     W.queue = queue; W.n = n; W.head = head; W.ctrl = ctrl;
     W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
+    if (pl->small) {
+        // a frame that cannot fill the GPU: one CTA of kWideWarps warps per item, the cell's tiles spread over the warps
+        switch (P->moment_npt) {
+            case 2: cell_flush_wide_kernel<2><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+            case 3: cell_flush_wide_kernel<3><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+            case 4: cell_flush_wide_kernel<4><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+            default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
+        }
+        count_launch();
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(e, "cell_flush_wide_kernel launch");
+        return E2E_OK;
+    }
     switch (P->moment_npt) {
         case 2: cell_flush_kernel<2><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
         case 3: cell_flush_kernel<3><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
@@ -1808,14 +1825,17 @@ int e2e_render_kernel_info(const e2e_format_t* fmt, const e2e_psf_t* psf, const 
         static const char* names[] = {"", "", "render_moment_kernel<2>", "render_moment_kernel<3>", "render_moment_kernel<4>"};
         static const char* map_names[] = {"", "", "render_moment_kernel<2, map>", "render_moment_kernel<3, map>", "render_moment_kernel<4, map>"};
         static const char* split_names[] = {"", "", "cell_flush_kernel<2>", "cell_flush_kernel<3>", "cell_flush_kernel<4>"};
+        static const char* wide_names[] = {"", "", "cell_flush_wide_kernel<2>", "cell_flush_wide_kernel<3>", "cell_flush_wide_kernel<4>"};
         const MomentParam& M = psf->mom;
         const int npt = psf->moment_npt, jp = (M.njt + 2) / 3, ip = (M.nit + 2) / 3;
         e2e_plan* pl = nullptr;
         const bool split = build_plan(const_cast<e2e_format*>(fmt), psf, &pl) == E2E_OK && use_split(fmt, psf, pl);
-        nm = split ? split_names[npt] : psf->is_map ? map_names[npt] : names[npt];
+        const bool wide = split && pl->small;
+        nm = wide ? wide_names[npt] : split ? split_names[npt] : psf->is_map ? map_names[npt] : names[npt];
         const double nodes = psf->is_map ? (M.gx > 1 ? 2.0 : 1.0) * (M.gy > 1 ? 2.0 : 1.0) : 1.0;
         // step 2 is redone for every column panel; tiles are 8 wide, power tiles 8 deep (render_moment.cuh)
         pc = nodes * 256.0 * M.T * (2.0 * npt * M.nit * jp + 2.0 * M.nit * M.njt);         // step 2 (redone per row panel) + step 3
+        if (wide) pc = 256.0 * M.T * (2.0 * npt + 2.0) * M.nit * M.njt;                      // step 2 redone per 8 x 8 tile
         // step 1 (npt DMMAs per 4 samples and node) + powers: on the two-kernel path they belong to cell_moment_kernel, not to the
         // kernel named here
         ps = split ? 0.0 : nodes * 64.0 * npt + 8.0 * npt + 8.0;

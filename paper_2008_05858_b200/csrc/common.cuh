@@ -185,6 +185,7 @@ struct e2e_plan {                  // schedule for one (format, footprint) pair;
     e2e::Item* d_items = nullptr;
     int n_items = 0;
     int n_colors = 0;
+    bool small = false;            // a frame whose items cannot fill the GPU (K > 2 run classes): wide CTAs render its items
     // dependency lists of the persistent render launch (render_moment.cuh): item i waits for dep_idx[dep_off[i] .. dep_off[i+1])
     // -- every item earlier in the queue (= lower index) whose pixels may overlap its own
     int* d_dep_off = nullptr;

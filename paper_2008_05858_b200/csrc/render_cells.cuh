@@ -210,4 +210,87 @@ cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__
     queue_done(W, W.ctrl, item_id, lane);
 }
 
+// ---- small frames (a single strip, a few hundred items): the launch cannot fill the GPU, the frame time is the serial chain of
+// cells that share pixels, and one warp per cell (180 dependent-ish DMMAs, ~4 us) is the wrong shape.  Here one CTA of kWideWarps
+// warps renders an item: every warp owns 8 x 8 tiles of the window (tile w, w + kWideWarps, ...), computes Y_t for its column tile
+// itself (redundantly across the row tiles) and contracts it with its row tile's cy: (2 NPT + 2) T DMMAs per tile and cell
+// instead of 30 T in one warp.  Every output element sees the same DMMA sequence as in moment_flush_cell (terms in order, k-slot x
+// then y; Y_t by power tile, x then y): the frame has the same bits.  Consecutive cells of the item overlap, and their tiles
+// belong to different warps, so a CTA barrier (instead of __syncwarp) orders one cell's reductions before the next cell's.
+constexpr int kWideWarps = 9;
+template <int NPT>
+__global__ void __launch_bounds__(kWideWarps * 32)
+cell_flush_wide_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny)
+{
+    __shared__ int s_item;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lq = lane >> 2, lr = lane & 3;
+    if (warp == 0) {
+        const int id = queue_ticket(W, W.ctrl, lane);
+        if (lane == 0) s_item = id;
+    }
+    __syncthreads();
+    const int item_id = s_item;
+    if (item_id < 0) return;
+    const long long c0 = C.cell_off[item_id], c1 = C.cell_off[item_id + 1];
+    // the first record travels while warp 0 waits for the item's dependencies (records are final before this launch)
+    CellHeader hn = {};
+    double2 mn[NPT] = {};
+    auto fetch = [&](long long cell) {
+        hn = C.hdr[cell];
+        const double* src = C.mom + ((size_t)cell * 32 + lane) * (2 * NPT);
+#pragma unroll
+        for (int qt = 0; qt < NPT; ++qt) mn[qt] = __ldg(reinterpret_cast<const double2*>(src + 2 * qt));
+    };
+    if (c0 < c1) fetch(c0);
+    if (warp == 0) queue_wait(W.ctrl, item_id);
+    __syncthreads();
+    const int ntile = Q.nit * Q.njt;
+    for (long long cell = c0; cell < c1; ++cell) {
+        const CellHeader h = hn;
+        double mc[NPT][2];
+#pragma unroll
+        for (int qt = 0; qt < NPT; ++qt) { mc[qt][0] = mn[qt].x; mc[qt][1] = mn[qt].y; }
+        if (cell + 1 < c1) fetch(cell + 1);
+        const bool dead = h.i1 < 0 || h.i0 >= nx || h.j1 < 0 || h.j0 >= ny || h.i1 < h.i0 || h.j1 < h.j0;
+        const int rlim = min(h.j1, ny - 1), clim = min(h.i1, nx - 1);
+        for (int tile = warp; tile < ntile && !dead; tile += kWideWarps) {
+            const int it = tile / Q.njt, jt = tile - it * Q.njt;
+            if (h.i0 + 8 * it > clim || h.j0 + 8 * jt > rlim) continue;
+            double o0 = 0.0, o1 = 0.0;
+#pragma unroll 2
+            for (int t = 0; t < Q.T; ++t) {
+                const double2 cy = __ldg(Q.fy + ((size_t)(h.yb * Q.T + t) * Q.njt + jt) * 32 + lane);
+                const double2* fx = Q.fx + ((size_t)(t * Q.nit + it) * NPT) * 32 + lane;
+                double2 cx[NPT];
+#pragma unroll
+                for (int qt = 0; qt < NPT; ++qt) cx[qt] = __ldg(fx + qt * 32);
+                double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+                for (int qt = 0; qt < NPT; ++qt) {
+                    dmma_m8n8k4(y0, y1, cx[qt].x, mc[qt][0]);
+                    dmma_m8n8k4(y0, y1, cx[qt].y, mc[qt][1]);
+                }
+                dmma_m8n8k4(o0, o1, y0, cy.x);
+                dmma_m8n8k4(o0, o1, y1, cy.y);
+            }
+            const int col = h.i0 + 8 * it + lq;
+            const int row = h.j0 + 8 * jt + 2 * lr;
+            if (col >= 0 && col <= clim) {
+                if (row >= 0 && row <= rlim) atomicAdd(frame + (size_t)row * nx + col, o0);
+                if (row + 1 >= 0 && row + 1 <= rlim) atomicAdd(frame + (size_t)(row + 1) * nx + col, o1);
+            }
+        }
+        __syncthreads();                                       // the next cell's window overlaps this one
+    }
+    // every warp's reductions are performed before any successor's counter moves
+    __threadfence();
+    __syncthreads();
+    if (warp == 0) {
+        unsigned* const pend = W.ctrl + kCtrlHeads;
+        const int s1 = W.succ_off[item_id + 1];
+        for (int d = W.succ_off[item_id] + lane; d < s1; d += 32) red_release_dec_u32(pend + W.succ_idx[d]);
+    }
+}
+
 }  // namespace e2e

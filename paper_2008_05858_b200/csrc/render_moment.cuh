@@ -92,16 +92,25 @@ __device__ __forceinline__ void red_release_dec_u32(unsigned* p)
 // is held by a warp that is already running (deadlock freedom).  The wait is a warp-uniform spin on ONE word (a per-lane
 // loop over dependency flags made ptxas spill 500 bytes of the render loop's state at 96 registers).  Returns -1 when the
 // queue is exhausted.
-__device__ __forceinline__ int queue_take(const QueueParam& W, unsigned* ctrl, int lane)
+// ticket: the next item of the queue (-1: none left); the item may not touch the frame before queue_wait returns
+__device__ __forceinline__ int queue_ticket(const QueueParam& W, unsigned* ctrl, int lane)
 {
     unsigned qpos = 0;
     if (lane == 0) qpos = atomicAdd(ctrl + W.head, 1u);
     qpos = __shfl_sync(0xffffffffu, qpos, 0);
     if (qpos >= (unsigned)W.n) return -1;
-    const int item_id = W.queue ? W.queue[qpos] : (int)qpos;
+    return W.queue ? W.queue[qpos] : (int)qpos;
+}
+__device__ __forceinline__ void queue_wait(unsigned* ctrl, int item_id)
+{
     const unsigned* f = ctrl + kCtrlHeads + item_id;
     while (ld_acquire_u32(f) != 0u) __nanosleep(100);
     __syncwarp();
+}
+__device__ __forceinline__ int queue_take(const QueueParam& W, unsigned* ctrl, int lane)
+{
+    const int item_id = queue_ticket(W, ctrl, lane);
+    if (item_id >= 0) queue_wait(ctrl, item_id);
     return item_id;
 }
 

@@ -75,10 +75,10 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
     // the open cell is complete: hand it to the flush kernel
     auto emit = [&]() {
         if (!COUNT) {
-            if (lane == 0) {
-                CellHeader h;
-                h.i0 = cI0; h.i1 = cI1; h.j0 = cJ0; h.j1 = cJ1; h.yb = cYb; h.pad[0] = h.pad[1] = h.pad[2] = 0;
-                C.hdr[cell] = h;
+            if (lane == 0) {                                   // the header as two 16-byte stores
+                int4* hd = reinterpret_cast<int4*>(C.hdr + cell);
+                hd[0] = make_int4(cI0, cI1, cJ0, cJ1);
+                hd[1] = make_int4(cYb, 0, 0, 0);
             }
             double* dst = C.mom + ((size_t)cell * 32 + lane) * (2 * NPT);
 #pragma unroll
@@ -156,22 +156,23 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
             const int pend = min(pos + run, nb);
             if (!COUNT) {
                 __syncwarp();                                  // the previous run's step-1 reads of vy are done
-                const double d2 = dl * dl, d3 = d2 * dl, d4 = d2 * d2;
-                S.vy[0 * kMomLdk + lane] = 1.0;
-                S.vy[1 * kMomLdk + lane] = dl;
+                // samples outside the run [pos, pend) stage zeros: the k-steps at the run's ends need no select
+                const bool mine = lane >= pos && lane < pend;
+                const double d1 = mine ? dl : 0.0;
+                const double d2 = d1 * d1, d3 = d2 * d1, d4 = d2 * d2;
+                S.vy[0 * kMomLdk + lane] = mine ? 1.0 : 0.0;
+                S.vy[1 * kMomLdk + lane] = d1;
                 S.vy[2 * kMomLdk + lane] = d2;
                 S.vy[3 * kMomLdk + lane] = d3;
                 S.vy[4 * kMomLdk + lane] = d4;
-                S.vy[5 * kMomLdk + lane] = d4 * dl;
+                S.vy[5 * kMomLdk + lane] = d4 * d1;
                 S.vy[6 * kMomLdk + lane] = d4 * d2;
                 S.vy[7 * kMomLdk + lane] = d4 * d3;
                 __syncwarp();
                 // ---- step 1: MT += VX VY^T over the samples [pos, pend)
                 for (int ks = pos >> 2; ks <= (pend - 1) >> 2; ++ks) {
                     const int ksamp = 4 * ks + lr;
-                    const bool in = ksamp >= pos && ksamp < pend;
-                    const double vv = S.vy[lq * kMomLdk + ksamp];
-                    const double a = in ? vv : 0.0;
+                    const double a = S.vy[lq * kMomLdk + ksamp];
                     double b[NPT];
 #pragma unroll
                     for (int qt = 0; qt < NPT; ++qt) b[qt] = S.vx[(8 * qt + lq) * kMomLdk + ksamp];

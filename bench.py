@@ -540,7 +540,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "data": "synthetic",
             "config": {"workload": m["wname"], "n_samples": n_samples, "contributions": contrib, "footprint_nominal_px": nominal,
                        "chord_nodes_Q": info["n_nodes"], "frame": [scene.ny, scene.nx], "stages": "a1-a6 (zero-fill, setup, render, detector)",
-                       "l2": "inputs larger than L2: sample arrays %.0f MB + frame %.0f MB vs 126 MB L2" % (n_samples * 24 / 1e6, scene.nx * scene.ny * 8 / 1e6),
+                       "l2": ("inputs larger than L2: cell records %.0f MB + frame %.0f MB vs 126 MB L2" % (m["n_cells"] * (32 + 512 * int(m["kinfo"]["name"].split("<")[1].rstrip(">"))) / 1e6, scene.nx * scene.ny * 8 / 1e6))
+                             if m["kinfo"]["name"].startswith("cell_flush_") else
+                             ("inputs larger than L2: sample arrays %.0f MB + frame %.0f MB vs 126 MB L2" % (n_samples * 24 / 1e6, scene.nx * scene.ny * 8 / 1e6)),
                        "multi_gpu": "replicas only", "others": others or None},
             "frame_ms": m["ms_step"], "samples_per_s": world * n_samples / (m["ms_step"] * 1e-3),
             "stage_ms_per_step": m["stage_ms"], "stage_roofline": {k: v for k, v in stages.items() if k != "render"},

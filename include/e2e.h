@@ -192,10 +192,10 @@ typedef struct {
     double doppler;                 /* 1 + v/c: the fiber sees S(lam / doppler) */
 } e2e_spectrum_t;
 
-/* bytes of device scratch e2e_render_frame needs for this (format, psf): the per-sample arrays x, y, w of
- * step a1-a3 (24 B per sample; the kernels that materialise the samples), the control block of the render queue (4 B per
- * work item) and, on the two-kernel analytic path, one record per footprint cell (32 B + 512 B per power tile: 1056 B per
- * cell for the ESPRESSO-like PSF, 1.6 GB per frame).  256-byte aligned workspace required. */
+/* bytes of device scratch e2e_render_frame needs for this (format, psf): the control block of the render queue (4 B per
+ * work item) and either, on the two-kernel analytic path (which never materialises the samples), one record per footprint
+ * cell (32 B + 512 B per power tile: 1056 B per cell for the ESPRESSO-like PSF, 1.6 GB per frame) or, for the other
+ * kernels, the per-sample arrays x, y, w of step a1-a3 (24 B per sample).  256-byte aligned workspace required. */
 E2E_API int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, size_t* bytes);
 
 /* a1-a3 only, for one (fiber, order): writes lam, x, y, w of its samples to DEVICE arrays of length

@@ -1062,6 +1062,13 @@ static size_t cell_bytes(const e2e_format* F, const e2e_psf* P, const e2e_plan* 
     return use_split(F, P, pl) ? cell_hdr_bytes(pl) + cell_mom_bytes(pl, P) : 0;
 }
 
+// bytes of the per-sample arrays x | y | w at the head of the workspace: none on the two-kernel path, which never materialises
+// the samples
+static size_t sample_arrays_bytes(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl)
+{
+    return use_split(F, P, pl) ? 0 : 3 * sample_array_bytes(pl->total_samples);
+}
+
 static CellStore cell_store(const e2e_plan* pl, unsigned* ctrl)
 {
     CellStore cs;
@@ -1271,7 +1278,7 @@ int e2e_render_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, si
     e2e_plan* pl = nullptr;
     int rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
-    *bytes = 3 * sample_array_bytes(pl->total_samples) + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl);
+    *bytes = sample_arrays_bytes(fmt, psf, pl) + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl);
     return E2E_OK;
 }
 
@@ -1312,13 +1319,14 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     if (rc) return rc;
     const size_t per = sample_array_bytes(pl->total_samples);
     if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace NULL or not 256-byte aligned");
-    if (workspace_bytes < 3 * per + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
+    const size_t arrays = sample_arrays_bytes(fmt, psf, pl);
+    if (workspace_bytes < arrays + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, "render_frame: workspace too small");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
-    double* d_x = (double*)d_workspace;
-    double* d_y = (double*)((char*)d_workspace + per);
-    double* d_w = (double*)((char*)d_workspace + 2 * per);
+    double* d_x = arrays ? (double*)d_workspace : nullptr;
+    double* d_y = arrays ? (double*)((char*)d_workspace + per) : nullptr;
+    double* d_w = arrays ? (double*)((char*)d_workspace + 2 * per) : nullptr;
     QueueSel qs;
-    qs.ctrl = (unsigned*)((char*)d_workspace + 3 * per);
+    qs.ctrl = (unsigned*)((char*)d_workspace + arrays);
     qs.n = pl->n_items;
     const bool persistent = choose_moment(fmt, psf);
     // the two-kernel path zero-fills inside its first kernel (no separate pass over the frame) when the frame can be written
@@ -1567,11 +1575,12 @@ static int render_frame_host_impl(const e2e_format_t* fmt, const e2e_psf_t* psf,
     // to the host on the library's copy stream while the next bands render
     const size_t per = sample_array_bytes(pl->total_samples);
     const bool split = use_split(fmt, psf, pl);
-    if (workspace_bytes - used < 3 * per + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
-    double* d_x = (double*)p;
-    double* d_y = (double*)(p + per);
-    double* d_w = (double*)(p + 2 * per);
-    unsigned* d_ctrl = (unsigned*)(p + 3 * per);
+    const size_t arrays = sample_arrays_bytes(fmt, psf, pl);
+    if (workspace_bytes - used < arrays + ctrl_bytes(pl) + cell_bytes(fmt, psf, pl)) return fail(E2E_ERR_WORKSPACE, w + ": workspace too small");
+    double* d_x = arrays ? (double*)p : nullptr;
+    double* d_y = arrays ? (double*)(p + per) : nullptr;
+    double* d_w = arrays ? (double*)(p + 2 * per) : nullptr;
+    unsigned* d_ctrl = (unsigned*)(p + arrays);
     if (part.n_bands > kCtrlHeads) return fail(E2E_ERR_UNSUPPORTED, w + ": too many row bands");
     std::lock_guard<std::mutex> lk(hp->mu);            // one banded call at a time owns the copy stream and its events
     // bands share no pixel (build_plan): even bands on the caller's stream, odd bands on the library's second stream

@@ -217,6 +217,25 @@ E2E_API int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, cons
                      double* d_frame, int32_t accumulate, void* d_workspace, size_t workspace_bytes,
                      void* cuda_stream);
 
+/* e2e_render_frame for callers that cannot allocate device memory or hold a workspace (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same arguments without the workspace: the scratch of the
+ * two-kernel analytic render (queue control block + one record per footprint cell, see e2e_render_workspace_bytes) lives in
+ * ONE static device array of E2E_NOALLOC_SCRATCH_BYTES bytes inside the library; every GPU that loads the library holds it
+ * until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating routine; the frame has the bits
+ * of e2e_render_frame's.  Conditions (else an error and nothing is launched):
+ *   - the cached schedule of this (format, psf) pair exists: call e2e_render_workspace_bytes(fmt, psf, &n) once at set-up
+ *     (that call builds it and allocates)                                                      -> E2E_ERR_UNSUPPORTED;
+ *   - the pair renders with the two-kernel analytic path (analytic PSF with constant sigma, dense sampling)
+ *                                                                                              -> E2E_ERR_UNSUPPORTED;
+ *   - its scratch fits: n from e2e_render_workspace_bytes <= E2E_NOALLOC_SCRATCH_BYTES (frames up to ~20 000 footprint
+ *     cells: a single order, not a full echellogram)                                           -> E2E_ERR_WORKSPACE.
+ * Every call on a GPU shares the one array: calls that overlap on the GPU (different streams, different threads) RACE on it
+ * and corrupt each other's frames -- serialise them on one stream or with events.  Nothing must be cleared by the caller:
+ * each call rewrites the control block and every record it reads.  Asynchronous on cuda_stream. */
+#define E2E_NOALLOC_SCRATCH_BYTES (32u << 20)   /* 32 MiB */
+E2E_API int e2e_render_frame_noalloc(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra,
+                             double* d_frame, int32_t accumulate, void* cuda_stream);
+
 /* Batch render on fixed geometry ("[the database] can be computed only once and used for
  * different simulation scenarios"): n_frames frames of the SAME format and PSF, each with its own spectra --
  * e.g. object / flat / Fabry-Perot exposures, or the Doppler-shifted copies of one spectrum (BJ "Precision/RV sweep").

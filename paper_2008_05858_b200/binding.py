@@ -26,7 +26,8 @@ SYMBOLS = ["e2e_last_error", "e2e_version", "e2e_format_create", "e2e_format_des
            "e2e_apply_detector_adu16", "e2e_measure_fp64_peak",
            "e2e_launch_count", "e2e_profile_enable", "e2e_profile_read", "e2e_render_kernel_info",
            "e2e_render_algorithmic_fma", "e2e_render_frames_workspace_bytes", "e2e_render_frames",
-           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check", "e2e_spectrograph_format", "e2e_probe_fp64_pipe"]
+           "e2e_render_frame_host_ex", "e2e_render_frame_host_adu16", "e2e_plan_check", "e2e_spectrograph_format", "e2e_probe_fp64_pipe",
+           "e2e_render_frame_noalloc"]
 
 
 class E2EError(RuntimeError):
@@ -133,6 +134,8 @@ def load():
     L.e2e_setup_samples.argtypes = [vp, C.POINTER(SpectrumDesc), i32, i32, vp, vp, vp, vp, i64, vp]
     L.e2e_render_frame.restype = C.c_int
     L.e2e_render_frame.argtypes = [vp, vp, C.POINTER(SpectrumDesc), vp, i32, vp, C.c_size_t, vp]
+    L.e2e_render_frame_noalloc.restype = C.c_int
+    L.e2e_render_frame_noalloc.argtypes = [vp, vp, C.POINTER(SpectrumDesc), vp, i32, vp]
     L.e2e_render_host_workspace_bytes.restype = C.c_int
     L.e2e_render_host_workspace_bytes.argtypes = [vp, vp, C.POINTER(SpectrumDesc), C.POINTER(C.c_size_t)]
     L.e2e_render_frame_host.restype = C.c_int
@@ -329,6 +332,15 @@ def e2e_render_frame(fmt: Format, psf: Psf, spectra_desc, d_frame, accumulate: b
     _check(load().e2e_render_frame(fmt.handle, psf.handle, spectra_desc, int(d_frame.data_ptr()), int(bool(accumulate)),
                                    int(d_workspace.data_ptr()), int(d_workspace.numel() * d_workspace.element_size()),
                                    _stream_ptr(stream)))
+
+
+NOALLOC_SCRATCH_BYTES = 32 << 20   # E2E_NOALLOC_SCRATCH_BYTES of include/e2e.h
+
+
+def e2e_render_frame_noalloc(fmt: Format, psf: Psf, spectra_desc, d_frame, accumulate: bool, stream=None):
+    """e2e_render_frame with the scratch in the library's static device array (no workspace, no allocation)."""
+    _check(load().e2e_render_frame_noalloc(fmt.handle, psf.handle, spectra_desc, int(d_frame.data_ptr()), int(bool(accumulate)),
+                                           _stream_ptr(stream)))
 
 
 def e2e_render_frames_workspace_bytes(fmt: Format, psf: Psf, n_frames: int) -> int:

@@ -1380,6 +1380,85 @@ int e2e_render_frame(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_sp
     return rc;
 }
 
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// e2e_render_frame_noalloc: the two-kernel render with its scratch (queue control block + cell records) in a file-scope device
+// array instead of a caller workspace, for callers that cannot allocate.  The array exists once per GPU that loads the
+// library, for the life of the process.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[E2E_NOALLOC_SCRATCH_BYTES];
+
+// In host code `g_noalloc_scratch` is a host-side stand-in for the symbol, not a device address: the kernels get the address
+// cudaGetSymbolAddress returns, resolved once per device with that device current.
+static int noalloc_scratch_ptr(unsigned char** out)
+{
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned char* ptr[kMaxDev] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "render_frame_noalloc: cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDev) return fail(E2E_ERR_UNSUPPORTED, "render_frame_noalloc: device ordinal above 63");
+    std::lock_guard<std::mutex> lk(mu);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return fail_cuda(e, "render_frame_noalloc: cudaGetSymbolAddress");
+        if (!p || ((uintptr_t)p & 255) != 0) return fail(E2E_ERR_CUDA, "render_frame_noalloc: scratch symbol has no aligned device address");
+        ptr[dev] = (unsigned char*)p;
+    }
+    *out = ptr[dev];
+    return E2E_OK;
+}
+
+// the cached schedule of (format, psf), or nullptr: a lookup only (build_plan would allocate)
+static e2e_plan* find_plan(e2e_format* F, const e2e_psf* P)
+{
+    std::lock_guard<std::mutex> lock(F->plan_mu);
+    const int nyb_key = (P->kind == 0 && P->moment_npt > 0 && !P->is_map) ? P->mom.nyb : 0;
+    for (auto& p : F->plans)
+        if (p->hbx == P->hbx && p->hby == P->hby && p->nyb == nyb_key) return p.get();
+    return nullptr;
+}
+
+extern "C" {
+
+int e2e_render_frame_noalloc(const e2e_format_t* fmt, const e2e_psf_t* psf, const e2e_spectrum_t* spectra, double* d_frame,
+                             int32_t accumulate, void* cuda_stream)
+{
+    if (!fmt || !psf || !d_frame) return fail(E2E_ERR_INVALID_ARG, "render_frame_noalloc: NULL argument");
+    if (psf->nx != fmt->view.nx || psf->ny != fmt->view.ny)
+        return fail(E2E_ERR_INVALID_ARG, "render_frame_noalloc: psf was created for another detector size");
+    int rc = check_spectra(fmt, spectra, "render_frame_noalloc");
+    if (rc) return rc;
+    e2e_plan* pl = find_plan(const_cast<e2e_format*>(fmt), psf);
+    if (!pl)
+        return fail(E2E_ERR_UNSUPPORTED, "render_frame_noalloc: no cached schedule for this (format, psf): call e2e_render_workspace_bytes "
+                                         "once at set-up (that call builds it and allocates)");
+    if (!use_split(fmt, psf, pl))
+        return fail(E2E_ERR_UNSUPPORTED, "render_frame_noalloc: only the two-kernel analytic render (dense sampling, constant analytic PSF) "
+                                         "has a no-allocation form");
+    const size_t need = ctrl_bytes(pl) + cell_bytes(fmt, psf, pl);
+    if (need > (size_t)E2E_NOALLOC_SCRATCH_BYTES)
+        return fail(E2E_ERR_WORKSPACE, "render_frame_noalloc: this frame needs " + std::to_string(need) + " bytes of scratch, the static array holds " +
+                                           std::to_string((size_t)E2E_NOALLOC_SCRATCH_BYTES) + " (E2E_NOALLOC_SCRATCH_BYTES): use e2e_render_frame");
+    unsigned char* scratch = nullptr;
+    rc = noalloc_scratch_ptr(&scratch);
+    if (rc) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    unsigned* ctrl = (unsigned*)scratch;
+    // the array keeps the last call's contents: the control block is rewritten from the plan's template here, and
+    // cell_moment_kernel writes every cell record cell_flush_kernel reads
+    const bool fused_zero = !accumulate && ((uintptr_t)d_frame & 15) == 0 && ((size_t)fmt->view.nx * fmt->view.ny) % 2 == 0 &&
+                            pl->n_items >= 4 * 148;
+    if (!accumulate && !fused_zero) E2E_CUDA(cudaMemsetAsync(d_frame, 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
+    E2E_CUDA(ctrl_reset(pl, ctrl, stream));
+    rc = launch_cell_moments(fmt, psf, pl, spectra, ctrl, nullptr, pl->n_items, stream, fused_zero ? d_frame : nullptr);
+    if (rc) return rc;
+    return launch_cell_flush(fmt, psf, pl, d_frame, ctrl, nullptr, pl->n_items, 0, stream);
+}
+
 int e2e_render_frames_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_frames, size_t* bytes)
 {
     if (n_frames < 1 || n_frames > 65535) return fail(E2E_ERR_INVALID_ARG, "render_frames_workspace_bytes: n_frames must be 1..65535");

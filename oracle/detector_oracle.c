@@ -4,26 +4,32 @@
  * TEST INFRASTRUCTURE ONLY (see e2e_oracle.c).  P:79: "photon noise and all other specific detector noises
  * (e.g. dark current, RON, pixels non-uniform response and cross-talk) are added on the final synthetic echellogram".
  * The paper names the noises only; the algorithm below is reading G12 of DESIGN.md as re-specified in round 2
- * ("G12 (round 2)": a fixed number of Philox blocks per pixel and no rejection loop), made of
+ * (G12: a fixed number of Philox blocks and no rejection loop; pixel pairs share the blocks), made of
  * IEEE-exact operations (+ - * / sqrt fma, integer ops) only, so that a second implementation can match it bit for bit:
  *
  *   mu       = max(0, gain * frame[p] + dark_e)
- *   (z1, z2) = Box-Muller pair from block 0 of the pixel's Philox stream:
- *                u1 = U(w0, w1), u2 = U(w2, w3),  rho = sqrt(-2 log u1),  z1 = rho cos(2 pi u2),  z2 = rho sin(2 pi u2)
+ *   Pixels are keyed in PAIRS (G12 round 3): pixel p belongs to pair q = p >> 1 with parity s = p & 1, and the two pixels of a
+ *   pair share each Philox block of the pair's stream -- every block yields two independent variates, one per pixel:
+ *   z1       = read-noise normal from block 0 of the pair:  u1 = U(w0, w1), u2 = U(w2, w3),  rho = sqrt(-2 log u1),
+ *                z1 = rho cos(2 pi u2) for s = 0,  rho sin(2 pi u2) for s = 1      (the two halves of one Box-Muller pair)
  *   n        = Poisson(mu):  0 if mu == 0;
- *              mu < 64:  inversion by sequential search with ONE uniform v = U(w0, w1) of block 1:
+ *              mu < 64:  inversion by sequential search with ONE uniform of block 1 of the pair, v = U(w0, w1) for s = 0,
+ *                        U(w2, w3) for s = 1:
  *                        p = exp(-mu), F = p, n = 0;  while (v > F and n < 255) { n += 1; p = (p mu) (1/n); F += p; }
- *              else      max(0, floor(mu + sqrt(mu) z2 + (z2^2 - 1)/6 + 1/2))      (normal + first Cornish-Fisher term:
+ *              else      max(0, floor(mu + sqrt(mu) z2 + (z2^2 - 1)/6 + 1/2)) with z2 from block 2 of the pair, formed like z1 from
+ *                        block 0 (cos half for s = 0, sin half for s = 1)           (normal + first Cornish-Fisher term:
  *                        mean mu, skewness 1/sqrt(mu) as Poisson, variance mu + 5/36 -- an approximation, 0.2 % high at mu = 64)
  *   out[p]   = (n + bias) + ron_e * z1
  *
- * Random stream of pixel p: Philox4x32-10 (Salmon et al., SC'11), key = (seed_lo, seed_hi),
- * counter = (p_lo, p_hi, block, 0); a uniform takes two 32-bit words: U(hi, lo) = ((hi >> 5) * 2^26 + (lo >> 6) + 1/2) * 2^-53
+ * Random stream of pair q: Philox4x32-10 (Salmon et al., SC'11), key = (seed_lo, seed_hi),
+ * counter = (q_lo, q_hi, block, 0); a uniform takes two 32-bit words: U(hi, lo) = ((hi >> 5) * 2^26 + (lo >> 6) + 1/2) * 2^-53
  * in (0, 1).  log, exp, sin and cos are spelled out below (no libm call), every a*b+c that is meant fused is written fma().
  *
  * Pins (tests/test_oracle_detector.py): Philox known-answer vectors of the Random123 distribution; orc_log / orc_exp /
- * orc_sin2pi against libm; Box-Muller pair: moments, independence, tail; Poisson pmf (chi-square) at several mu and the
- * mean / variance / third cumulant across both branches; independence of how the frame is split into calls (pixel_offset);
+ * orc_sin2pi against libm; which words of which block feed which pixel (libm / scipy restatement); Box-Muller pair: moments,
+ * independence of the two pixels of a pair, tail; Poisson pmf (chi-square) at several mu and the mean / variance / third cumulant
+ * across both branches; the two pixels of a pair: counts uncorrelated with each other and with the read noise, in both branches;
+ * independence of how the frame is split into calls (pixel_offset, even and odd: a pair may straddle two calls);
  * full stage: reductions, (prnu, dark) grid, ADC moments, saturation; cross-talk: matrix form, charge bookkeeping.
  */
 #include <math.h>
@@ -50,11 +56,11 @@ void orc_philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint3
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* block `block` of pixel `pixel`: 4 words */
-static void pixel_block(uint64_t seed, uint64_t pixel, uint32_t block, uint32_t w[4])
+/* block `block` of pixel pair `pair`: 4 words */
+static void pair_block(uint64_t seed, uint64_t pair, uint32_t block, uint32_t w[4])
 {
     uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
-    uint32_t ctr[4] = {(uint32_t)pixel, (uint32_t)(pixel >> 32), block, 0u};
+    uint32_t ctr[4] = {(uint32_t)pair, (uint32_t)(pair >> 32), block, 0u};
     orc_philox4x32_10(ctr, key, w);
 }
 static double uniform53(uint32_t hi, uint32_t lo)
@@ -153,19 +159,26 @@ double orc_sin2pi(double y)
     return y * P;
 }
 
+/* the standard normal of pixel `pixel` from block `block` of its pair: one half of the block's Box-Muller pair */
+static double pair_normal(uint64_t seed, uint64_t pixel, uint32_t block)
+{
+    uint32_t w[4];
+    pair_block(seed, pixel >> 1, block, w);
+    double u1 = uniform53(w[0], w[1]), u2 = uniform53(w[2], w[3]);
+    double rho = sqrt(-2.0 * orc_log(u1));
+    return (pixel & 1u) ? rho * orc_sin2pi(u2) : rho * orc_sin2pi(u2 + 0.25);      /* sin half : cos half */
+}
+
 /* the draws for one pixel: z1 (read noise), n (Poisson count) */
 void orc_detector_draws(const orc_detector_t *d, uint64_t pixel, double mu, double *z1_out, double *n_out)
 {
-    uint32_t w[4];
-    pixel_block(d->seed, pixel, 0u, w);
-    double u1 = uniform53(w[0], w[1]), u2 = uniform53(w[2], w[3]);
-    double rho = sqrt(-2.0 * orc_log(u1));
-    double z1 = rho * orc_sin2pi(u2 + 0.25);                    /* cos(2 pi u2) */
+    double z1 = pair_normal(d->seed, pixel, 0u);
     double n;
     if (!(mu > 0.0)) n = 0.0;
     else if (mu < 64.0) {
-        pixel_block(d->seed, pixel, 1u, w);
-        double v = uniform53(w[0], w[1]);
+        uint32_t w[4];
+        pair_block(d->seed, pixel >> 1, 1u, w);
+        double v = (pixel & 1u) ? uniform53(w[2], w[3]) : uniform53(w[0], w[1]);
         double p = orc_exp(-mu), F = p;
         n = 0.0;
         while (v > F && n < 255.0) {
@@ -174,7 +187,7 @@ void orc_detector_draws(const orc_detector_t *d, uint64_t pixel, double mu, doub
             F = F + p;
         }
     } else {
-        double z2 = rho * orc_sin2pi(u2);
+        double z2 = pair_normal(d->seed, pixel, 2u);
         double a = sqrt(mu) * z2;
         double b = (z2 * z2 - 1.0) * (1.0 / 6.0);
         n = floor(((mu + a) + b) + 0.5);
@@ -183,15 +196,11 @@ void orc_detector_draws(const orc_detector_t *d, uint64_t pixel, double mu, doub
     *z1_out = z1; *n_out = n;
 }
 
-/* the gaussian pair alone (pins: moments, independence) */
-void orc_gaussian_pair(uint64_t seed, uint64_t pixel, double *z1, double *z2)
+/* the read-noise normals of the two pixels of pair `pair` (pins: moments, independence) */
+void orc_gaussian_pair(uint64_t seed, uint64_t pair, double *z1, double *z2)
 {
-    uint32_t w[4];
-    pixel_block(seed, pixel, 0u, w);
-    double u1 = uniform53(w[0], w[1]), u2 = uniform53(w[2], w[3]);
-    double rho = sqrt(-2.0 * orc_log(u1));
-    *z1 = rho * orc_sin2pi(u2 + 0.25);
-    *z2 = rho * orc_sin2pi(u2);
+    *z1 = pair_normal(seed, 2 * pair, 0u);
+    *z2 = pair_normal(seed, 2 * pair + 1, 0u);
 }
 
 /* a6 over n pixels; pixel p of this call has global index pixel_offset + p (so results do not depend on

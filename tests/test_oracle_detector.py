@@ -56,33 +56,63 @@ def _uniform53(hi, lo):
 
 
 def test_draws_follow_the_stated_word_order():
-    """which Philox words feed which quantity (G12 round 2), checked with libm in place of the self-specified functions:
-    block 0 -> u1 = U(w0, w1), u2 = U(w2, w3), z1 = sqrt(-2 ln u1) cos(2 pi u2); block 1 -> v = U(w0, w1) for the Poisson
-    inversion (scipy's Poisson ppf of the same v); mu >= 64 -> z2 = sqrt(-2 ln u1) sin(2 pi u2) in the Cornish-Fisher formula"""
+    """which Philox words feed which pixel (G12 rounds 2 + 3), checked with libm in place of the self-specified functions.
+    Pixel p = pair q = p >> 1, parity s = p & 1; counter = (q, block).  Block 0 -> u1 = U(w0, w1), u2 = U(w2, w3),
+    z1 = sqrt(-2 ln u1) cos(2 pi u2) for s = 0, sin for s = 1; block 1 -> v = U(w0, w1) (s = 0) or U(w2, w3) (s = 1) for the
+    Poisson inversion (scipy's Poisson ppf of the same v); mu >= 64 -> z2 from block 2, formed like z1, in the Cornish-Fisher
+    formula"""
     from scipy.stats import poisson
     seed = 0x0123_4567_89AB_CDEF
     key = (seed & 0xffffffff, seed >> 32)
-    for pixel, mu in [(0, 0.0), (1, 3.3), (77, 20.5), (2 ** 33 + 5, 63.5), (123456789, 64.0), (31337, 4.1e4), (5, 0.01)]:
-        ctr = (pixel & 0xffffffff, pixel >> 32)
-        w = oracle.philox4x32_10(ctr + (0, 0), key)
+
+    def normal(q, s, block):
+        w = oracle.philox4x32_10((q & 0xffffffff, q >> 32, block, 0), key)
         u1, u2 = _uniform53(w[0], w[1]), _uniform53(w[2], w[3])
         rho = math.sqrt(-2.0 * math.log(u1))
+        return rho * (math.sin(2 * math.pi * u2) if s else math.cos(2 * math.pi * u2))
+
+    for pixel, mu in [(0, 0.0), (1, 3.3), (77, 20.5), (76, 20.5), (2 ** 33 + 5, 63.5), (2 ** 33 + 4, 63.5), (123456789, 64.0),
+                      (123456788, 64.0), (31337, 4.1e4), (5, 0.01), (4, 0.01)]:
+        q, par = pixel >> 1, pixel & 1
         det = Detector(gain=1.0, dark_e=0.0, ron_e=1.0, bias=0.0, seed=seed)
         z1 = float(oracle.detector(np.array([0.0]), det, pixel_offset=pixel)[0])        # mu = 0: out = ron z1
         cnt = float(oracle.detector(np.array([mu]), Detector(gain=1.0, ron_e=0.0, seed=seed), pixel_offset=pixel)[0])
-        assert z1 == pytest.approx(rho * math.cos(2 * math.pi * u2), abs=1e-14)
+        assert z1 == pytest.approx(normal(q, par, 0), abs=1e-14)
         assert float(oracle.detector(np.array([mu]), det, pixel_offset=pixel)[0]) == cnt + z1
         if mu == 0.0:
             assert cnt == 0.0
         elif mu < 64.0:
-            w1 = oracle.philox4x32_10(ctr + (1, 0), key)
-            assert cnt == poisson.ppf(_uniform53(w1[0], w1[1]), mu)
+            w1 = oracle.philox4x32_10((q & 0xffffffff, q >> 32, 1, 0), key)
+            v = _uniform53(w1[2], w1[3]) if par else _uniform53(w1[0], w1[1])
+            assert cnt == poisson.ppf(v, mu)
         else:
-            z2 = rho * math.sin(2 * math.pi * u2)
+            z2 = normal(q, par, 2)
             assert cnt == max(0.0, math.floor(mu + math.sqrt(mu) * z2 + (z2 * z2 - 1.0) / 6.0 + 0.5))
 
 
+@pytest.mark.parametrize("mu", [0.4, 12.0, 64.0, 900.0])
+def test_the_two_pixels_of_a_pair_are_independent(mu):
+    """G12 round 3: the pixels 2q and 2q + 1 share their Philox blocks; each block yields two independent variates, so their
+    counts, their read-noise normals and count x partner's read noise must be uncorrelated (4-sigma), in both Poisson
+    branches, and each parity alone must have the Poisson mean and variance"""
+    n = 400_000
+    cnt = oracle.detector(np.full(n, mu), Detector(ron_e=0.0, seed=99))
+    z = oracle.detector(np.zeros(n), Detector(ron_e=1.0, seed=99))
+    ce, co, ze, zo = cnt[0::2], cnt[1::2], z[0::2], z[1::2]
+    se = 4.0 / math.sqrt(n / 2)
+    assert abs(np.corrcoef(ce, co)[0, 1]) < se
+    assert abs(np.corrcoef(ze, zo)[0, 1]) < se
+    assert abs(np.corrcoef(ce, zo)[0, 1]) < se and abs(np.corrcoef(co, ze)[0, 1]) < se
+    assert abs(np.corrcoef(ce, ze)[0, 1]) < se and abs(np.corrcoef(co, zo)[0, 1]) < se
+    assert abs(np.corrcoef((ce - mu) ** 2, (co - mu) ** 2)[0, 1]) < se                # not just uncorrelated
+    var = mu + (5.0 / 36.0 if mu >= 64.0 else 0.0)
+    for c in (ce, co):
+        assert abs(c.mean() - mu) < 4.0 * math.sqrt(var / (n / 2))
+        assert abs(c.var() - var) < 4.0 * var * math.sqrt((2.0 + 1.0 / mu) / (n / 2))
+
+
 def test_box_muller_pair_is_standard_normal_and_independent():
+    # (z1, z2) = the read-noise normals of the two pixels of a pair (the cos and the sin half of one Box-Muller pair)
     n = 200_000
     z1, z2 = oracle.gaussian_pairs(424242, n)
     se = 1.0 / math.sqrt(n)
@@ -148,8 +178,10 @@ def test_independent_of_call_split_and_seed_dependent():
     frame = rng.uniform(0.0, 200.0, 5000)
     det = Detector(gain=1.3, dark_e=0.2, ron_e=3.0, bias=10.0, seed=5005)
     whole = oracle.detector(frame, det)
-    parts = np.concatenate([oracle.detector(frame[:1234], det, 0), oracle.detector(frame[1234:], det, 1234)])
-    assert np.array_equal(whole, parts)
+    for cut in (1234, 1235, 1):                                   # an odd cut puts the two pixels of a pair into different calls
+        parts = np.concatenate([oracle.detector(frame[:cut], det, 0), oracle.detector(frame[cut:], det, cut)])
+        assert np.array_equal(whole, parts)
+    assert np.array_equal(oracle.detector(frame, det, 777)[1:], oracle.detector(frame[1:], det, 778))
     assert not np.array_equal(whole, oracle.detector(frame, Detector(gain=1.3, dark_e=0.2, ron_e=3.0, bias=10.0, seed=5006)))
     # negative flux is clamped: mu = 0 -> pure read noise around the bias
     neg = oracle.detector(np.full(20000, -5.0), Detector(ron_e=2.0, bias=0.0, seed=1))

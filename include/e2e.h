@@ -286,10 +286,12 @@ E2E_API int e2e_render_frame_host_adu16(const e2e_format_t* fmt, const e2e_psf_t
  * Detector stage (a6; "photon noise and all other specific detector noises ... are added on the
  * final synthetic echellogram").  out[p] = (n + bias) + ron_e * z1 with mu = max(0, gain*in[p] + dark_e),
  * n ~ Poisson(mu), z1 ~ N(0,1), drawn from a Philox4x32-10 stream keyed by (seed, pixel index p = j*nx + i): the
- * result does not depend on launch geometry and is reproducible bit for bit.  Algorithm (G12, round 2):
- * block 0 of the pixel's stream gives a Box-Muller pair (z1, z2); mu < 64: n by inversion (sequential search) with one
- * uniform of block 1 -- an exact Poisson draw up to the 53-bit uniform, capped at n = 255 (probability < 1e-70);
- * mu >= 64: n = max(0, floor(mu + sqrt(mu) z2 + (z2^2 - 1)/6 + 1/2)), the normal approximation with the first
+ * result does not depend on launch geometry and is reproducible bit for bit.  Algorithm (G12, rounds 2 + 3):
+ * the pixels 2q and 2q + 1 share the stream of pair q = p >> 1, and every block serves both with independent variates:
+ * block 0 gives one Box-Muller pair, its cos half is z1 of the even pixel and its sin half z1 of the odd one; mu < 64:
+ * n by inversion (sequential search) with the pixel's own uniform of block 1 (words 0-1 even, 2-3 odd) -- an exact Poisson
+ * draw up to the 53-bit uniform, capped at n = 255 (probability < 1e-70); mu >= 64: with z2 from block 2 (formed like z1),
+ * n = max(0, floor(mu + sqrt(mu) z2 + (z2^2 - 1)/6 + 1/2)), the normal approximation with the first
  * Cornish-Fisher term -- NOT an exact Poisson draw: mean mu, skewness 1/sqrt(mu) as Poisson, variance mu + 5/36
  * (0.2 % high at mu = 64, 3e-6 at 4e4 e-), and the law changes at mu = 64.
  * ------------------------------------------------------------------------------------------------ */

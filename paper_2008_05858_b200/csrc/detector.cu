@@ -2,11 +2,11 @@
 //
 // P:79 "photon noise and all other specific detector noises (e.g. dark current, RON, pixels non-uniform response and
 // cross-talk) are added on the final synthetic echellogram".  The paper names the noises only; the algorithm is reading
-// G12 of DESIGN.md as re-specified in round 2 (a FIXED number of Philox blocks per pixel: one for the Box-Muller pair,
-// at most one more for the Poisson count; no rejection loop), G19 (PRNU / dark maps, full well, ADC) and G20 (cross-talk
+// G12 of DESIGN.md as re-specified in rounds 2 and 3 (a FIXED number of Philox blocks, shared by the two pixels of a pair: one for
+// the Box-Muller pair, at most one more for the Poisson counts; no rejection loop), G19 (PRNU / dark maps, full well, ADC) and G20 (cross-talk
 // between read-out ports).  Everything is made of IEEE-exact operations (+ - * / sqrt fma, integer ops; log, exp and
 // sin 2 pi y are spelled out below) and this file is compiled with --fmad=false, so the result is reproducible bit for bit
-// and independent of the launch geometry: pixel p owns the Philox4x32-10 stream (key = seed, counter = (p, block)).
+// and independent of the launch geometry: pixel pair q = p >> 1 owns the Philox4x32-10 stream (key = seed, counter = (q, block)).
 #include "common.cuh"
 
 #include <algorithm>
@@ -142,54 +142,76 @@ __device__ __forceinline__ double sin2pi(double y)
     return y * P;
 }
 
-// the draws of NP pixels (G12 round 2): z1 for the read noise, cnt = Poisson(mu).  The straight-line part (Philox block 0,
-// Box-Muller) runs for the NP pixels side by side so that their dependent fp64 chains overlap; the Poisson part branches.
-template <int NP>
-__device__ __forceinline__ void detector_draws(const DetTables& T, const PhiloxKeys& rk, const unsigned long long (&p)[NP],
-                                               const double (&mu)[NP], double (&z1_out)[NP], double (&cnt_out)[NP])
+// the draws of the two pixels 2q, 2q + 1 of pair q (G12 rounds 2 + 3): z1 for the read noise, cnt = Poisson(mu).  The pixels of a
+// pair share the Philox blocks of the pair's stream (counter = (q, block)): block 0 -> one Box-Muller pair, its cos half for
+// pixel 2q and its sin half for pixel 2q + 1; block 1 -> the two uniforms of the Poisson inversions; block 2 -> the normals of
+// the Cornish-Fisher branch.  want: bit i set = pixel i is asked for (the other one must come with mu = 0).
+__device__ __forceinline__ void pair_draws(const DetTables& T, const PhiloxKeys& rk, unsigned long long q, const double (&mu)[2],
+                                           unsigned want, double (&z1_out)[2], double (&cnt_out)[2])
 {
-    double u2[NP], rho[NP];
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-        uint32_t w0, w1, w2, w3;
-        philox_block(rk, (uint32_t)p[i], (uint32_t)(p[i] >> 32), 0u, w0, w1, w2, w3);
-        const double u1 = uniform53(w0, w1);
-        u2[i] = uniform53(w2, w3);
-        rho[i] = sqrt(-2.0 * table_log(T, u1));
+    uint32_t w0, w1, w2, w3;
+    philox_block(rk, (uint32_t)q, (uint32_t)(q >> 32), 0u, w0, w1, w2, w3);
+    {
+        const double u1 = uniform53(w0, w1), u2 = uniform53(w2, w3);
+        const double rho = sqrt(-2.0 * table_log(T, u1));
+        z1_out[0] = (want & 1u) ? rho * sin2pi(u2 + 0.25) : 0.0;      // cos(2 pi u2)
+        z1_out[1] = (want & 2u) ? rho * sin2pi(u2) : 0.0;
+    }
+    const bool lit0 = mu[0] > 0.0, lit1 = mu[1] > 0.0;
+    const bool small = (lit0 && mu[0] < 64.0) || (lit1 && mu[1] < 64.0);
+    const bool large = (lit0 && !(mu[0] < 64.0)) || (lit1 && !(mu[1] < 64.0));
+    double v[2] = {0.0, 0.0}, z2[2] = {0.0, 0.0};
+    if (small) {                                          // inversion by sequential search, one uniform per pixel
+        philox_block(rk, (uint32_t)q, (uint32_t)(q >> 32), 1u, w0, w1, w2, w3);
+        v[0] = uniform53(w0, w1);
+        v[1] = uniform53(w2, w3);
+    }
+    if (large) {                                          // normal + first Cornish-Fisher term
+        philox_block(rk, (uint32_t)q, (uint32_t)(q >> 32), 2u, w0, w1, w2, w3);
+        const double u1 = uniform53(w0, w1), u2 = uniform53(w2, w3);
+        const double rho = sqrt(-2.0 * table_log(T, u1));
+        z2[0] = rho * sin2pi(u2 + 0.25);
+        z2[1] = rho * sin2pi(u2);
     }
 #pragma unroll
-    for (int i = 0; i < NP; ++i) z1_out[i] = rho[i] * sin2pi(u2[i] + 0.25);      // cos(2 pi u2)
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
+    for (int i = 0; i < 2; ++i) {
         double cnt;
         if (!(mu[i] > 0.0)) {
             cnt = 0.0;
-        } else if (mu[i] < 64.0) {                        // inversion by sequential search, one uniform of block 1
-            uint32_t w0, w1, w2, w3;
-            philox_block(rk, (uint32_t)p[i], (uint32_t)(p[i] >> 32), 1u, w0, w1, w2, w3);
-            const double v = uniform53(w0, w1);
+        } else if (mu[i] < 64.0) {
             int n = 0;
             // Exact shortcut for the PSF wings (mu << 1, about half of an echellogram's illuminated pixels): the search
             // returns n = 0 iff v <= F0 = spec_exp(-mu), and F0 >= (1 - mu)(1 - 6e-16) (e^-mu >= 1 - mu; spec_exp is within
             // 5e-16 relative of e^y, pinned by the oracle's tests), so v < (1 - mu) - 1e-15 implies v <= F0: same n, no exp.
-            if (!(mu[i] < 0.5 && v < (1.0 - mu[i]) - 1.0e-15)) {
+            if (!(mu[i] < 0.5 && v[i] < (1.0 - mu[i]) - 1.0e-15)) {
                 double pr = spec_exp(-mu[i]), F = pr;
-                while (v > F && n < 255) {
+                while (v[i] > F && n < 255) {
                     n += 1;
                     pr = (pr * mu[i]) * T.rcp[n];
                     F = F + pr;
                 }
             }
             cnt = (double)n;
-        } else {                                          // normal + first Cornish-Fisher term
-            const double z2 = rho[i] * sin2pi(u2[i]);
-            const double a = sqrt(mu[i]) * z2;
-            const double b = (z2 * z2 - 1.0) * (1.0 / 6.0);
+        } else {
+            const double a = sqrt(mu[i]) * z2[i];
+            const double b = (z2[i] * z2[i] - 1.0) * (1.0 / 6.0);
             cnt = floor(((mu[i] + a) + b) + 0.5);
             if (cnt < 0.0) cnt = 0.0;
         }
         cnt_out[i] = cnt;
     }
+}
+
+// one pixel alone (the cross-talk kernel walks the ports, not the pairs): the draws of its pair, its own half
+__device__ __forceinline__ void pixel_draws(const DetTables& T, const PhiloxKeys& rk, unsigned long long gp, double mu, double& z1,
+                                            double& cnt)
+{
+    const bool odd = (gp & 1ull) != 0;
+    const double mu2[2] = {odd ? 0.0 : mu, odd ? mu : 0.0};
+    double z[2], c[2];
+    pair_draws(T, rk, gp >> 1, mu2, odd ? 2u : 1u, z, c);
+    z1 = odd ? z[1] : z[0];
+    cnt = odd ? c[1] : c[0];
 }
 
 // parameters of one launch (by value)
@@ -222,44 +244,68 @@ __device__ __forceinline__ void store_out<uint16_t>(uint16_t* out, long long p, 
 // in / out point at pixel p0 of the frame (the host path applies the stage band by band); the stream is keyed by the
 // pixel's index in the whole frame, so the result does not depend on how the frame is split into launches.  in may
 // alias out (each pixel is read before it is written, by the same thread): no __restrict__ on the two.
-// GENERAL = false: the basic stage (no maps, no well, no ADC) without the tests for them; kDetPix pixels per thread and
-// iteration, 256 pixels apart (coalesced).
-constexpr int kDetPix = 2;
-template <typename OutT, bool GENERAL>
+// GENERAL = false: the basic stage (no maps, no well, no ADC) without the tests for them.  Thread <-> pixel pair (G12 round 3):
+// pair j of the launch = global pair (p0 >> 1) + j = local pixels 2 j - (p0 & 1) + {0, 1}; a launch that starts or ends inside
+// a pair computes that pair's draws for the one pixel it owns.  VEC: p0 is even and both pointers allow 16-byte (in, fp64 out)
+// and 4-byte (uint16 out) accesses: one load and one store per pair.
+template <typename OutT>
+struct OutPair;
+template <>
+struct OutPair<double> { typedef double2 type; static __device__ __forceinline__ double2 make(double a, double b) { return make_double2(a, b); } };
+template <>
+struct OutPair<uint16_t> {
+    typedef ushort2 type;
+    static __device__ __forceinline__ ushort2 make(double a, double b) { return make_ushort2((unsigned short)(unsigned)a, (unsigned short)(unsigned)b); }
+};
+
+template <typename OutT, bool GENERAL, bool VEC>
 __global__ void __launch_bounds__(256) detector_kernel(const double* in, OutT* out, long long n, long long p0, DetParams D)
 {
     __shared__ DetTables T;
     build_tables(T);
-    const long long stride = (long long)gridDim.x * (256 * kDetPix);
+    const long long stride = (long long)gridDim.x * 256;
     const bool use_adc = GENERAL && D.e_per_adu > 0.0;
-    for (long long base = (long long)blockIdx.x * (256 * kDetPix) + threadIdx.x; base < n; base += stride) {
-        unsigned long long gp[kDetPix];
-        double mu[kDetPix], z1[kDetPix], e[kDetPix];
+    const long long shift = p0 & 1;                              // local index of the first pair's even pixel is -shift
+    const long long npairs = (n + shift + 1) >> 1;
+    const unsigned long long q0 = (unsigned long long)p0 >> 1;
+    for (long long j = (long long)blockIdx.x * 256 + threadIdx.x; j < npairs; j += stride) {
+        const long long pl = 2 * j - shift;                      // local index of the pair's even pixel
+        const bool ok0 = pl >= 0, ok1 = pl + 1 < n;
+        double f[2];
+        if (VEC && ok1) {
+            const double2 v = *reinterpret_cast<const double2*>(in + pl);
+            f[0] = v.x; f[1] = v.y;
+        } else {
+            f[0] = ok0 ? in[pl] : 0.0;
+            f[1] = ok1 ? in[pl + 1] : 0.0;
+        }
+        double mu[2], z1[2], e[2];
 #pragma unroll
-        for (int i = 0; i < kDetPix; ++i) {
-            const long long p = base + 256 * i;
-            const bool ok = p < n;
-            gp[i] = (unsigned long long)(p0 + p);
+        for (int i = 0; i < 2; ++i) {
+            const bool ok = i ? ok1 : ok0;
             double g = D.base.gain, dk = D.base.dark_e;
             if (GENERAL) {
-                if (D.prnu && ok) g = g * __ldg(D.prnu + gp[i]);
-                if (D.dark && ok) dk = __ldg(D.dark + gp[i]);
+                const unsigned long long gp = (unsigned long long)(p0 + pl + i);
+                if (D.prnu && ok) g = g * __ldg(D.prnu + gp);
+                if (D.dark && ok) dk = __ldg(D.dark + gp);
             }
-            double m = g * (ok ? in[p] : 0.0) + dk;
-            if (!(m > 0.0)) m = 0.0;
+            double m = g * f[i] + dk;
+            if (!(m > 0.0) || !ok) m = 0.0;
             mu[i] = m;
         }
-        detector_draws<kDetPix>(T, D.rk, gp, mu, z1, e);
+        pair_draws(T, D.rk, q0 + (unsigned long long)j, mu, 3u, z1, e);
+        double r[2];
 #pragma unroll
-        for (int i = 0; i < kDetPix; ++i) {
-            const long long p = base + 256 * i;
-            if (p < n) {
-                double r;
-                if (GENERAL && D.full_well > 0.0 && e[i] > D.full_well) e[i] = D.full_well;
-                if (!use_adc) r = (e[i] + D.base.bias) + D.base.ron_e * z1[i];
-                else r = adc(D, e[i] + D.base.ron_e * z1[i]);
-                store_out<OutT>(out, p, r);
-            }
+        for (int i = 0; i < 2; ++i) {
+            if (GENERAL && D.full_well > 0.0 && e[i] > D.full_well) e[i] = D.full_well;
+            if (!use_adc) r[i] = (e[i] + D.base.bias) + D.base.ron_e * z1[i];
+            else r[i] = adc(D, e[i] + D.base.ron_e * z1[i]);
+        }
+        if (VEC && ok1) {
+            *reinterpret_cast<typename OutPair<OutT>::type*>(out + pl) = OutPair<OutT>::make(r[0], r[1]);
+        } else {
+            if (ok0) store_out<OutT>(out, pl, r[0]);
+            if (ok1) store_out<OutT>(out, pl + 1, r[1]);
         }
     }
 }
@@ -288,7 +334,7 @@ __global__ void __launch_bounds__(128) detector_xtalk_kernel(const double* in, O
                 double mu[1] = {g * in[p] + (D.dark ? __ldg(D.dark + gp[0]) : D.base.dark_e)};
                 if (!(mu[0] > 0.0)) mu[0] = 0.0;
                 double z1[1], e[1];
-                detector_draws<1>(T, D.rk, gp, mu, z1, e);
+                pixel_draws(T, D.rk, gp[0], mu[0], z1[0], e[0]);
                 if (D.full_well > 0.0 && e[0] > D.full_well) e[0] = D.full_well;
                 V[b][threadIdx.x] = e[0] + D.base.ron_e * z1[0];
             }
@@ -325,11 +371,14 @@ static int launch_detector_any(const double* d_in, OutT* d_out, long long n, int
         const long long blocks = std::min<long long>(rows * per_row, resident_ctas(128));
         detector_xtalk_kernel<OutT><<<(unsigned)blocks, 128, 0, stream>>>(d_in, d_out, rows, p0, D);
     } else {
-        const long long per = 256 * kDetPix;
-        const long long blocks = std::min<long long>((n + per - 1) / per, resident_ctas(256));
+        const long long per = 256 * 2;                               // one pixel pair per thread and iteration
+        const long long blocks = std::min<long long>((n + 1 + per - 1) / per, resident_ctas(256));
         const bool general = D.prnu || D.dark || D.full_well > 0.0 || D.e_per_adu > 0.0;
-        if (general) detector_kernel<OutT, true><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
-        else detector_kernel<OutT, false><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        const bool vec = (p0 & 1) == 0 && ((uintptr_t)d_in & 15) == 0 && ((uintptr_t)d_out & (2 * sizeof(OutT) - 1)) == 0;
+        if (general && vec) detector_kernel<OutT, true, true><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        else if (general) detector_kernel<OutT, true, false><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        else if (vec) detector_kernel<OutT, false, true><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
+        else detector_kernel<OutT, false, false><<<(unsigned)blocks, 256, 0, stream>>>(d_in, d_out, n, p0, D);
     }
     count_launch();
     cudaError_t e = cudaGetLastError();

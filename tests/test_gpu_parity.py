@@ -716,6 +716,43 @@ def test_detector_bit_exact(B):
     B.e2e_apply_detector(d_in, d_in, nx, ny, det)
     assert np.array_equal(d_in.cpu().numpy(), O)
     assert abs(G[-1].mean() / (0.9 * fr[-1].mean() + 0.4 + 100.0) - 1.0) < 0.01
+    # buffers that are only 8-byte aligned (the kernel's one-load-per-pixel-pair form does not apply), odd pixel count
+    src = torch.empty(nx * ny + 1, dtype=torch.float64, device="cuda")
+    dst = torch.full((nx * ny + 2,), -1.0, dtype=torch.float64, device="cuda")
+    src[1:] = torch.from_numpy(fr).cuda().reshape(-1)
+    B.e2e_apply_detector(src[1:], dst[1:-1], nx, ny, det)
+    assert np.array_equal(dst[1:-1].cpu().numpy().reshape(ny, nx), O)
+    assert dst[0].item() == -1.0 and dst[-1].item() == -1.0
+
+
+def test_detector_pairs_that_straddle_host_bands(B):
+    """G12 round 3 keys the noise stream by pixel PAIR; on a frame of odd width the row bands of the host path start at odd
+    pixel indices, so a pair's two pixels land in different launches.  Still bit-exact against the oracle's stage applied to
+    the host path's own noise-free frame, fp64 and uint16"""
+    import torch
+    s = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=[0, 1, 2, 40, 41, 83, 84])
+    s.nx = 9215
+    det = W.Detector(gain=1.0, dark_e=0.5, ron_e=3.0, bias=100.0, seed=31337)
+    r = B.Renderer(s)
+    try:
+        pc = B.e2e_plan_check(r.fmt, r.psf)
+        assert pc["n_host_bands"] >= 3
+        host_tabs = [np.ascontiguousarray(sp.flux, dtype=np.float64) for sp in s.spectra]
+        desc = B.spectra_array(s.spectra, [t.ctypes.data for t in host_tabs])
+        ws = torch.empty(B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc), dtype=torch.uint8, device="cuda")
+        clean = torch.empty((s.ny, s.nx), dtype=torch.float64).pin_memory()
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, clean.data_ptr(), ws)
+        H = clean.numpy().copy()
+        assert H.max() > 0
+        noisy = torch.empty_like(clean)
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, noisy.data_ptr(), ws, det=det)
+        assert np.array_equal(noisy.numpy(), oracle.detector(H, det))
+        d_ex, keep = B.detector_ex_desc(det, e_per_adu=1.1, adu_max=65535.0)
+        out16 = torch.zeros((s.ny, s.nx), dtype=torch.uint16).pin_memory()
+        B.e2e_render_frame_host_ex(r.fmt, r.psf, desc, out16.data_ptr(), ws, d_ex, adu16=True)
+        assert np.array_equal(out16.numpy(), oracle.detector_adu16(H, det, e_per_adu=1.1, adu_max=65535.0))
+    finally:
+        r.close()
 
 
 def test_detector_ex_bit_exact(B):

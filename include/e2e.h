@@ -240,9 +240,10 @@ E2E_API int e2e_render_frame_noalloc(const e2e_format_t* fmt, const e2e_psf_t* p
  * different simulation scenarios"): n_frames frames of the SAME format and PSF, each with its own spectra --
  * e.g. object / flat / Fabry-Perot exposures, or the Doppler-shifted copies of one spectrum (BJ "Precision/RV sweep").
  * spectra: HOST array [n_frames][n_fibers] (DEVICE tables); d_frames: HOST array of n_frames distinct DEVICE frame
- * pointers ([ny*nx] each).  Frame b equals e2e_render_frame(spectra + b * n_fibers, d_frames[b]) bit for bit; a1 and a3
- * (positions) are computed once, and one launch renders one phase of all the frames (grid.y = frame), so small frames
- * that cannot fill the GPU alone do so together.  Workspace: e2e_render_frames_workspace_bytes.  Errors as
+ * pointers ([ny*nx] each).  Frame b equals e2e_render_frame(spectra + b * n_fibers, d_frames[b]) bit for bit.  The frames
+ * are rendered by the same launches (two kernel launches for the whole batch on the two-kernel analytic path,
+ * one ticket queue per frame), so small frames that cannot fill the GPU alone do so together; the kernels that materialise
+ * the samples compute a1 and a3 (positions) once for the batch.  Workspace: e2e_render_frames_workspace_bytes.  Errors as
  * e2e_render_frame; n_frames outside 1..65535 or two equal frame pointers -> E2E_ERR_INVALID_ARG. */
 E2E_API int e2e_render_frames_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_frames, size_t* bytes);
 E2E_API int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_frames, const e2e_spectrum_t* spectra,

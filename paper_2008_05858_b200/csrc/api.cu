@@ -869,9 +869,9 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         static SpectraParam no_spectra;
         const unsigned blocks = (unsigned)((ni + kCellWarps - 1) / kCellWarps);
         switch (P->moment_npt) {
-            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
-            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
-            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0); break;
+            case 2: cell_moment_kernel<2, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0, nullptr); break;
+            case 3: cell_moment_kernel<3, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0, nullptr); break;
+            default: cell_moment_kernel<4, true, false><<<blocks, kCellWarps * 32>>>(nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, ni, P->mom, none, d_counts, F->view, no_spectra, nullptr, 0, nullptr); break;
         }
         count_launch();
         std::vector<int> counts(ni);
@@ -1075,6 +1075,8 @@ static CellStore cell_store(const e2e_plan* pl, unsigned* ctrl)
     cs.cell_off = pl->d_cell_off;
     cs.hdr = (CellHeader*)((char*)ctrl + align_up(sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)), 256));
     cs.mom = (double*)((char*)cs.hdr + cell_hdr_bytes(pl));
+    cs.frame_cells = 0;
+    cs.n_frames = 1;
     return cs;
 }
 
@@ -1094,7 +1096,7 @@ static int launch_cell_moments(const e2e_format* F, const e2e_psf* P, const e2e_
 #define E2E_CELL_CASE(NPT)                                                                                                     \
     case NPT:                                                                                                                   \
         cell_moment_kernel<NPT, false, true><<<blocks, kCellWarps * 32, sizeof(MomentWarpSmem<NPT, false>) * kCellWarps, stream>>>( \
-            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ids, n, P->mom, cs, nullptr, F->view, sp, zero, n_zero);      \
+            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, ids, n, P->mom, cs, nullptr, F->view, sp, zero, n_zero, nullptr); \
         break;
     switch (P->moment_npt) {
         E2E_CELL_CASE(2) E2E_CELL_CASE(3) E2E_CELL_CASE(4)
@@ -1120,9 +1122,9 @@ static int launch_cell_flush(const e2e_format* F, const e2e_psf* P, const e2e_pl
     if (pl->small) {
         // a frame that cannot fill the GPU: one CTA of kWideWarps warps per item, the cell's tiles spread over the warps
         switch (P->moment_npt) {
-            case 2: cell_flush_wide_kernel<2><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
-            case 3: cell_flush_wide_kernel<3><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
-            case 4: cell_flush_wide_kernel<4><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+            case 2: cell_flush_wide_kernel<2><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
+            case 3: cell_flush_wide_kernel<3><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
+            case 4: cell_flush_wide_kernel<4><<<(unsigned)n, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
             default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
         }
         count_launch();
@@ -1131,9 +1133,9 @@ static int launch_cell_flush(const e2e_format* F, const e2e_psf* P, const e2e_pl
         return E2E_OK;
     }
     switch (P->moment_npt) {
-        case 2: cell_flush_kernel<2><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
-        case 3: cell_flush_kernel<3><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
-        case 4: cell_flush_kernel<4><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny); break;
+        case 2: cell_flush_kernel<2><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
+        case 3: cell_flush_kernel<3><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
+        case 4: cell_flush_kernel<4><<<(unsigned)n, 32, 0, stream>>>(W, P->mom, cs, d_frame, F->view.nx, F->view.ny, nullptr); break;
         default: return fail(E2E_ERR_UNSUPPORTED, "render: no moment kernel for this polynomial degree");
     }
     count_launch();
@@ -1147,6 +1149,58 @@ static cudaError_t ctrl_reset(const e2e_plan* pl, unsigned* ctrl, cudaStream_t s
 {
     return cudaMemcpyAsync(ctrl, pl->d_ctrl_init, sizeof(unsigned) * ((size_t)kCtrlHeads + (size_t)std::max(pl->n_items, 1)),
                            cudaMemcpyDeviceToDevice, stream);
+}
+
+// ---- batch form of the two-kernel render (e2e_render_frames): 1-D grids, frame = blockIdx.x % n_frames.  Workspace after the frame-pointer array:
+//      SpectraParam[n_frames] | control blocks [n_frames] | cell headers [n_frames][n_cells] | moment tiles [n_frames][n_cells]
+struct BatchLayout {
+    size_t sp_off, ctrl_off, hdr_off, mom_off, bytes;
+};
+static BatchLayout batch_layout(const e2e_psf* P, const e2e_plan* pl, int n_frames, size_t ptr_bytes)
+{
+    BatchLayout L;
+    const size_t cells = (size_t)std::max<long long>(pl->n_cells, 1) * (size_t)n_frames;
+    L.sp_off = ptr_bytes;
+    L.ctrl_off = L.sp_off + align_up(sizeof(SpectraParam) * (size_t)n_frames, 256);
+    L.hdr_off = L.ctrl_off + ctrl_bytes(pl) * (size_t)n_frames;
+    L.mom_off = L.hdr_off + align_up(sizeof(CellHeader) * cells, 256);
+    L.bytes = L.mom_off + align_up(sizeof(double) * 64 * (size_t)P->moment_npt * cells, 256);
+    return L;
+}
+
+static int launch_cells_batch(const e2e_format* F, const e2e_psf* P, const e2e_plan* pl, int n_frames, const SpectraParam* d_sp,
+                              unsigned* d_ctrl, const CellStore& cs, double* const* d_frames, cudaStream_t stream)
+{
+    const int n = pl->n_items;
+    if (n <= 0) return E2E_OK;
+    SpectraParam none;
+    memset(&none, 0, sizeof(none));
+    const long long bm = (long long)((n + kCellWarps - 1) / kCellWarps) * n_frames, bf = (long long)n * n_frames;
+    if (bf > 0x7fffffffLL) return fail(E2E_ERR_UNSUPPORTED, "render_frames: more than 2^31 (item, frame) pairs");
+    const unsigned gm = (unsigned)bm;
+    QueueParam W;
+    memset(&W, 0, sizeof(W));
+    W.n = n; W.ctrl = d_ctrl; W.ctrl_stride = (long long)(ctrl_bytes(pl) / sizeof(unsigned));
+    W.succ_off = pl->d_succ_off; W.succ_idx = pl->d_succ_idx; W.dep_off = pl->d_dep_off; W.dep_idx = pl->d_dep_idx;
+    const unsigned gf = (unsigned)bf;
+    const bool wide = pl->small;
+#define E2E_BATCH_CASE(NPT)                                                                                                      \
+    case NPT:                                                                                                                    \
+        cell_moment_kernel<NPT, false, true, true><<<gm, kCellWarps * 32, sizeof(MomentWarpSmem<NPT, false>) * kCellWarps, stream>>>( \
+            nullptr, nullptr, nullptr, pl->d_strips, pl->d_items, nullptr, n, P->mom, cs, nullptr, F->view, none, nullptr, 0, d_sp); \
+        count_launch();                                                                                                          \
+        if (wide) cell_flush_wide_kernel<NPT, true><<<gf, kWideWarps * 32, 0, stream>>>(W, P->mom, cs, nullptr, F->view.nx, F->view.ny, d_frames); \
+        else cell_flush_kernel<NPT, true><<<gf, 32, 0, stream>>>(W, P->mom, cs, nullptr, F->view.nx, F->view.ny, d_frames);      \
+        count_launch();                                                                                                          \
+        break;
+    switch (P->moment_npt) {
+        E2E_BATCH_CASE(2) E2E_BATCH_CASE(3) E2E_BATCH_CASE(4)
+        default: return fail(E2E_ERR_UNSUPPORTED, "render_frames: no moment kernel for this polynomial degree");
+    }
+#undef E2E_BATCH_CASE
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "render_frames: cell kernel launch");
+    return E2E_OK;
 }
 
 // one queue of a persistent launch: the whole plan (queue = nullptr) or one row band of the host path
@@ -1468,8 +1522,9 @@ int e2e_render_frames_workspace_bytes(const e2e_format_t* fmt, const e2e_psf_t* 
     e2e_plan* pl = nullptr;
     rc = build_plan(const_cast<e2e_format*>(fmt), psf, &pl);
     if (rc) return rc;
-    *bytes = sample_array_bytes(pl->total_samples) * (2 + (size_t)n_frames) + align_up(sizeof(double*) * (size_t)n_frames, 256) +
-             ctrl_bytes(pl) * (size_t)n_frames;
+    const size_t ptr_bytes = align_up(sizeof(double*) * (size_t)n_frames, 256);
+    if (use_split(fmt, psf, pl)) *bytes = batch_layout(psf, pl, n_frames, ptr_bytes).bytes;   // no per-sample arrays on this path
+    else *bytes = sample_array_bytes(pl->total_samples) * (2 + (size_t)n_frames) + ptr_bytes + ctrl_bytes(pl) * (size_t)n_frames;
     return E2E_OK;
 }
 
@@ -1493,10 +1548,44 @@ int e2e_render_frames(const e2e_format_t* fmt, const e2e_psf_t* psf, int32_t n_f
     if (rc) return rc;
     const size_t per = sample_array_bytes(pl->total_samples);
     const size_t ptr_bytes = align_up(sizeof(double*) * (size_t)n_frames, 256);
-    const size_t need = per * (2 + (size_t)n_frames) + ptr_bytes + ctrl_bytes(pl) * (size_t)n_frames;
+    const bool split = use_split(fmt, psf, pl);
+    const BatchLayout BL = split ? batch_layout(psf, pl, n_frames, ptr_bytes) : BatchLayout{};
+    const size_t need = split ? BL.bytes : per * (2 + (size_t)n_frames) + ptr_bytes + ctrl_bytes(pl) * (size_t)n_frames;
     if (!d_workspace || ((uintptr_t)d_workspace & 255) != 0) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace NULL or not 256-byte aligned");
     if (workspace_bytes < need) return fail(E2E_ERR_WORKSPACE, "render_frames: workspace too small");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
+    if (split) {
+        // two-kernel form, the frames interleaved in one grid: the moments of every frame's cells (each frame's own spectra; a1 and a3 are recomputed
+        // per frame inside the kernel, a few instructions next to a2), then ONE flush launch with one ticket queue per frame
+        char* base = (char*)d_workspace;
+        double** d_ptrs = (double**)base;
+        SpectraParam* d_sp = (SpectraParam*)(base + BL.sp_off);
+        unsigned* d_ctrl = (unsigned*)(base + BL.ctrl_off);
+        CellStore cs;
+        cs.cell_off = pl->d_cell_off;
+        cs.hdr = (CellHeader*)(base + BL.hdr_off);
+        cs.mom = (double*)(base + BL.mom_off);
+        cs.frame_cells = std::max<long long>(pl->n_cells, 1);
+        cs.n_frames = n_frames;
+        std::vector<SpectraParam> sp((size_t)n_frames);
+        memset(sp.data(), 0, sizeof(SpectraParam) * sp.size());
+        for (int b = 0; b < n_frames; ++b)
+            for (int f = 0; f < nf; ++f) sp[(size_t)b].s[f] = spectra[(size_t)b * nf + f];
+        // pageable sources: both copies are staged before cudaMemcpyAsync returns, so neither array needs to outlive the call
+        E2E_CUDA(cudaMemcpyAsync(d_ptrs, d_frames, sizeof(double*) * (size_t)n_frames, cudaMemcpyHostToDevice, stream));
+        E2E_CUDA(cudaMemcpyAsync(d_sp, sp.data(), sizeof(SpectraParam) * sp.size(), cudaMemcpyHostToDevice, stream));
+        for (int b = 0; b < n_frames; ++b) E2E_CUDA(ctrl_reset(pl, (unsigned*)((char*)d_ctrl + ctrl_bytes(pl) * (size_t)b), stream));
+        if (!accumulate) {
+            StageTimer tm(kStageZero, stream);
+            for (int b = 0; b < n_frames; ++b)
+                E2E_CUDA(cudaMemsetAsync(d_frames[b], 0, (size_t)fmt->view.nx * fmt->view.ny * 8, stream));
+        }
+        StageTimer tm(kStageRender, stream);
+        const long long before = g_launches.load();
+        rc = launch_cells_batch(fmt, psf, pl, n_frames, d_sp, d_ctrl, cs, d_ptrs, stream);
+        if (tm.on) { std::lock_guard<std::mutex> lk(g_prof_mu); g_prof_tot.n_render += g_launches.load() - before; g_prof_tot.n_calls += 1; }
+        return rc;
+    }
     double* d_x = (double*)d_workspace;
     double* d_y = (double*)((char*)d_workspace + per);
     double* d_w = (double*)((char*)d_workspace + 2 * per);

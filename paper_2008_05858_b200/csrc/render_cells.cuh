@@ -14,7 +14,8 @@
 //                       render_moment.cuh: DMMAs, table loads and the frame reductions only -- no scalar fp64 at all.
 //
 // The cell walk (where a cell ends) and the arithmetic are those of render_moment_kernel, operation for operation, so the frame
-// has the same bits; tests compare the two paths with torch.equal (the batch call still runs the one-kernel path).
+// has the same bits as the one-kernel form's (which still renders analytic PSF maps).  The batch call (e2e_render_frames) runs
+// these kernels with the frames interleaved in one grid (BATCH).
 #pragma once
 #include "common.cuh"
 #include "render_moment.cuh"
@@ -34,17 +35,23 @@ struct CellStore {
     const long long* cell_off;         // [n_items + 1] first cell of every item (from the counting pass of the plan)
     CellHeader* hdr;                   // [n_cells]
     double* mom;                       // [n_cells][32 lanes][2 NPT]
+    long long frame_cells;             // batch render: the records of frame b start at cell b * frame_cells of both arrays
+    int n_frames;                      // batch render: 1-D grid, frame = blockIdx.x % n_frames (the frames advance together: a
+                                       // grid.y per frame would run them one after the other, each at its own serial chain)
 };
 
 // FUSED: steps a1-a3 run here (setup.cuh's device functions: the oracle's operation sequence, the same bits as
 // setup_samples_kernel) and the samples are never materialised; else they are read from the arrays setup_samples_kernel wrote
 // NPT = 2: 8 CTAs per SM (64 registers; the shared-memory staging allows 8), measured 1.41 against 1.43 ms at 7 CTAs
-template <int NPT, bool COUNT, bool FUSED>
+// BATCH (e2e_render_frames): frame = blockIdx.x % n_frames; same geometry, the frame's own spectra (sp_batch[frame], device
+// memory) and record region
+template <int NPT, bool COUNT, bool FUSED, bool BATCH = false>
 __global__ void __launch_bounds__(kCellWarps * 32, NPT == 2 ? 8 : 0)
 cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ ws,
                    const Strip* __restrict__ strips, const Item* __restrict__ items, const int* __restrict__ ids, int n_items,
                    MomentParam Q, CellStore C, int* __restrict__ counts, const __grid_constant__ FormatView F,
-                   const __grid_constant__ SpectraParam SP, double2* __restrict__ zero, long long n_zero)
+                   const __grid_constant__ SpectraParam SP, double2* __restrict__ zero, long long n_zero,
+                   const SpectraParam* __restrict__ sp_batch)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -53,7 +60,8 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
     if (!COUNT && zero)
         for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_zero; i += (long long)gridDim.x * blockDim.x)
             __stcs(zero + i, make_double2(0.0, 0.0));
-    const int slot = blockIdx.x * kCellWarps + warp;
+    const int bframe = BATCH ? (int)(blockIdx.x % (unsigned)C.n_frames) : 0;
+    const int slot = (BATCH ? (int)(blockIdx.x / (unsigned)C.n_frames) : (int)blockIdx.x) * kCellWarps + warp;
     if (slot >= n_items) return;
     const int item_id = ids ? ids[slot] : slot;              // ids: the items of one row band (host path), else all of them
     MomentWarpSmem<NPT, false>& S = reinterpret_cast<MomentWarpSmem<NPT, false>*>(smem_raw)[warp];
@@ -70,7 +78,7 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
     bool have = false;
     int cI0 = 0, cI1 = 0, cJ0 = 0, cJ1 = 0, cYb = 0;
     double cYc = 0.0;
-    long long cell = COUNT ? 0 : C.cell_off[item_id];
+    long long cell = COUNT ? 0 : C.cell_off[item_id] + (BATCH ? (long long)bframe * C.frame_cells : 0);
     int n_cells = 0;
 
     // the open cell is complete: hand it to the flush kernel
@@ -101,7 +109,7 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
             xk = __dadd_rn(X, F.fiber_dx[fiber]);
             yk = __dadd_rn(Y, F.fiber_dy[fiber]);
             if (FUSED && !COUNT) {                              // a2: the photon weight, setup_samples_kernel's expression
-                const e2e_spectrum_t& sf = SP.s[fiber];
+                const e2e_spectrum_t& sf = BATCH ? sp_batch[bframe].s[fiber] : SP.s[fiber];
                 const double wv = __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(sf.scale, spectrum_at(sf, lam)), blaze_at(F, o, lam)),
                                                       eff_at(F, lam)), F.dl[o]);
                 wk = valid ? wv : 0.0;
@@ -190,14 +198,23 @@ cell_moment_kernel(const double* __restrict__ xs, const double* __restrict__ ys,
 }
 
 // steps 2 + 3 + a5 for the cells of one item, in order, under the ticket queue (render_moment.cuh queue_take / queue_done)
-template <int NPT>
+// BATCH (e2e_render_frames): frame = blockIdx.x % n_frames, with its own target, control block and record region
+template <int NPT, bool BATCH = false>
 __global__ void __launch_bounds__(32, NPT == 2 ? E2E_MOM_MINB : 1)
-cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny)
+cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny, double* const* __restrict__ frames)
 {
     const int lane = threadIdx.x & 31;
-    const int item_id = queue_take(W, W.ctrl, lane);
+    unsigned* ctrl = W.ctrl;
+    long long cbase = 0;
+    if (BATCH) {
+        const unsigned b = blockIdx.x % (unsigned)C.n_frames;
+        frame = frames[b];
+        ctrl += (long long)b * W.ctrl_stride;
+        cbase = (long long)b * C.frame_cells;
+    }
+    const int item_id = queue_take(W, ctrl, lane);
     if (item_id < 0) return;
-    const long long c0 = C.cell_off[item_id], c1 = C.cell_off[item_id + 1];
+    const long long c0 = C.cell_off[item_id] + cbase, c1 = C.cell_off[item_id + 1] + cbase;
     for (long long cell = c0; cell < c1; ++cell) {
         const CellHeader h = C.hdr[cell];
         double mt[1][NPT][2];
@@ -209,7 +226,7 @@ cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__
         }
         moment_flush_cell<NPT, false>(Q, mt, h.i0, h.i1, h.j0, h.j1, h.yb, 0, 0, frame, nx, ny, lane);
     }
-    queue_done(W, W.ctrl, item_id, lane);
+    queue_done(W, ctrl, item_id, lane);
 }
 
 // ---- small frames (a single strip, a few hundred items): the launch cannot fill the GPU, the frame time is the serial chain of
@@ -220,21 +237,30 @@ cell_flush_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__
 // then y; Y_t by power tile, x then y): the frame has the same bits.  Consecutive cells of the item overlap, and their tiles
 // belong to different warps, so a CTA barrier (instead of __syncwarp) orders one cell's reductions before the next cell's.
 constexpr int kWideWarps = 9;
-template <int NPT>
+template <int NPT, bool BATCH = false>
 __global__ void __launch_bounds__(kWideWarps * 32)
-cell_flush_wide_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny)
+cell_flush_wide_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restrict__ frame, int nx, int ny,
+                       double* const* __restrict__ frames)
 {
     __shared__ int s_item;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int lq = lane >> 2, lr = lane & 3;
+    unsigned* ctrl = W.ctrl;
+    long long cbase = 0;
+    if (BATCH) {                                               // e2e_render_frames
+        const unsigned b = blockIdx.x % (unsigned)C.n_frames;
+        frame = frames[b];
+        ctrl += (long long)b * W.ctrl_stride;
+        cbase = (long long)b * C.frame_cells;
+    }
     if (warp == 0) {
-        const int id = queue_ticket(W, W.ctrl, lane);
+        const int id = queue_ticket(W, ctrl, lane);
         if (lane == 0) s_item = id;
     }
     __syncthreads();
     const int item_id = s_item;
     if (item_id < 0) return;
-    const long long c0 = C.cell_off[item_id], c1 = C.cell_off[item_id + 1];
+    const long long c0 = C.cell_off[item_id] + cbase, c1 = C.cell_off[item_id + 1] + cbase;
     // the first record travels while warp 0 waits for the item's dependencies (records are final before this launch)
     CellHeader hn = {};
     double2 mn[NPT] = {};
@@ -245,7 +271,7 @@ cell_flush_wide_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restr
         for (int qt = 0; qt < NPT; ++qt) mn[qt] = __ldg(reinterpret_cast<const double2*>(src + 2 * qt));
     };
     if (c0 < c1) fetch(c0);
-    if (warp == 0) queue_wait(W.ctrl, item_id);
+    if (warp == 0) queue_wait(ctrl, item_id);
     __syncthreads();
     const int ntile = Q.nit * Q.njt;
     for (long long cell = c0; cell < c1; ++cell) {
@@ -289,7 +315,7 @@ cell_flush_wide_kernel(QueueParam W, MomentParam Q, CellStore C, double* __restr
     __threadfence();
     __syncthreads();
     if (warp == 0) {
-        unsigned* const pend = W.ctrl + kCtrlHeads;
+        unsigned* const pend = ctrl + kCtrlHeads;
         const int s1 = W.succ_off[item_id + 1];
         for (int d = W.succ_off[item_id] + lane; d < s1; d += 32) red_release_dec_u32(pend + W.succ_idx[d]);
     }

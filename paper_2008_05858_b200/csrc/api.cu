@@ -757,7 +757,6 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
 #endif
     const int K = items_k2 < kSmallFrameItems ? ((P->kind == 0 && P->moment_npt > 0) ? E2E_SMALL_K : 4) : 2;
     pl->small = K > 2;
-    const bool cell_moment_path = P->kind == 0 && P->moment_npt > 0 && !P->is_map;
     std::vector<std::vector<Item>> phases((size_t)n_colors * K);
     for (int s = 0; s < n_strips; ++s) {
         const int o = s % no;
@@ -766,12 +765,9 @@ static int build_plan(e2e_format* F, const e2e_psf* P, e2e_plan** out)
         const long long nchunks = (N + 31) / 32;
         long long G = run_length(o, nchunks);
         if (K > 2 && G < nchunks) G = (G + K - 2) / (K - 1);
-#ifndef E2E_RUN_SCALE
-#define E2E_RUN_SCALE 2.0
-#endif
-        // frames that fill the GPU: runs twice the minimum length (the per-item cost -- ticket, dependency wait, fence, release --
-        // halves; 56 780 -> 28 400 items on the ESPRESSO-like frame measured 4.39 against 4.48 ms; 1.5x 4.43, 3x 4.49)
-        if (K == 2 && cell_moment_path) G = std::min<long long>(nchunks, (long long)((double)G * E2E_RUN_SCALE));
+        // runs are kept at the minimum length: twice as long measured 4.39 against 4.48 ms for the device-resident flush launch
+        // (fewer cells cut at item ends), but the host path's per-band launches then have too few items to fill the GPU
+        // (e2e 15.3 against 13.9 ms fp64, 9.9 against 8.1 ms uint16)
         int run = 0;
         for (long long c0 = 0; c0 < nchunks; c0 += G, ++run)
             phases[(size_t)color[s] * K + (run % K)].push_back(Item{s, (int)c0, (int)std::min(G, nchunks - c0)});

@@ -529,6 +529,16 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             o["r"].close()
             del o
             torch.cuda.empty_cache()
+        # BASELINE.json configs[4] as a whole: the 5 Doppler-shifted RV-sweep frames in ONE e2e_render_frames call per step
+        o = measure_device(B, W, torch, "rv_sweep", max(3, min(args.steps, 5)), 3, 0, 1, dev, 5)
+        others["rv_sweep_batch5"] = {"workload": o["wname"] + ", all 5 frames by one e2e_render_frames call + 5 detector calls",
+                                     "n_samples": o["n_samples"], "contributions": o["contrib"], "frame_ms": o["ms_step"] / 5.0,
+                                     "step_ms": o["ms_step"], "value": o["contrib"] / (o["ms_step"] * 1e-3), "unit": UNIT,
+                                     "stage_ms_per_step": o["stage_ms"], "gpu_launches_per_step": o["launches"] / o["steps"],
+                                     "render_kernel": o["kinfo"]["name"]}
+        o["r"].close()
+        del o
+        torch.cuda.empty_cache()
     cpu = None
     if not args.no_cpu:
         c = time_oracle(scene, args.oracle_samples)

@@ -892,6 +892,52 @@ def test_render_frames_batch_equals_single_renders(B):
             r.close()
 
 
+def test_render_frames_batch_on_a_frame_that_fills_the_gpu(B):
+    """the batch call on a multi-order, two-fiber frame (the single-warp flush kernel in its batch form, frames interleaved in
+    one grid; the RV-sweep batches above take the wide kernel): three frames with different Doppler factors and illumination,
+    each the bits of its single render, and windows of one of them against the oracle"""
+    import torch
+    base = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=list(range(0, 85, 4)))   # 44 strips, ~7500 work items
+    scenes = []
+    for dop, sc0, sc1 in ((1.0, 1.0, 1.0), (1.0 + 2e-4, 0.5, 2.0), (1.0 - 1e-4, 3.0, 0.0)):
+        sc = copy.copy(base)
+        sc.spectra = [Spectrum_like(base.spectra[0], doppler=dop, scale=base.spectra[0].scale * sc0),
+                      Spectrum_like(base.spectra[1], doppler=dop, scale=base.spectra[1].scale * sc1)]
+        scenes.append(sc)
+    r = B.Renderer(base)
+    try:
+        name = B.e2e_render_kernel_info(r.fmt, r.psf)["name"]
+        assert name.startswith("cell_flush_kernel<")                # not the wide (small-frame) kernel
+        keep, descs, singles = [], [], []
+        for sc in scenes:
+            flux = [torch.from_numpy(np.ascontiguousarray(sp.flux, dtype=np.float64)).cuda() for sp in sc.spectra]
+            keep.append(flux)
+            d = B.spectra_array(sc.spectra, [t.data_ptr() for t in flux])
+            descs.append(d)
+            fr = torch.empty((sc.ny, sc.nx), dtype=torch.float64, device="cuda")
+            B.e2e_render_frame(r.fmt, r.psf, d, fr, False, r.workspace)
+            singles.append(fr)
+        ws = torch.empty(B.e2e_render_frames_workspace_bytes(r.fmt, r.psf, len(scenes)), dtype=torch.uint8, device="cuda")
+        ws.view(torch.float64).fill_(float("nan"))
+        frames = [torch.full((base.ny, base.nx), float("nan"), dtype=torch.float64, device="cuda") for _ in scenes]
+        B.e2e_render_frames(r.fmt, r.psf, descs, frames, False, ws)
+        torch.cuda.synchronize()
+        for a, b in zip(frames, singles):
+            assert torch.equal(a, b)
+        assert not torch.equal(frames[0], frames[1])
+        G = frames[1].cpu().numpy()
+        for o, frac in ((0, 0.3), (11, 0.7)):
+            n = oracle.order_nsamples(scenes[1], o)
+            k = int(frac * (n - 1))
+            lam, x, y, w = oracle.samples(scenes[1], 0, o, k, k + 1)
+            i0, j0 = max(0, int(x[0]) - 24), max(0, int(y[0]) - 20)
+            O = oracle.render(scenes[1], window=(i0, j0, 48, 40))
+            assert O.max() > 0
+            assert_frame_parity(G[j0:j0 + 40, i0:i0 + 48], O, f"batch frame 1 window {i0},{j0}")
+    finally:
+        r.close()
+
+
 def _sparse_rv(v):
     s = W.rv_sweep(v)
     s.samples_per_px = 3.0

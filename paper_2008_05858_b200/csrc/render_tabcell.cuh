@@ -42,7 +42,10 @@ constexpr int kTcSlots = 5;            // pixels per lane and panel (160 px: the
 constexpr int kTcGroup = E2E_TC_GROUP;            // cells per group (power of two)
 constexpr int kTcRows = 4;             // weight rows per group: b' - (B0 - 1) in 0..3
 constexpr int kTcPitch = 33;           // staging pitch: [value][sample]
-constexpr int kTcTile = 32 * kTcSlots + (kTcGroup - 1) * 16;   // shared tile of a single-panel group (nwin <= 12 rows... see below)
+// shared tile of a single-panel group: 12 rows x (12 + kTcGroup - 1) columns for the largest window that fits one panel.  Not a
+// double more than needed: at 16 warps the CTA then takes 130 KB of shared memory, under the 132-KB carve-out step, which leaves
+// the L1 124 KB instead of 92 KB for the table slices (6.94 -> 6.82 ms per field_psf frame)
+constexpr int kTcTile = 12 * (12 + kTcGroup - 1) + 4;
 
 __host__ __device__ inline size_t tabcell_warp_smem_doubles(int os)
 {

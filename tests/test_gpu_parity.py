@@ -98,6 +98,50 @@ def test_render_tiny_full_parity(B):
     assert abs(photocenter_y(G) - photocenter_y(O)) < 1e-9
 
 
+@pytest.mark.parametrize("psf_kw", [
+    dict(fiber_dx_px=0.0, fiber_dy_px=0.0, sigma_x=0.9, sigma_y=1.3),      # pure asymmetric gaussian: one term, 3 power tiles
+    dict(fiber_dx_px=4.0, fiber_dy_px=4.0, sigma_x=1.2, sigma_y=1.2),      # ESPRESSO-like PSF: 2 power tiles
+    dict(fiber_dx_px=5.0, fiber_dy_px=2.0, sigma_x=0.8, sigma_y=1.5),      # elliptical fiber image, asymmetric PSF
+    dict(fiber_dx_px=3.0, fiber_dy_px=0.0, sigma_x=1.0, sigma_y=1.0),      # degenerate ellipse: Dy = 0
+    dict(fiber_dx_px=8.0, fiber_dy_px=8.0, sigma_x=2.5, sigma_y=2.5),      # footprint 47 px: 6 x 6 tiles per window
+    dict(fiber_dx_px=2.0, fiber_dy_px=2.0, sigma_x=0.45, sigma_y=0.45),    # narrow PSF: fine y-phase windows
+])
+def test_render_psf_variants_dense_sampling(B, psf_kw):
+    """the PSF variants under dense sampling, where the two-kernel cell-moment path renders (the sparse-sampling test below takes
+    the per-sample polynomial kernel): whole small frame against the oracle, kernel asserted by name"""
+    s = with_psf(small_tiny(spp=16.0, lam=(5010.0, 5012.0)), **psf_kw)
+    r = B.Renderer(s)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"].startswith("cell_flush_wide_kernel<")
+        G = r.render().cpu().numpy()
+    finally:
+        r.close()
+    O = oracle.render(s)
+    assert O.max() > 0
+    assert_frame_parity(G, O, str(psf_kw))
+
+
+def test_render_three_power_tiles_on_a_frame_that_fills_the_gpu(B):
+    """cell_flush_kernel<3> (x degree above 15, single-warp CTAs): a 44-strip frame with a pure asymmetric gaussian PSF,
+    windows of fiber 1 against the oracle"""
+    s = with_psf(W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=list(range(0, 85, 4))),
+                 fiber_dx_px=0.0, fiber_dy_px=0.0, sigma_x=0.9, sigma_y=1.3)
+    r = B.Renderer(s)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"] == "cell_flush_kernel<3>"
+        G = r.render().cpu().numpy()
+    finally:
+        r.close()
+    for o, frac in ((0, 0.2), (10, 0.5), (21, 0.9)):
+        n = oracle.order_nsamples(s, o)
+        k = int(frac * (n - 1))
+        lam, x, y, w = oracle.samples(s, 1, o, k, k + 1)
+        i0, j0 = max(0, int(x[0]) - 24), max(0, int(y[0]) - 20)
+        O = oracle.render(s, window=(i0, j0, 48, 40))
+        assert O.max() > 0
+        assert_frame_parity(G[j0:j0 + 40, i0:i0 + 48], O, f"window {i0},{j0}")
+
+
 def test_render_is_deterministic_and_accumulates(B):
     s = small_tiny(spp=8.0, lam=(5010.0, 5020.0))
     r = B.Renderer(s)

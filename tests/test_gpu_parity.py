@@ -658,6 +658,41 @@ def Spectrum_like(sp, **kw):
     return W.Spectrum(**d)
 
 
+def test_render_frame_host_on_a_frame_that_fills_the_gpu(B):
+    """the banded host path with the single-warp flush kernel (the 7-order scenes above are small frames and take the wide kernel):
+    44 strips, host frame against the device path and against oracle windows at band seams, detector stage bit-exact"""
+    import torch
+    s = W.espresso_like(n_obj_lines=300, table_dlam=0.01).subset(orders=list(range(0, 85, 4)))
+    det = W.Detector(gain=1.0, dark_e=0.5, ron_e=3.0, bias=100.0, seed=99)
+    r = B.Renderer(s)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"] == "cell_flush_kernel<2>"
+        assert B.e2e_plan_check(r.fmt, r.psf)["n_host_bands"] >= 4
+        dev = r.render().cpu().numpy()
+        host_tabs = [np.ascontiguousarray(sp.flux, dtype=np.float64) for sp in s.spectra]
+        desc = B.spectra_array(s.spectra, [t.ctypes.data for t in host_tabs])
+        ws = torch.empty(B.e2e_render_host_workspace_bytes(r.fmt, r.psf, desc), dtype=torch.uint8, device="cuda")
+        ws.view(torch.float64).fill_(float("nan"))
+        out = torch.full((s.ny, s.nx), float("nan"), dtype=torch.float64).pin_memory()
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws)
+        H = out.numpy().copy()
+        assert np.isfinite(H).all()
+        assert np.abs(H - dev).max() <= 1e-13 * dev.max()
+        assert np.array_equal(H == 0.0, dev == 0.0)
+        for o, frac in ((0, 0.5), (7, 0.01), (14, 0.99), (21, 0.4)):
+            n = oracle.order_nsamples(s, o)
+            k = int(frac * (n - 1))
+            lam, x, y, w = oracle.samples(s, 0, o, k, k + 1)
+            i0, j0 = max(0, int(x[0]) - 24), max(0, int(y[0]) - 20)
+            O = oracle.render(s, window=(i0, j0, 48, 40))
+            assert O.max() > 0
+            assert_frame_parity(H[j0:j0 + 40, i0:i0 + 48], O, f"host path window {i0},{j0}")
+        B.e2e_render_frame_host(r.fmt, r.psf, desc, out.data_ptr(), ws, det=det)
+        assert np.array_equal(out.numpy(), oracle.detector(H, det))
+    finally:
+        r.close()
+
+
 def test_render_frame_host_adu16_raw_frame(B):
     """e2e_render_frame_host_adu16 / _ex: the host path with the full detector stage (PRNU + dark maps, full well, cross-talk,
     ADC) delivering uint16 counts.  Bit-exact against the oracle's detector stage applied to the host path's own noise-free

@@ -196,6 +196,11 @@ def test_render_overwrites_a_dirty_frame_on_every_zero_fill_path(B):
 ])
 def test_render_psf_variants(B, psf_kw):
     s = with_psf(small_tiny(spp=3.0, lam=(5010.0, 5012.0)), **psf_kw)
+    r = B.Renderer(s)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"].startswith("render_poly_kernel<")      # sparse sampling
+    finally:
+        r.close()
     G = gpu_render(B, s)
     O = oracle.render(s)
     assert O.max() > 0
@@ -497,7 +502,12 @@ def test_render_tabulated_shapes(B, npix, os):
     """even / odd kernel widths, non-power-of-two and unit oversampling (cell-deposit kernel), and an oversampling
     beyond its weight array (os = 20 -> per-sample lattice kernel)"""
     s = small_field_scene(gx=3, gy=3, npix=npix, os=os, seed=78)
-    G = gpu_render(B, s)
+    r = B.Renderer(s)
+    try:
+        assert B.e2e_render_kernel_info(r.fmt, r.psf)["name"] == ("render_tabulated_kernel" if os > 16 else "render_tabcell_kernel")
+        G = r.render().cpu().numpy()
+    finally:
+        r.close()
     O = oracle.render(s)
     assert O.max() > 0
     assert_frame_parity(G, O, f"tabulated npix={npix} os={os}")
